@@ -1,0 +1,140 @@
+/*
+ * include/fdtd.h -- C ABI of libfdtd_b200: the 3-D FDTD Yee update of arXiv 2502.20610 on one B200.
+ *
+ * The library advances Maxwell's curl equations on a Yee grid with the leapfrog update of the paper's
+ * eq. (1) (section 2: "E_x += dt/dy (H_z[i,j,k]-H_z[i,j-1,k]) - dt/dz (H_y[i,j,k]-H_y[i,j,k-1])"),
+ * the five sibling updates "in the vein of" it, and per-cell structural fields
+ * ("permittivity and conductivity", section 4) expressed as update coefficients:
+ *
+ *     E_a <- ca_a * E_a + cb_a * [ (H_c - H_c[-e_b]) / d_b - (H_b - H_b[-e_c]) / d_c ]      (a,b,c) cyclic
+ *     H_a <- H_a  - db_a * [ (E_c[+e_b] - E_c) / d_b - (E_b[+e_c] - E_b) / d_c ]
+ *
+ * One step = E half-step over the whole grid, soft source, H half-step over the whole grid (Fig. 7 caption,
+ * "all the E-field nodes ... after which all the H-field nodes").  Two schedules compute it:
+ *   FDTD_KERNEL_NAIVE     one HBM-bound kernel per half-step (the paper's "very straightforward" baseline,
+ *                         PAPER.md:54-57, section 2);
+ *   FDTD_KERNEL_SYSTOLIC  the paper's systolic scheme (sections 3-4): persistent CTAs keep a
+ *                         subdomain on chip, slide it along the x-y-z-t diagonal, exchange only faces through
+ *                         global memory and hand off with per-tile flags.  It performs "the exact same update
+ *                         equations", so results are identical per cell to the naive schedule.
+ *
+ * Layout contract.  Every field / coefficient component is ONE contiguous fp32 array of nx*ny*nz elements,
+ * x fastest:  idx = i + nx*(j + ny*k).  Yee positions: E_x(i+1/2,j,k) E_y(i,j+1/2,k) E_z(i,j,k+1/2)
+ * H_x(i,j+1/2,k+1/2) H_y(i+1/2,j,k+1/2) H_z(i+1/2,j+1/2,k)  (fixed by eq. (1)'s index pattern).
+ * Device pointers must be 16-byte aligned.
+ *
+ * Time contract.  At entry E holds E^n and H holds H^{n+1/2}; fdtd_step(ctx, n) leaves E^{n0+n}, H^{n0+n+1/2}.
+ *
+ * Walls (the paper is silent; reading #5).  FDTD_PEC on an axis: tangential E stored at index 0 of
+ * that axis is never updated (keeps what the caller put there), tangential E one past the last index is a
+ * ghost equal to 0.  FDTD_PERIODIC: indices wrap, every cell is updated.
+ *
+ * Errors.  Every function except fdtd_destroy / fdtd_last_error returns an FDTD_* status; no exception crosses
+ * the ABI.  The Courant limit is NOT enforced.  There is no CPU fallback: without a CUDA device fdtd_create
+ * returns FDTD_ECUDA.
+ *
+ * Thread safety: one ctx per host thread at a time.
+ */
+#ifndef FDTD_B200_H
+#define FDTD_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdtd_ctx fdtd_ctx; /* opaque; owned by the library */
+
+enum { FDTD_PEC = 0, FDTD_PERIODIC = 1 };
+enum { FDTD_OK = 0, FDTD_EINVAL = 1, FDTD_ENOMEM = 2, FDTD_ECUDA = 3, FDTD_ESTATE = 4, FDTD_ETIMEOUT = 5 };
+enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1 };
+
+/* Create a context for an nx*ny*nz grid with cell sizes dx,dy,dz (> 0, finite), time step dt (> 0, finite)
+ * and per-axis wall type boundary[3] (host array of FDTD_PEC | FDTD_PERIODIC).
+ * cuda_stream: a cudaStream_t (as void*) on which all work is enqueued; NULL = the legacy default stream.
+ * The default kernel is FDTD_KERNEL_SYSTOLIC with library-chosen tile shape and temporal depth.
+ * *out is written only on FDTD_OK.  FDTD_EINVAL: bad dims (each 1..2^15, product < 2^40), spacings, dt, boundary.
+ * FDTD_ECUDA: no usable sm_100 device / CUDA failure.   (problem statement: PAPER.md:35-37) */
+int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, float dt,
+                const int boundary[3], void* cuda_stream);
+
+/* Bind the six field arrays: E[3] = {Ex,Ey,Ez}, H[3] = {Hx,Hy,Hz}; host arrays of DEVICE pointers.
+ * The buffers are BORROWED (config 5 is 81 GiB: no copy is affordable) and updated in place by fdtd_step;
+ * they must stay valid until rebinding or fdtd_destroy, and must not alias each other.
+ * FDTD_EINVAL: NULL or misaligned pointer.   (the six arrays of eq. (1) and its siblings) */
+int fdtd_set_fields(fdtd_ctx* ctx, float* const E[3], float* const H[3]);
+
+/* Copy initial data from six caller arrays (HOST or device pointers, same layout) into the bound field
+ * buffers, asynchronously on the ctx stream.  NULL entries are skipped.  This is the host-buffer entry of
+ * the end-to-end path (bench.py `e2e`).  FDTD_ESTATE before fdtd_set_fields. */
+int fdtd_load_fields(fdtd_ctx* ctx, const float* const E[3], const float* const H[3]);
+
+/* Bind update coefficients ("structural fields"; reading #2).
+ * ca[3], cb[3]: host arrays of DEVICE pointers to per-cell, per-component fp32 arrays (borrowed, read-only),
+ *   ca == NULL -> ca_a = 1 everywhere (the multiply is skipped, which is exact);
+ *   cb == NULL -> cb_a = dt everywhere (eq. (1)'s vacuum form with 1/d applied inside the curl).
+ *   If ca / cb is non-NULL all three entries must be non-NULL.
+ * db[3]: HOST array of three scalars (non-magnetic media); NULL -> {dt, dt, dt}.
+ * Generator side (not the library's business): ca=(2eps-sigma dt)/(2eps+sigma dt), cb=2dt/(2eps+sigma dt). */
+int fdtd_set_coeffs(fdtd_ctx* ctx, const float* const ca[3], const float* const cb[3], const float db[3]);
+
+/* Additive soft source on one E component over a box (excluded from the paper's own benchmark, PAPER.md:106;
+ * DESIGN.md reading #6): after the E half-step of step t,  E_comp[box] += amp[q] * wave[t]  while 0 <= t < nwave
+ * (product rounded to fp32, then the add).  comp 0..2 = Ex,Ey,Ez; box origin (i0,j0,k0), extent (ni,nj,nk);
+ * amp: HOST array ni*nj*nk, x fastest; wave: HOST array nwave.  Both are copied (caller may free them).
+ * amp == NULL removes the source.  FDTD_EINVAL: box outside the grid, comp out of range, nwave < 1. */
+int fdtd_set_source(fdtd_ctx* ctx, int comp, int i0, int j0, int k0, int ni, int nj, int nk,
+                    const float* amp, const float* wave, int nwave);
+
+/* Advance n >= 0 steps; enqueues on the ctx stream and returns without synchronising; ctx time += n.
+ * FDTD_ESTATE before fdtd_set_fields.  A device-side failure (hand-off watchdog) is reported by the next
+ * fdtd_get_fields / fdtd_sync as FDTD_ETIMEOUT.   (eq. (1); sections 3-4 for the schedule) */
+int fdtd_step(fdtd_ctx* ctx, int n);
+
+/* Synchronise the ctx stream, then copy the fields out to E[3], H[3] (HOST or device pointers; a NULL array or
+ * NULL entry, or an entry equal to the bound pointer, is skipped -- fdtd_get_fields(ctx, NULL, NULL) = sync only).
+ * Returns FDTD_ETIMEOUT / FDTD_ECUDA if the enqueued work failed. */
+int fdtd_get_fields(fdtd_ctx* ctx, float* const E[3], float* const H[3]);
+int fdtd_sync(fdtd_ctx* ctx);
+
+/* Step counter used to index wave[] (resume after a checkpoint: state = six arrays + t). */
+int fdtd_set_time(fdtd_ctx* ctx, long long t);
+long long fdtd_get_time(const fdtd_ctx* ctx);
+
+/* Choose the schedule.  which = FDTD_KERNEL_NAIVE | FDTD_KERNEL_SYSTOLIC.
+ * For the systolic kernel (Nx,Ny,Nz) is the updated tile ("subdomain": 31x15x15 updated inside a
+ * 32x16x16 cached block) and T the temporal depth (steps a tile stays resident per launch); 0 = library default.
+ * FDTD_EINVAL if the shape is not one the kernel was built for or the grid cannot run it (see fdtd_last_error). */
+int fdtd_set_kernel(fdtd_ctx* ctx, int which, int Nx, int Ny, int Nz, int T);
+
+/* What fdtd_step will run: out[0]=which, out[1..3]=tile Nx,Ny,Nz, out[4]=T, out[5]=tiles per launch,
+ * out[6]=CTAs per launch, out[7]=dynamic shared memory bytes per CTA. */
+int fdtd_get_kernel(const fdtd_ctx* ctx, int out[8]);
+
+/* Counters since creation: out[0] = kernels launched by fdtd_step, out[1] = steps advanced,
+ * out[2] = systolic chunks launched, out[3] = tiles processed. */
+int fdtd_get_counters(const fdtd_ctx* ctx, long long out[4]);
+
+/* GPU time of the most recent fdtd_step call in milliseconds (CUDA events recorded on the ctx stream around
+ * the enqueued kernels).  Synchronises on the closing event. */
+int fdtd_last_step_ms(fdtd_ctx* ctx, float* ms);
+
+/* Pure host function (no device needed): the tile schedule the systolic kernel would use for this grid.
+ * ntiles[3] = tiles per axis for a launch of T steps with tile (Nx,Ny,Nz): ceil((n+T)/N) on a PEC axis
+ * (tiles enter empty at the high wall and drain at the low wall), ceil(n/N) on a periodic axis (a ring).
+ * Returns FDTD_EINVAL for non-positive arguments. */
+int fdtd_plan_tiles(const int n[3], const int boundary[3], const int N[3], int T, int ntiles[3]);
+
+/* Pure host function: which tile updates cell coordinate g (0 <= g < n) of one axis at step s of a launch
+ * (0 <= s < T) and the cell's offset inside that tile's current region.  start[] are the nb tile starts the
+ * library uses for that axis (uniform b*N on a PEC axis; as even as possible on a ring).
+ * Writes *tile, *offset.  (reading #11: cell g at step s belongs to the tile whose region [a_b - s, a_{b+1} - s) holds it) */
+int fdtd_plan_owner(int n, int boundary, int N, int T, int g, int s, int* tile, int* offset);
+
+const char* fdtd_last_error(const fdtd_ctx* ctx); /* text of the last failure on this ctx; never NULL */
+const char* fdtd_build_info(void);                /* e.g. "sm_100a fmad=true" */
+void fdtd_destroy(fdtd_ctx* ctx);                 /* NULL-safe; never frees borrowed buffers */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDTD_B200_H */

@@ -1,0 +1,222 @@
+"""Thin ctypes binding of libfdtd_b200 (include/fdtd.h): argument marshalling only -- every step of the path
+runs in the library's CUDA kernels.  PyTorch supplies device memory and the stream, nothing else.
+
+There is NO CPU fallback: if the shared library is missing `load()` raises, and on a box without a B200
+`Fdtd(...)` raises FdtdError(FDTD_ECUDA).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+PEC, PERIODIC = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ETIMEOUT = range(6)
+KERNEL_NAIVE, KERNEL_SYSTOLIC = 0, 1
+_ERRNAME = {1: "FDTD_EINVAL", 2: "FDTD_ENOMEM", 3: "FDTD_ECUDA", 4: "FDTD_ESTATE", 5: "FDTD_ETIMEOUT"}
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBFILES = {"fma": "libfdtd_b200.so", "nofma": "libfdtd_b200_nofma.so"}
+_libs = {}
+
+_F3 = C.c_void_p * 3
+_PROTOS = {
+    "fdtd_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float,
+                              C.POINTER(C.c_int), C.c_void_p]),
+    "fdtd_set_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "fdtd_load_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "fdtd_set_coeffs": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_float)]),
+    "fdtd_set_source": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
+                                  C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int]),
+    "fdtd_step": (C.c_int, [C.c_void_p, C.c_int]),
+    "fdtd_get_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "fdtd_sync": (C.c_int, [C.c_void_p]),
+    "fdtd_set_time": (C.c_int, [C.c_void_p, C.c_longlong]),
+    "fdtd_get_time": (C.c_longlong, [C.c_void_p]),
+    "fdtd_set_kernel": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]),
+    "fdtd_get_kernel": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
+    "fdtd_get_counters": (C.c_int, [C.c_void_p, C.POINTER(C.c_longlong)]),
+    "fdtd_last_step_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
+    "fdtd_plan_tiles": (C.c_int, [C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_int)]),
+    "fdtd_plan_owner": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+    "fdtd_last_error": (C.c_char_p, [C.c_void_p]),
+    "fdtd_build_info": (C.c_char_p, []),
+    "fdtd_destroy": (None, [C.c_void_p]),
+}
+EXPORTS = tuple(_PROTOS)
+
+
+class FdtdError(RuntimeError):
+    def __init__(self, code, msg=""):
+        self.code = code
+        super().__init__(f"{_ERRNAME.get(code, code)}: {msg}" if msg else str(_ERRNAME.get(code, code)))
+
+
+def lib_path(variant="fma"):
+    return os.path.join(HERE, _LIBFILES[variant])
+
+
+def load(variant="fma"):
+    """dlopen the in-tree library; raises if it has not been built (python -m paper_2502_20610_b200.build)."""
+    if variant not in _libs:
+        path = lib_path(variant)
+        if not os.path.exists(path):
+            raise FileNotFoundError(f"{path} is missing: build it with `python -m paper_2502_20610_b200.build` "
+                                    "(there is no CPU fallback)")
+        lib = C.CDLL(path)
+        for name, (res, args) in _PROTOS.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _libs[variant] = lib
+    return _libs[variant]
+
+
+def _ptr3(tensors):
+    if tensors is None:
+        return None
+    arr = _F3()
+    for a in range(3):
+        t = tensors[a]
+        arr[a] = None if t is None else (t.data_ptr() if hasattr(t, "data_ptr") else t.ctypes.data)
+    return C.cast(arr, C.POINTER(C.c_void_p))
+
+
+def plan_tiles(n, boundary, N, T, variant="fma"):
+    out = (C.c_int * 3)()
+    rc = load(variant).fdtd_plan_tiles((C.c_int * 3)(*n), (C.c_int * 3)(*boundary), (C.c_int * 3)(*N), int(T), out)
+    if rc != OK:
+        raise FdtdError(rc)
+    return tuple(out)
+
+
+def plan_owner(n, boundary, N, T, g, s, variant="fma"):
+    tile, off = C.c_int(), C.c_int()
+    rc = load(variant).fdtd_plan_owner(int(n), int(boundary), int(N), int(T), int(g), int(s), C.byref(tile), C.byref(off))
+    if rc != OK:
+        raise FdtdError(rc)
+    return tile.value, off.value
+
+
+class Fdtd:
+    """One simulation context.  E, H (and ca, cb) are lists of three float32 CUDA tensors of shape (nz, ny, nx),
+    contiguous, which the library borrows and updates in place."""
+
+    def __init__(self, n, d, dt, boundary, stream=None, variant="fma"):
+        import torch
+        self._lib = load(variant)
+        self.variant = variant
+        self.n = tuple(int(x) for x in n)
+        self._h = C.c_void_p()
+        self._keep = []
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+        rc = self._lib.fdtd_create(C.byref(self._h), *self.n, *[float(x) for x in d], float(dt),
+                                   (C.c_int * 3)(*[int(b) for b in boundary]), C.c_void_p(int(stream) or None))
+        if rc != OK:
+            self._h = C.c_void_p()
+            raise FdtdError(rc, "fdtd_create failed (no B200 / bad arguments)")
+
+    def _check(self, rc):
+        if rc != OK:
+            raise FdtdError(rc, self._lib.fdtd_last_error(self._h).decode())
+
+    def _check_tensors(self, ts):
+        import torch
+        shape = (self.n[2], self.n[1], self.n[0])
+        for t in ts:
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shape, "bad field tensor"
+
+    def set_fields(self, E, H):
+        self._check_tensors(list(E) + list(H))
+        self._keep = [list(E), list(H)] + self._keep[2:]
+        self._check(self._lib.fdtd_set_fields(self._h, _ptr3(E), _ptr3(H)))
+
+    def load_fields(self, E, H):
+        """Copy initial data from host (pinned numpy / CPU tensors) or device arrays into the bound buffers."""
+        self._check(self._lib.fdtd_load_fields(self._h, _ptr3(E), _ptr3(H)))
+
+    def set_coeffs(self, ca=None, cb=None, db=None):
+        if ca is not None:
+            self._check_tensors(ca)
+        if cb is not None:
+            self._check_tensors(cb)
+        self._keep.append((ca, cb))
+        dbp = None if db is None else (C.c_float * 3)(*[float(x) for x in db])
+        self._check(self._lib.fdtd_set_coeffs(self._h, _ptr3(ca), _ptr3(cb), dbp))
+
+    def set_source(self, comp, box, amp, wave):
+        import numpy as np
+        if amp is None:
+            self._check(self._lib.fdtd_set_source(self._h, 0, 0, 0, 0, 0, 0, 0, None, None, 0))
+            return
+        amp = np.ascontiguousarray(amp, dtype=np.float32).reshape(-1)
+        wave = np.ascontiguousarray(wave, dtype=np.float32).reshape(-1)
+        fp = C.POINTER(C.c_float)
+        self._check(self._lib.fdtd_set_source(self._h, int(comp), *[int(x) for x in box], amp.ctypes.data_as(fp),
+                                              wave.ctypes.data_as(fp), int(wave.size)))
+
+    def set_kernel(self, which, tile=None, T=0):
+        tx, ty, tz = tile if tile is not None else (0, 0, 0)
+        self._check(self._lib.fdtd_set_kernel(self._h, int(which), int(tx), int(ty), int(tz), int(T)))
+
+    def get_kernel(self):
+        out = (C.c_int * 8)()
+        self._check(self._lib.fdtd_get_kernel(self._h, out))
+        return {"which": out[0], "tile": (out[1], out[2], out[3]), "T": out[4], "tiles": out[5], "ctas": out[6], "smem": out[7]}
+
+    def step(self, n):
+        self._check(self._lib.fdtd_step(self._h, int(n)))
+
+    def sync(self):
+        self._check(self._lib.fdtd_sync(self._h))
+
+    def get_fields(self, E=None, H=None):
+        self._check(self._lib.fdtd_get_fields(self._h, _ptr3(E), _ptr3(H)))
+
+    def set_time(self, t):
+        self._check(self._lib.fdtd_set_time(self._h, int(t)))
+
+    @property
+    def time(self):
+        return int(self._lib.fdtd_get_time(self._h))
+
+    def counters(self):
+        out = (C.c_longlong * 4)()
+        self._check(self._lib.fdtd_get_counters(self._h, out))
+        return {"launches": out[0], "steps": out[1], "chunks": out[2], "tiles": out[3]}
+
+    def last_step_ms(self):
+        ms = C.c_float()
+        self._check(self._lib.fdtd_last_step_ms(self._h, C.byref(ms)))
+        return ms.value
+
+    def close(self):
+        if self._h:
+            self._lib.fdtd_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def run_workload(w, kernel=KERNEL_SYSTOLIC, tile=None, T=0, steps=None, variant="fma", device="cuda:0"):
+    """Build the seeded inputs of workload `w` on the device, run `steps` steps, return (E, H) CUDA tensors and the
+    context (still open).  Convenience used by tests, smoke() and bench.py."""
+    import torch
+    from . import workloads
+    dev = torch.device(device)
+    E, H = workloads.make_fields(w, device=dev)
+    ca, cb = workloads.make_coeffs(w, device=dev)
+    sim = Fdtd(w.n, w.d, w.dt, w.boundary, variant=variant)
+    sim.set_fields(E, H)
+    if ca is not None:
+        sim.set_coeffs(ca, cb, None)
+    src = workloads.make_source(w)
+    if src is not None:
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(kernel, tile, T)
+    sim.step(w.steps if steps is None else steps)
+    sim.sync()
+    return E, H, sim

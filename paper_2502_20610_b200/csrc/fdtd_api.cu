@@ -1,0 +1,577 @@
+// fdtd_api.cu -- the C ABI of include/fdtd.h: context, argument checking, schedule planning and launches.
+// Every step of the hot path runs in the kernels of naive_kernels.cu / systolic_kernel.cu; this file only
+// marshals.  There is no CPU fallback: without a device fdtd_create fails with FDTD_ECUDA.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "fdtd_internal.h"
+
+struct fdtd_ctx {
+    GridParams g;
+    float d[3];
+    float dt;
+    cudaStream_t stream;
+    bool fields_set;
+    float* d_amp;
+    float* d_wave;
+    std::vector<float> h_wave;
+    long long t;
+    // schedule
+    int which;
+    int reqN[3];      // requested tile (0 = default)
+    int reqT;         // requested temporal depth (0 = default)
+    int cfg_idx;      // resolved systolic configuration, -1 = unresolved
+    int T;            // resolved temporal depth
+    int ctas;
+    // systolic state
+    int* d_flags;     // flagE[cap] then flagH[cap]
+    size_t flags_cap;
+    unsigned int* d_counter;
+    int* d_abort;
+    int flag_base;
+    long long spin_budget;
+    unsigned int delay_seed;
+    // device
+    int device, num_sms, clock_khz;
+    cudaEvent_t ev0, ev1;
+    bool ev_valid;
+    long long counters[4];
+    std::string err;
+};
+
+namespace {
+
+int fail(fdtd_ctx* c, int code, const std::string& msg)
+{
+    if (c) c->err = msg;
+    return code;
+}
+
+int cuda_fail(fdtd_ctx* c, cudaError_t e, const char* what)
+{
+    return fail(c, FDTD_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+bool has_coef(const fdtd_ctx* c) { return c->g.ca[0] != nullptr; }
+
+// both-or-neither rule for the systolic kernel (the naive kernel takes any combination)
+bool coef_mixed(const fdtd_ctx* c) { return (c->g.ca[0] != nullptr) != (c->g.cb[0] != nullptr); }
+
+int default_T(const fdtd_ctx* c)
+{
+    // Temporal depth: the launch ramp costs ~ prod(1 + T/n_a) tile slots on PEC axes (a11), the residency
+    // load/store is amortised over T steps (a6).  n/8 clamped to [4, 32] keeps both near 1.4x or better.
+    int m = 1 << 30;
+    for (int a = 0; a < 3; ++a)
+        if (!c->g.per[a] && c->g.n[a] < m) m = c->g.n[a];
+    if (m == (1 << 30)) return 32;
+    int T = m / 8;
+    if (T < 4) T = 4;
+    if (T > 32) T = 32;
+    if (const char* e = getenv("FDTD_T")) {
+        const int v = atoi(e);
+        if (v > 0) T = v;
+    }
+    return T;
+}
+
+int resolve_systolic(fdtd_ctx* c)
+{
+    if (coef_mixed(c)) return fail(c, FDTD_EINVAL, "systolic kernel needs ca and cb both bound or both NULL");
+    const int want_coef = has_coef(c) ? 1 : 0;
+    int N[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};
+    if (N[0] == 0) {
+        if (want_coef) { N[0] = 31; N[1] = 15; N[2] = 7; }
+        else           { N[0] = 31; N[1] = 15; N[2] = 15; }
+        if (const char* e = getenv("FDTD_TILE")) {
+            int x, y, z;
+            if (sscanf(e, "%dx%dx%d", &x, &y, &z) == 3) { N[0] = x; N[1] = y; N[2] = z; }
+        }
+    }
+    int found = -1;
+    for (int i = 0; i < systolic_num_configs(); ++i) {
+        const SysConfig* s = systolic_config(i);
+        if (s->Bx - 1 == N[0] && s->By - 1 == N[1] && s->Bz - 1 == N[2] && s->coef == want_coef) { found = i; break; }
+    }
+    if (found < 0) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "no systolic kernel built for tile %dx%dx%d %s coefficient arrays", N[0], N[1], N[2],
+                 want_coef ? "with" : "without");
+        return fail(c, FDTD_EINVAL, buf);
+    }
+    cudaError_t e = systolic_prepare(found);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+    const SysConfig* s = systolic_config(found);
+    // persistent grid: every CTA resident at once (one per SM for the 192 KB boxes)
+    int per_sm = (int)((227u * 1024u) / (s->smem + 1024u));
+    if (per_sm < 1) per_sm = 1;
+    int by_threads = 2048 / s->threads;
+    if (per_sm > by_threads) per_sm = by_threads;
+    if (per_sm > 4) per_sm = 4;
+    c->ctas = c->num_sms * per_sm;
+    c->T = c->reqT > 0 ? c->reqT : default_T(c);
+    // a ring of tiles along a periodic axis advances in lock step: all of it (and everything the claim order
+    // interleaves with it) must be resident at once (SURVEY.md section 7 hard part 2)
+    int span = 1, ring = 1;
+    for (int a = 0; a < 3; ++a) {
+        const AxisPlan ap = make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T);
+        span *= ap.nb;
+        if (c->g.per[a]) ring = span;
+    }
+    if (ring > c->ctas) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "periodic ring of %d tiles exceeds the %d resident CTAs; use a larger tile or the naive kernel", ring, c->ctas);
+        return fail(c, FDTD_EINVAL, buf);
+    }
+    c->cfg_idx = found;
+    return FDTD_OK;
+}
+
+int ensure_flags(fdtd_ctx* c, size_t ntiles)
+{
+    if (ntiles <= c->flags_cap) return FDTD_OK;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    if (c->d_flags) cudaFree(c->d_flags);
+    c->d_flags = nullptr;
+    c->flags_cap = 0;
+    e = cudaMalloc(&c->d_flags, 2 * ntiles * sizeof(int));
+    if (e != cudaSuccess) return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(flags): ") + cudaGetErrorString(e));
+    e = cudaMemsetAsync(c->d_flags, 0, 2 * ntiles * sizeof(int), c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(flags)");
+    c->flags_cap = ntiles;
+    c->flag_base = 0;
+    return FDTD_OK;
+}
+
+int step_naive(fdtd_ctx* c, int n)
+{
+    for (int s = 0; s < n; ++s) {
+        cudaError_t e = launch_e_half_naive(c->g, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "E half-step launch");
+        c->counters[0]++;
+        if (c->g.src_comp >= 0 && c->t >= 0 && c->t < c->g.src_nwave) {
+            e = launch_source_w(c->g, c->h_wave[(size_t)c->t], c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "source launch");
+            c->counters[0]++;
+        }
+        e = launch_h_half_naive(c->g, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "H half-step launch");
+        c->counters[0]++;
+        c->t++;
+        c->counters[1]++;
+    }
+    return FDTD_OK;
+}
+
+int step_systolic(fdtd_ctx* c, int n)
+{
+    if (c->cfg_idx < 0) {
+        const int rc = resolve_systolic(c);
+        if (rc != FDTD_OK) return rc;
+    }
+    const SysConfig* s = systolic_config(c->cfg_idx);
+    const int N[3] = {s->Bx - 1, s->By - 1, s->Bz - 1};
+    int left = n;
+    while (left > 0) {
+        const int T = left < c->T ? left : c->T;
+        SysParams P;
+        memset(&P, 0, sizeof P);
+        P.g = c->g;
+        long long ntiles = 1;
+        for (int a = 0; a < 3; ++a) {
+            P.ax[a] = make_axis_plan(c->g.n[a], c->g.per[a], N[a], T);
+            ntiles *= P.ax[a].nb;
+        }
+        if (ntiles >= (1ll << 30)) return fail(c, FDTD_EINVAL, "too many tiles for one launch");
+        const int rc = ensure_flags(c, (size_t)ntiles);
+        if (rc != FDTD_OK) return rc;
+        if (c->flag_base > (1 << 30)) {   // monotone epochs: rewind long before int overflow
+            cudaError_t e = cudaMemsetAsync(c->d_flags, 0, 2 * c->flags_cap * sizeof(int), c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(flags)");
+            c->flag_base = 0;
+        }
+        P.T = T;
+        P.t0 = c->t;
+        P.flag_base = c->flag_base;
+        P.ntiles = (int)ntiles;
+        P.flagE = c->d_flags;
+        P.flagH = c->d_flags + c->flags_cap;
+        P.counter = c->d_counter;
+        P.abort_flag = c->d_abort;
+        P.spin_budget = c->spin_budget;
+        P.delay_seed = c->delay_seed;
+        cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
+        const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
+        e = launch_systolic(c->cfg_idx, P, ctas, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "systolic launch");
+        c->flag_base += T + 2;
+        c->t += T;
+        left -= T;
+        c->counters[0]++;
+        c->counters[1] += T;
+        c->counters[2]++;
+        c->counters[3] += ntiles;
+    }
+    return FDTD_OK;
+}
+
+int check_async(fdtd_ctx* c)
+{
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    int flag = 0;
+    e = cudaMemcpy(&flag, c->d_abort, sizeof(int), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(abort flag)");
+    if (flag != 0) {
+        cudaMemset(c->d_abort, 0, sizeof(int));
+        return fail(c, FDTD_ETIMEOUT, "systolic hand-off watchdog fired: a tile waited longer than the spin budget; fields are invalid");
+    }
+    return FDTD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, float dt, const int boundary[3],
+                void* cuda_stream)
+{
+    if (!out || !boundary) return FDTD_EINVAL;
+    const int n[3] = {nx, ny, nz};
+    const float d[3] = {dx, dy, dz};
+    for (int a = 0; a < 3; ++a) {
+        if (n[a] < 1 || n[a] > (1 << 15)) return FDTD_EINVAL;
+        if (!(d[a] > 0.0f) || !isfinite(d[a])) return FDTD_EINVAL;
+        if (boundary[a] != FDTD_PEC && boundary[a] != FDTD_PERIODIC) return FDTD_EINVAL;
+    }
+    if (!(dt > 0.0f) || !isfinite(dt)) return FDTD_EINVAL;
+    if ((long long)nx * ny * nz >= (1ll << 40)) return FDTD_EINVAL;
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return FDTD_ECUDA;
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) return FDTD_ECUDA;
+    if (prop.major != 10) return FDTD_ECUDA;   // built for sm_100a only
+
+    fdtd_ctx* c = new fdtd_ctx();
+    memset(&c->g, 0, sizeof c->g);
+    for (int a = 0; a < 3; ++a) {
+        c->g.n[a] = n[a];
+        c->g.per[a] = boundary[a] == FDTD_PERIODIC;
+        c->g.rd[a] = (float)(1.0 / (double)d[a]);
+        c->g.db[a] = dt;
+        c->d[a] = d[a];
+        c->reqN[a] = 0;
+    }
+    c->g.cb_scalar = dt;
+    c->g.src_comp = -1;
+    c->dt = dt;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->fields_set = false;
+    c->d_amp = c->d_wave = nullptr;
+    c->t = 0;
+    c->which = FDTD_KERNEL_SYSTOLIC;
+    c->reqT = 0;
+    c->cfg_idx = -1;
+    c->T = 0;
+    c->ctas = 0;
+    c->d_flags = nullptr;
+    c->flags_cap = 0;
+    c->d_counter = nullptr;
+    c->d_abort = nullptr;
+    c->flag_base = 0;
+    c->delay_seed = 0;
+    c->device = dev;
+    c->num_sms = prop.multiProcessorCount;
+    c->clock_khz = prop.clockRate;
+    double budget_ms = 10000.0;
+    if (const char* env = getenv("FDTD_SPIN_BUDGET_MS")) budget_ms = atof(env);
+    c->spin_budget = (long long)(budget_ms * (double)(prop.clockRate > 0 ? prop.clockRate : 1965000));
+    if (const char* env = getenv("FDTD_DEBUG_DELAY")) c->delay_seed = (unsigned int)strtoul(env, nullptr, 10);
+    c->ev_valid = false;
+    memset(c->counters, 0, sizeof c->counters);
+    e = cudaMalloc(&c->d_counter, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_abort, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(c->d_abort, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
+    if (e != cudaSuccess) {
+        fdtd_destroy(c);
+        return FDTD_ECUDA;
+    }
+    *out = c;
+    return FDTD_OK;
+}
+
+int fdtd_set_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
+{
+    if (!c) return FDTD_EINVAL;
+    if (!E || !H) return fail(c, FDTD_EINVAL, "fdtd_set_fields: NULL array");
+    for (int a = 0; a < 3; ++a) {
+        if (!E[a] || !H[a]) return fail(c, FDTD_EINVAL, "fdtd_set_fields: NULL field pointer");
+        if (!aligned16(E[a]) || !aligned16(H[a])) return fail(c, FDTD_EINVAL, "fdtd_set_fields: pointers must be 16-byte aligned");
+    }
+    for (int a = 0; a < 3; ++a) {
+        c->g.E[a] = E[a];
+        c->g.H[a] = H[a];
+    }
+    c->fields_set = true;
+    return FDTD_OK;
+}
+
+int fdtd_load_fields(fdtd_ctx* c, const float* const E[3], const float* const H[3])
+{
+    if (!c) return FDTD_EINVAL;
+    if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_load_fields before fdtd_set_fields");
+    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * sizeof(float);
+    for (int a = 0; a < 3; ++a) {
+        if (E && E[a] && E[a] != c->g.E[a]) {
+            cudaError_t e = cudaMemcpyAsync(c->g.E[a], E[a], bytes, cudaMemcpyDefault, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(E in)");
+        }
+        if (H && H[a] && H[a] != c->g.H[a]) {
+            cudaError_t e = cudaMemcpyAsync(c->g.H[a], H[a], bytes, cudaMemcpyDefault, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(H in)");
+        }
+    }
+    return FDTD_OK;
+}
+
+int fdtd_set_coeffs(fdtd_ctx* c, const float* const ca[3], const float* const cb[3], const float db[3])
+{
+    if (!c) return FDTD_EINVAL;
+    for (int a = 0; a < 3; ++a) {
+        if (ca && (!ca[a] || !aligned16(ca[a]))) return fail(c, FDTD_EINVAL, "fdtd_set_coeffs: ca needs three aligned device pointers");
+        if (cb && (!cb[a] || !aligned16(cb[a]))) return fail(c, FDTD_EINVAL, "fdtd_set_coeffs: cb needs three aligned device pointers");
+        if (db && !isfinite(db[a])) return fail(c, FDTD_EINVAL, "fdtd_set_coeffs: db not finite");
+    }
+    for (int a = 0; a < 3; ++a) {
+        c->g.ca[a] = ca ? ca[a] : nullptr;
+        c->g.cb[a] = cb ? cb[a] : nullptr;
+        c->g.db[a] = db ? db[a] : c->dt;
+    }
+    c->cfg_idx = -1;   // the coefficient-carrying kernels are separate instantiations
+    return FDTD_OK;
+}
+
+int fdtd_set_source(fdtd_ctx* c, int comp, int i0, int j0, int k0, int ni, int nj, int nk, const float* amp,
+                    const float* wave, int nwave)
+{
+    if (!c) return FDTD_EINVAL;
+    cudaError_t e = cudaStreamSynchronize(c->stream);   // the old tables may still be in use
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    if (c->d_amp) cudaFree(c->d_amp);
+    if (c->d_wave) cudaFree(c->d_wave);
+    c->d_amp = c->d_wave = nullptr;
+    c->g.src_comp = -1;
+    c->g.src_amp = c->g.src_wave = nullptr;
+    c->g.src_nwave = 0;
+    c->h_wave.clear();
+    if (!amp) return FDTD_OK;
+    const int o[3] = {i0, j0, k0}, m[3] = {ni, nj, nk};
+    if (comp < 0 || comp > 2 || !wave || nwave < 1) return fail(c, FDTD_EINVAL, "fdtd_set_source: bad component, wave or nwave");
+    for (int a = 0; a < 3; ++a)
+        if (o[a] < 0 || m[a] < 1 || o[a] + m[a] > c->g.n[a]) return fail(c, FDTD_EINVAL, "fdtd_set_source: box outside the grid");
+    const size_t na = (size_t)ni * nj * nk;
+    e = cudaMalloc(&c->d_amp, na * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_wave, (size_t)nwave * sizeof(float));
+    if (e != cudaSuccess) return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(source): ") + cudaGetErrorString(e));
+    e = cudaMemcpy(c->d_amp, amp, na * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_wave, wave, (size_t)nwave * sizeof(float), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(source)");
+    c->h_wave.assign(wave, wave + nwave);
+    c->g.src_comp = comp;
+    for (int a = 0; a < 3; ++a) {
+        c->g.src_box[a] = o[a];
+        c->g.src_box[3 + a] = m[a];
+    }
+    c->g.src_amp = c->d_amp;
+    c->g.src_wave = c->d_wave;
+    c->g.src_nwave = nwave;
+    return FDTD_OK;
+}
+
+int fdtd_step(fdtd_ctx* c, int n)
+{
+    if (!c) return FDTD_EINVAL;
+    if (n < 0) return fail(c, FDTD_EINVAL, "fdtd_step: n < 0");
+    if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_step before fdtd_set_fields");
+    cudaError_t e = cudaEventRecord(c->ev0, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
+    const int rc = (c->which == FDTD_KERNEL_NAIVE) ? step_naive(c, n) : step_systolic(c, n);
+    e = cudaEventRecord(c->ev1, c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
+    c->ev_valid = true;
+    return rc;
+}
+
+int fdtd_sync(fdtd_ctx* c)
+{
+    if (!c) return FDTD_EINVAL;
+    return check_async(c);
+}
+
+int fdtd_get_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
+{
+    if (!c) return FDTD_EINVAL;
+    const int rc = check_async(c);
+    if (rc != FDTD_OK) return rc;
+    if (!E && !H) return FDTD_OK;
+    if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_get_fields before fdtd_set_fields");
+    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * sizeof(float);
+    for (int a = 0; a < 3; ++a) {
+        if (E && E[a] && E[a] != c->g.E[a]) {
+            cudaError_t e = cudaMemcpyAsync(E[a], c->g.E[a], bytes, cudaMemcpyDefault, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(E out)");
+        }
+        if (H && H[a] && H[a] != c->g.H[a]) {
+            cudaError_t e = cudaMemcpyAsync(H[a], c->g.H[a], bytes, cudaMemcpyDefault, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpyAsync(H out)");
+        }
+    }
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    return FDTD_OK;
+}
+
+int fdtd_set_time(fdtd_ctx* c, long long t)
+{
+    if (!c) return FDTD_EINVAL;
+    c->t = t;
+    return FDTD_OK;
+}
+
+long long fdtd_get_time(const fdtd_ctx* c) { return c ? c->t : -1; }
+
+int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
+{
+    if (!c) return FDTD_EINVAL;
+    if (which != FDTD_KERNEL_NAIVE && which != FDTD_KERNEL_SYSTOLIC) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: unknown kernel");
+    if (Nx < 0 || Ny < 0 || Nz < 0 || T < 0) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: negative argument");
+    if ((Nx == 0) != (Ny == 0) || (Nx == 0) != (Nz == 0)) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: give all of Nx,Ny,Nz or none");
+    const int oldN[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};
+    const int oldT = c->reqT, oldw = c->which;
+    c->which = which;
+    c->reqN[0] = Nx; c->reqN[1] = Ny; c->reqN[2] = Nz;
+    c->reqT = T;
+    c->cfg_idx = -1;
+    if (which == FDTD_KERNEL_SYSTOLIC) {
+        const int rc = resolve_systolic(c);
+        if (rc != FDTD_OK) {
+            c->which = oldw; c->reqT = oldT;
+            c->reqN[0] = oldN[0]; c->reqN[1] = oldN[1]; c->reqN[2] = oldN[2];
+            c->cfg_idx = -1;
+            return rc;
+        }
+    }
+    return FDTD_OK;
+}
+
+int fdtd_get_kernel(const fdtd_ctx* cc, int out[8])
+{
+    fdtd_ctx* c = const_cast<fdtd_ctx*>(cc);
+    if (!c || !out) return FDTD_EINVAL;
+    memset(out, 0, 8 * sizeof(int));
+    out[0] = c->which;
+    if (c->which == FDTD_KERNEL_SYSTOLIC) {
+        if (c->cfg_idx < 0) {
+            const int rc = resolve_systolic(c);
+            if (rc != FDTD_OK) return rc;
+        }
+        const SysConfig* s = systolic_config(c->cfg_idx);
+        out[1] = s->Bx - 1; out[2] = s->By - 1; out[3] = s->Bz - 1;
+        out[4] = c->T;
+        long long nt = 1;
+        const int N[3] = {out[1], out[2], out[3]};
+        for (int a = 0; a < 3; ++a) nt *= make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T).nb;
+        out[5] = (int)nt;
+        out[6] = nt < c->ctas ? (int)nt : c->ctas;
+        out[7] = (int)s->smem;
+    }
+    return FDTD_OK;
+}
+
+int fdtd_get_counters(const fdtd_ctx* c, long long out[4])
+{
+    if (!c || !out) return FDTD_EINVAL;
+    for (int q = 0; q < 4; ++q) out[q] = c->counters[q];
+    return FDTD_OK;
+}
+
+int fdtd_last_step_ms(fdtd_ctx* c, float* ms)
+{
+    if (!c || !ms) return FDTD_EINVAL;
+    if (!c->ev_valid) return fail(c, FDTD_ESTATE, "fdtd_last_step_ms before fdtd_step");
+    cudaError_t e = cudaEventSynchronize(c->ev1);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventSynchronize");
+    e = cudaEventElapsedTime(ms, c->ev0, c->ev1);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventElapsedTime");
+    return FDTD_OK;
+}
+
+int fdtd_plan_tiles(const int n[3], const int boundary[3], const int N[3], int T, int ntiles[3])
+{
+    if (!n || !boundary || !N || !ntiles || T < 1) return FDTD_EINVAL;
+    for (int a = 0; a < 3; ++a) {
+        if (n[a] < 1 || N[a] < 1) return FDTD_EINVAL;
+        if (boundary[a] != FDTD_PEC && boundary[a] != FDTD_PERIODIC) return FDTD_EINVAL;
+    }
+    for (int a = 0; a < 3; ++a) ntiles[a] = make_axis_plan(n[a], boundary[a] == FDTD_PERIODIC, N[a], T).nb;
+    return FDTD_OK;
+}
+
+int fdtd_plan_owner(int n, int boundary, int N, int T, int g, int s, int* tile, int* offset)
+{
+    if (n < 1 || N < 1 || T < 1 || g < 0 || g >= n || s < 0 || s >= T || !tile || !offset) return FDTD_EINVAL;
+    if (boundary != FDTD_PEC && boundary != FDTD_PERIODIC) return FDTD_EINVAL;
+    const AxisPlan ap = make_axis_plan(n, boundary == FDTD_PERIODIC, N, T);
+    int u = g + s;                      // position in the frame that moves with the tiles
+    if (ap.per) u %= n;
+    for (int b = 0; b < ap.nb; ++b) {
+        const int a0 = ap.start(b), w = ap.width(b);
+        if (u >= a0 && u < a0 + w) {
+            *tile = b;
+            *offset = u - a0;
+            return FDTD_OK;
+        }
+    }
+    return FDTD_EINVAL;
+}
+
+const char* fdtd_last_error(const fdtd_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+const char* fdtd_build_info(void)
+{
+#ifdef FDTD_NOFMA
+    return "libfdtd_b200 sm_100a fmad=false (bit-exact build)";
+#else
+    return "libfdtd_b200 sm_100a fmad=true";
+#endif
+}
+
+void fdtd_destroy(fdtd_ctx* c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    if (c->d_amp) cudaFree(c->d_amp);
+    if (c->d_wave) cudaFree(c->d_wave);
+    if (c->d_flags) cudaFree(c->d_flags);
+    if (c->d_counter) cudaFree(c->d_counter);
+    if (c->d_abort) cudaFree(c->d_abort);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+}
+
+}  // extern "C"

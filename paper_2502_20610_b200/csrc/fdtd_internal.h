@@ -1,0 +1,18 @@
+// fdtd_internal.h -- launch entry points of libfdtd_b200 (CUDA path only).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "../../include/fdtd.h"
+#include "fdtd_types.h"
+
+// implemented in naive_kernels.cu
+cudaError_t launch_e_half_naive(const GridParams& g, cudaStream_t st);
+cudaError_t launch_h_half_naive(const GridParams& g, cudaStream_t st);
+cudaError_t launch_source_w(const GridParams& g, float w, cudaStream_t st);   // w = wave[t], looked up by the host
+
+// implemented in systolic_kernel.cu
+int systolic_num_configs();
+const SysConfig* systolic_config(int idx);
+// returns cudaSuccess and launches `ctas` persistent CTAs of configuration cfg_idx
+cudaError_t launch_systolic(int cfg_idx, const SysParams& p, int ctas, cudaStream_t st);
+cudaError_t systolic_prepare(int cfg_idx);   // set max dynamic smem attribute

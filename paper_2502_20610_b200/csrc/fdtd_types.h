@@ -1,0 +1,82 @@
+// fdtd_types.h -- plain structs of libfdtd_b200 shared by host and device code (CUDA path only; nothing under
+// oracle/ includes this).  No CUDA headers: tests/emu builds the tile stage functions with plain g++.
+#pragma once
+#include <stddef.h>
+#include <stdint.h>
+
+#ifndef FDTD_HD
+#ifdef __CUDACC__
+#define FDTD_HD __host__ __device__ __forceinline__
+#else
+#define FDTD_HD inline
+#endif
+#endif
+
+// Everything a kernel needs about the grid (passed by value as a __grid_constant__ kernel parameter).
+struct GridParams {
+    float* E[3];
+    float* H[3];
+    const float* ca[3];  // all NULL or all set
+    const float* cb[3];  // all NULL or all set
+    int n[3];
+    int per[3];          // 1 = periodic axis
+    float rd[3];         // (float)(1.0 / (double)d_a)                    (reading #2)
+    float cb_scalar;     // dt, used where cb == NULL
+    float db[3];
+    // soft source (reading #6)
+    int src_comp;        // -1: none
+    int src_box[6];      // i0 j0 k0 ni nj nk
+    const float* src_amp;   // device copy, ni*nj*nk
+    const float* src_wave;  // device copy, nwave
+    int src_nwave;
+};
+
+// One axis of the systolic tile schedule (SURVEY.md section 7 hard part 3 / DESIGN.md reading #11).
+//   PEC axis:      tiles b = 0 .. nb-1, nb = ceil((n+T)/N), start(b) = b*N, width N; regions are clipped to
+//                  [0,n): tiles enter empty at the high wall and drain at the low wall.
+//   periodic axis: a ring of nb = ceil(n/N) tiles of widths base+1 (first rem tiles) or base, all <= N.
+// At step s of a launch tile b owns [start(b) - s, start(b) + width(b) - s)  (the x-y-z-t diagonal).
+struct AxisPlan {
+    int n, per, N, nb, base, rem;
+    FDTD_HD int start(int b) const { return per ? b * base + (b < rem ? b : rem) : b * N; }
+    FDTD_HD int width(int b) const { return per ? base + (b < rem ? 1 : 0) : N; }
+};
+
+inline AxisPlan make_axis_plan(int n, int per, int N, int T)
+{
+    AxisPlan a;
+    a.n = n; a.per = per; a.N = N;
+    if (per) {
+        a.nb = (n + N - 1) / N;
+        a.base = n / a.nb;
+        a.rem = n % a.nb;
+    } else {
+        a.nb = (n + T + N - 1) / N;
+        a.base = N;
+        a.rem = 0;
+    }
+    return a;
+}
+
+struct SysParams {
+    GridParams g;
+    AxisPlan ax[3];
+    int T;                 // steps in this launch
+    long long t0;          // ctx time at launch start (indexes wave[])
+    int flag_base;         // epoch: flags of this launch count up from flag_base
+    int ntiles;
+    int* flagE;            // [ntiles]  = flag_base + (number of E phases published)
+    int* flagH;            // [ntiles]
+    unsigned int* counter; // tile claim counter, zeroed before the launch
+    int* abort_flag;       // != 0: a watchdog fired; every CTA leaves
+    long long spin_budget; // clock64 ticks a single wait may take
+    unsigned int delay_seed; // debug: != 0 inserts pseudo-random sleeps to perturb the inter-CTA order
+};
+
+struct SysConfig {        // one compiled instantiation
+    int Bx, By, Bz;       // cached box (powers of two); updated tile = (Bx-1, By-1, Bz-1)
+    int coef;             // 1: carries the six coefficient arrays on chip
+    int threads;
+    size_t smem;
+};
+

@@ -1,0 +1,268 @@
+// naive_kernels.cu -- the internal baseline: one HBM-bound kernel per half-step.
+//
+// This is the B200 version of the paper's "very straightforward" implementation (section 2):
+// every cell is loaded, updated once and stored, with a kernel boundary (= grid-wide barrier, PAPER.md:61
+// item 1) between the E and the H half-step.  Per cell-update it moves 72 B of HBM with uniform coefficients
+// (12 loads + 6 stores of 4 B: the paper's "6 memory operations" per component) and 96 B with
+// the six coefficient arrays.
+//
+// Mapping: the (x,y) plane is flattened (the layout is x-fastest with no padding, so a plane is one
+// contiguous run); a thread owns VEC consecutive x cells (float4 when nx % 4 == 0) of one (x,y) column and
+// marches ZC planes in z, carrying the z-neighbour plane in registers so that it is read from memory once.
+// y- and x-neighbours come through L1/L2 (the same CTA, or its neighbour, has just loaded those lines).
+//
+// Arithmetic: the expression tree of eq. (1) with coefficients, one rounding per operation when compiled
+// with -fmad=false (then bit-identical to the fp32 oracle); the default build lets ptxas contract mul+add.
+#include "fdtd_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kZChunk = 16;
+
+template <int VEC>
+__device__ __forceinline__ void ldv(const float* __restrict__ p, float (&v)[VEC])
+{
+    if constexpr (VEC == 4) {
+        const float4 t = *reinterpret_cast<const float4*>(p);
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    } else {
+#pragma unroll
+        for (int q = 0; q < VEC; ++q) v[q] = p[q];
+    }
+}
+
+template <int VEC>
+__device__ __forceinline__ void stv(float* __restrict__ p, const float (&v)[VEC])
+{
+    if constexpr (VEC == 4) {
+        *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < VEC; ++q) p[q] = v[q];
+    }
+}
+
+template <int VEC>
+__device__ __forceinline__ void zerov(float (&v)[VEC])
+{
+#pragma unroll
+    for (int q = 0; q < VEC; ++q) v[q] = 0.0f;
+}
+
+// E_a <- ca_a E_a + cb_a [ (H_c - H_c[-e_b]) rd_b - (H_b - H_b[-e_c]) rd_c ]        (eq. (1))
+__device__ __forceinline__ float e_update(float e, float hc, float hc_m, float hb, float hb_m, float rdb, float rdc,
+                                          bool has_ca, float ca, float cb)
+{
+    const float d1 = hc - hc_m;
+    const float d2 = hb - hb_m;
+    const float t1 = d1 * rdb;
+    const float t2 = d2 * rdc;
+    const float curl = t1 - t2;
+    const float keep = has_ca ? ca * e : e;
+    const float gain = cb * curl;
+    return keep + gain;
+}
+
+// H_a <- H_a - db_a [ (E_c[+e_b] - E_c) rd_b - (E_b[+e_c] - E_b) rd_c ]
+__device__ __forceinline__ float h_update(float h, float ec_p, float ec, float eb_p, float eb, float rdb, float rdc, float db)
+{
+    const float d1 = ec_p - ec;
+    const float d2 = eb_p - eb;
+    const float t1 = d1 * rdb;
+    const float t2 = d2 * rdc;
+    const float curl = t1 - t2;
+    const float loss = db * curl;
+    return h - loss;
+}
+
+template <int VEC>
+__global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__ GridParams g)
+{
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long plane = (long long)nx * ny;
+    const long long q = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (q * VEC >= plane) return;
+    const long long cell0 = q * VEC;
+    const int j = (int)(cell0 / nx);
+    const int i0 = (int)(cell0 - (long long)j * nx);
+    const int k0 = blockIdx.y * kZChunk;
+    const int k1 = min(k0 + kZChunk, nz);
+    const bool perx = g.per[0], pery = g.per[1], perz = g.per[2];
+    const bool wall_y = !pery && j == 0;
+    const long long ym_off = (j > 0) ? -(long long)nx : (long long)nx * (ny - 1);
+    const long long xm_off = (i0 > 0) ? -1 : (long long)(nx - 1);
+    const float rdx = g.rd[0], rdy = g.rd[1], rdz = g.rd[2];
+    const bool has_ca = g.ca[0] != nullptr, has_cb = g.cb[0] != nullptr;
+    const float* __restrict__ Hx = g.H[0];
+    const float* __restrict__ Hy = g.H[1];
+    const float* __restrict__ Hz = g.H[2];
+
+    float hx_m[VEC], hy_m[VEC];   // H_x, H_y one plane back in z
+    if (k0 > 0 || perz) {
+        const long long pm = cell0 + plane * (k0 > 0 ? k0 - 1 : nz - 1);
+        ldv<VEC>(Hx + pm, hx_m);
+        ldv<VEC>(Hy + pm, hy_m);
+    } else {
+        zerov<VEC>(hx_m);
+        zerov<VEC>(hy_m);
+    }
+    for (int k = k0; k < k1; ++k) {
+        const long long p = cell0 + plane * k;
+        const bool wall_z = !perz && k == 0;
+        float hx[VEC], hy[VEC], hz[VEC], hz_ym[VEC], hx_ym[VEC], ex[VEC], ey[VEC], ez[VEC];
+        ldv<VEC>(Hx + p, hx);
+        ldv<VEC>(Hy + p, hy);
+        ldv<VEC>(Hz + p, hz);
+        ldv<VEC>(Hz + p + ym_off, hz_ym);
+        ldv<VEC>(Hx + p + ym_off, hx_ym);
+        const float hz_xm = Hz[p + xm_off];
+        const float hy_xm = Hy[p + xm_off];
+        ldv<VEC>(g.E[0] + p, ex);
+        ldv<VEC>(g.E[1] + p, ey);
+        ldv<VEC>(g.E[2] + p, ez);
+        float ca0[VEC], ca1[VEC], ca2[VEC], cb0[VEC], cb1[VEC], cb2[VEC];
+        if (has_ca) { ldv<VEC>(g.ca[0] + p, ca0); ldv<VEC>(g.ca[1] + p, ca1); ldv<VEC>(g.ca[2] + p, ca2); }
+        if (has_cb) { ldv<VEC>(g.cb[0] + p, cb0); ldv<VEC>(g.cb[1] + p, cb1); ldv<VEC>(g.cb[2] + p, cb2); }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            const bool wall_x = !perx && (i0 + v) == 0;
+            const float hz_x = (v == 0) ? hz_xm : hz[v > 0 ? v - 1 : 0];
+            const float hy_x = (v == 0) ? hy_xm : hy[v > 0 ? v - 1 : 0];
+            if (!(wall_y || wall_z))   // E_x: (Hz - Hz[j-1])/dy - (Hy - Hy[k-1])/dz
+                ex[v] = e_update(ex[v], hz[v], hz_ym[v], hy[v], hy_m[v], rdy, rdz, has_ca, has_ca ? ca0[v] : 1.0f,
+                                 has_cb ? cb0[v] : g.cb_scalar);
+            if (!(wall_z || wall_x))   // E_y: (Hx - Hx[k-1])/dz - (Hz - Hz[i-1])/dx
+                ey[v] = e_update(ey[v], hx[v], hx_m[v], hz[v], hz_x, rdz, rdx, has_ca, has_ca ? ca1[v] : 1.0f,
+                                 has_cb ? cb1[v] : g.cb_scalar);
+            if (!(wall_x || wall_y))   // E_z: (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy
+                ez[v] = e_update(ez[v], hy[v], hy_x, hx[v], hx_ym[v], rdx, rdy, has_ca, has_ca ? ca2[v] : 1.0f,
+                                 has_cb ? cb2[v] : g.cb_scalar);
+        }
+        stv<VEC>(g.E[0] + p, ex);
+        stv<VEC>(g.E[1] + p, ey);
+        stv<VEC>(g.E[2] + p, ez);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) { hx_m[v] = hx[v]; hy_m[v] = hy[v]; }
+    }
+}
+
+template <int VEC>
+__global__ void __launch_bounds__(kThreads) h_half_naive(const __grid_constant__ GridParams g)
+{
+    const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
+    const long long plane = (long long)nx * ny;
+    const long long q = (long long)blockIdx.x * kThreads + threadIdx.x;
+    if (q * VEC >= plane) return;
+    const long long cell0 = q * VEC;
+    const int j = (int)(cell0 / nx);
+    const int i0 = (int)(cell0 - (long long)j * nx);
+    const int k0 = blockIdx.y * kZChunk;
+    const int k1 = min(k0 + kZChunk, nz);
+    const bool perx = g.per[0], pery = g.per[1], perz = g.per[2];
+    const bool last_y = (j == ny - 1);
+    const bool ghost_y = last_y && !pery;          // E beyond the high y wall is 0 (reading #5)
+    const long long yp_off = last_y ? -(long long)nx * (ny - 1) : (long long)nx;
+    const bool last_x = (i0 + VEC >= nx);
+    const bool ghost_x = last_x && !perx;
+    const long long xp_off = last_x ? (long long)VEC - nx : (long long)VEC;
+    const float rdx = g.rd[0], rdy = g.rd[1], rdz = g.rd[2];
+    const float* __restrict__ Ex = g.E[0];
+    const float* __restrict__ Ey = g.E[1];
+    const float* __restrict__ Ez = g.E[2];
+
+    float ex[VEC], ey[VEC];
+    ldv<VEC>(Ex + cell0 + plane * k0, ex);
+    ldv<VEC>(Ey + cell0 + plane * k0, ey);
+    for (int k = k0; k < k1; ++k) {
+        const long long p = cell0 + plane * k;
+        float ex_p[VEC], ey_p[VEC], ez[VEC], ez_yp[VEC], ex_yp[VEC], hx[VEC], hy[VEC], hz[VEC];
+        if (k < nz - 1) {
+            ldv<VEC>(Ex + p + plane, ex_p);
+            ldv<VEC>(Ey + p + plane, ey_p);
+        } else if (perz) {
+            ldv<VEC>(Ex + cell0, ex_p);
+            ldv<VEC>(Ey + cell0, ey_p);
+        } else {
+            zerov<VEC>(ex_p);
+            zerov<VEC>(ey_p);
+        }
+        ldv<VEC>(Ez + p, ez);
+        if (ghost_y) {
+            zerov<VEC>(ez_yp);
+            zerov<VEC>(ex_yp);
+        } else {
+            ldv<VEC>(Ez + p + yp_off, ez_yp);
+            ldv<VEC>(Ex + p + yp_off, ex_yp);
+        }
+        const float ey_xp = ghost_x ? 0.0f : Ey[p + xp_off];
+        const float ez_xp = ghost_x ? 0.0f : Ez[p + xp_off];
+        ldv<VEC>(g.H[0] + p, hx);
+        ldv<VEC>(g.H[1] + p, hy);
+        ldv<VEC>(g.H[2] + p, hz);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            const float ey_x = (v == VEC - 1) ? ey_xp : ey[v < VEC - 1 ? v + 1 : v];
+            const float ez_x = (v == VEC - 1) ? ez_xp : ez[v < VEC - 1 ? v + 1 : v];
+            hx[v] = h_update(hx[v], ez_yp[v], ez[v], ey_p[v], ey[v], rdy, rdz, g.db[0]);   // (Ez[j+1]-Ez)/dy - (Ey[k+1]-Ey)/dz
+            hy[v] = h_update(hy[v], ex_p[v], ex[v], ez_x, ez[v], rdz, rdx, g.db[1]);       // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
+            hz[v] = h_update(hz[v], ey_x, ey[v], ex_yp[v], ex[v], rdx, rdy, g.db[2]);      // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
+        }
+        stv<VEC>(g.H[0] + p, hx);
+        stv<VEC>(g.H[1] + p, hy);
+        stv<VEC>(g.H[2] + p, hz);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) { ex[v] = ex_p[v]; ey[v] = ey_p[v]; }
+    }
+}
+
+// E_comp[box] += amp[q] * wave[t]   (reading #6)
+__global__ void source_kernel(const __grid_constant__ GridParams g, float w)
+{
+    const int ni = g.src_box[3], nj = g.src_box[4], nk = g.src_box[5];
+    const long long total = (long long)ni * nj * nk;
+    float* __restrict__ Ec = g.E[g.src_comp];
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
+        const int ii = (int)(q % ni);
+        const int jj = (int)((q / ni) % nj);
+        const int kk = (int)(q / ((long long)ni * nj));
+        const long long p = (long long)(g.src_box[0] + ii) + (long long)g.n[0] * ((long long)(g.src_box[1] + jj) + (long long)g.n[1] * (g.src_box[2] + kk));
+        const float inj = g.src_amp[q] * w;
+        Ec[p] = Ec[p] + inj;
+    }
+}
+
+dim3 naive_grid(const GridParams& g, int vec)
+{
+    const long long plane_vecs = ((long long)g.n[0] * g.n[1] + vec - 1) / vec;
+    return dim3((unsigned)((plane_vecs + kThreads - 1) / kThreads), (unsigned)((g.n[2] + kZChunk - 1) / kZChunk), 1);
+}
+
+}  // namespace
+
+cudaError_t launch_e_half_naive(const GridParams& g, cudaStream_t st)
+{
+    if (g.n[0] % 4 == 0)
+        e_half_naive<4><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
+    else
+        e_half_naive<1><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_h_half_naive(const GridParams& g, cudaStream_t st)
+{
+    if (g.n[0] % 4 == 0)
+        h_half_naive<4><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
+    else
+        h_half_naive<1><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
+    return cudaGetLastError();
+}
+
+// host passes wave[t] by value (the host keeps a copy of the table), so the kernel needs no index
+cudaError_t launch_source_w(const GridParams& g, float w, cudaStream_t st)
+{
+    const long long total = (long long)g.src_box[3] * g.src_box[4] * g.src_box[5];
+    const int blocks = (int)((total + 255) / 256 > 1184 ? 1184 : (total + 255) / 256);
+    source_kernel<<<blocks, 256, 0, st>>>(g, w);
+    return cudaGetLastError();
+}

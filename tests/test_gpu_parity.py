@@ -1,0 +1,205 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Bar (BASELINE.json north_star): max|GPU - oracle| <= 1e-5 * max|field| for the default build, and
+BIT-EXACT for the -fmad=false build ("the systolic order does not change per-cell arithmetic").
+Floats are compared with == (so -0 == +0; reading #13)."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle.yee import YeeOracle
+from paper_2502_20610_b200 import binding, workloads
+from paper_2502_20610_b200.workloads import PEC, PERIODIC
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+def oracle_run(w, steps):
+    E, H = workloads.make_fields(w)
+    ca, cb = workloads.make_coeffs(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None)
+    src = workloads.make_source(w)
+    if src is not None:
+        orc.set_source(src.comp, src.box, src.amp, src.wave)
+    orc.step(steps)
+    return E, H
+
+
+def gpu_run(w, steps, kernel, tile=None, T=0, variant="fma"):
+    E, H, sim = binding.run_workload(w, kernel=kernel, tile=tile, T=T, steps=steps, variant=variant)
+    info = sim.get_kernel()
+    sim.close()
+    return [x.cpu().numpy() for x in E], [x.cpu().numpy() for x in H], info
+
+
+def compare(got, want, exact):
+    scale = max(float(np.abs(x).max()) for x in want[0] + want[1])
+    worst = 0.0
+    for g3, w3 in zip(got, want):
+        for g, w in zip(g3, w3):
+            assert np.all(np.isfinite(g))
+            if exact:
+                assert np.array_equal(g, w), f"not bit-exact: max diff {np.abs(g - w).max():.3e} at {np.unravel_index(np.abs(g - w).argmax(), g.shape)}"
+            worst = max(worst, float(np.abs(g.astype(np.float64) - w.astype(np.float64)).max()))
+    assert worst <= TOL * max(scale, 1e-30), f"max|GPU-oracle| = {worst:.3e} > {TOL} * {scale:.3e}"
+    return worst / max(scale, 1e-30)
+
+
+# reduced-size versions of every BASELINE config (same recipe, several tiles per axis, ragged tails)
+CASES = {
+    "C1": (workloads.config(0), 100),
+    "C2s": (workloads.config(1).scaled((72, 60, 52), steps=150), 150),
+    "C3s": (workloads.config(2).scaled((64, 56, 40), steps=120), 120),
+    "C4s": (workloads.config(3, 128).scaled((100, 96, 90), steps=40), 40),
+    "C5s": (workloads.config(4).scaled((48, 40, 36), steps=90), 90),
+    "ragged": (workloads.Workload("ragged", (37, 29, 23), (1, 0.8, 1.3), (PEC, PERIODIC, PEC), 50, "uniform", "lossy", "dipole"), 50),
+    "allper": (workloads.Workload("allper", (24, 20, 12), (1, 1, 1), (PERIODIC,) * 3, 30, "uniform", "blocks", "sheet"), 30),
+}
+
+
+@pytest.fixture(scope="module")
+def oracle_results():
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            w, steps = CASES[name]
+            cache[name] = oracle_run(w, steps)
+        return cache[name]
+    return get
+
+
+@pytest.mark.parametrize("variant", ["nofma", "fma"])
+@pytest.mark.parametrize("name", list(CASES))
+def test_naive_matches_oracle(cuda_device, oracle_results, name, variant):
+    w, steps = CASES[name]
+    E, H, _ = gpu_run(w, steps, binding.KERNEL_NAIVE, variant=variant)
+    compare((E, H), oracle_results(name), exact=(variant == "nofma"))
+
+
+SYS_RUNS = [
+    # name, tile, T
+    ("C1", (31, 15, 15), 8), ("C1", (15, 15, 15), 25), ("C1", (7, 7, 7), 16),
+    ("C2s", (31, 15, 7), 32), ("C2s", (15, 15, 15), 9), ("C2s", (7, 7, 7), 20),
+    ("C3s", (31, 15, 7), 16), ("C3s", (15, 7, 7), 11),
+    ("C4s", (31, 15, 15), 13), ("C4s", (31, 15, 7), 40),
+    ("C5s", (31, 15, 7), 32), ("C5s", (15, 7, 7), 7),
+    ("ragged", (15, 7, 7), 6), ("ragged", (7, 7, 7), 50),
+    ("allper", (7, 7, 7), 5),
+]
+
+
+@pytest.mark.parametrize("variant", ["nofma", "fma"])
+@pytest.mark.parametrize("name,tile,T", SYS_RUNS)
+def test_systolic_matches_oracle(cuda_device, oracle_results, name, tile, T, variant):
+    w, steps = CASES[name]
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=tile, T=T, variant=variant)
+    assert info["which"] == binding.KERNEL_SYSTOLIC and info["tile"] == tile and info["T"] == T
+    compare((E, H), oracle_results(name), exact=(variant == "nofma"))
+
+
+def test_systolic_default_configuration(cuda_device, oracle_results):
+    # whatever tile / depth the library picks by itself
+    for name in ("C1", "C2s"):
+        w, steps = CASES[name]
+        E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, variant="nofma")
+        assert info["tiles"] > 1
+        compare((E, H), oracle_results(name), exact=True)
+
+
+def test_systolic_under_perturbed_cta_order(cuda_device, oracle_results, monkeypatch):
+    """Pseudo-random sleeps between phases reorder the CTAs; the flag protocol must keep the result bit-exact."""
+    w, steps = CASES["C2s"]
+    for seed in (11, 12345):
+        monkeypatch.setenv("FDTD_DEBUG_DELAY", str(seed))
+        E, H, _ = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(7, 7, 7), T=10, variant="nofma")
+        compare((E, H), oracle_results("C2s"), exact=True)
+
+
+def test_step_splitting_and_time(cuda_device, oracle_results):
+    """fdtd_step(a); fdtd_step(b) == fdtd_step(a+b): launch boundaries leave every cell at the same time level (a11)."""
+    import torch
+    w, steps = CASES["C2s"]
+    dev = torch.device("cuda:0")
+    E, H = workloads.make_fields(w, device=dev)
+    ca, cb = workloads.make_coeffs(w, device=dev)
+    src = workloads.make_source(w)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant="nofma")
+    sim.set_fields(E, H)
+    sim.set_coeffs(ca, cb)
+    sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC, (15, 15, 15), 16)
+    for part in (1, 37, 0, 16, steps - 54):
+        sim.step(part)
+    sim.sync()
+    assert sim.time == steps and sim.counters()["steps"] == steps
+    compare(([x.cpu().numpy() for x in E], [x.cpu().numpy() for x in H]), oracle_results("C2s"), exact=True)
+    sim.close()
+
+
+def test_host_buffer_round_trip(cuda_device, oracle_results):
+    """The end-to-end entry: host arrays in (fdtd_load_fields), host arrays out (fdtd_get_fields)."""
+    import torch
+    w, steps = CASES["C1"]
+    dev = torch.device("cuda:0")
+    Eh, Hh = workloads.make_fields(w)
+    E = [torch.empty(x.shape, dtype=torch.float32, device=dev) for x in Eh]
+    H = [torch.empty(x.shape, dtype=torch.float32, device=dev) for x in Hh]
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant="nofma")
+    sim.set_fields(E, H)
+    sim.load_fields(Eh, Hh)
+    sim.step(steps)
+    Eo = [np.empty_like(x) for x in Eh]
+    Ho = [np.empty_like(x) for x in Hh]
+    sim.get_fields(Eo, Ho)
+    compare((Eo, Ho), oracle_results("C1"), exact=True)
+    sim.close()
+
+
+def test_api_errors(cuda_device):
+    import torch
+    with pytest.raises(binding.FdtdError) as e:
+        binding.Fdtd((0, 8, 8), (1, 1, 1), 0.1, (0, 0, 0))
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.FdtdError):
+        binding.Fdtd((8, 8, 8), (1, -1, 1), 0.1, (0, 0, 0))
+    sim = binding.Fdtd((8, 8, 8), (1, 1, 1), 0.1, (0, 0, 0))
+    with pytest.raises(binding.FdtdError) as e:
+        sim.step(1)
+    assert e.value.code == binding.ESTATE
+    with pytest.raises(binding.FdtdError) as e:
+        sim.set_kernel(binding.KERNEL_SYSTOLIC, (5, 5, 5), 4)     # not a built tile shape
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.FdtdError) as e:
+        sim.set_source(2, (7, 7, 7, 2, 1, 1), np.ones(2, np.float32), np.ones(3, np.float32))   # box leaves the grid
+    assert e.value.code == binding.EINVAL
+    t = [torch.zeros((8, 8, 8), dtype=torch.float32, device="cuda:0") for _ in range(6)]
+    sim.set_fields(t[:3], t[3:])
+    sim.step(0)
+    sim.sync()
+    assert all(float(x.abs().max()) == 0.0 for x in t)              # zero stays zero (P11)
+    sim.step(3)
+    sim.sync()
+    assert all(float(x.abs().max()) == 0.0 for x in t)
+    sim.close()
+    # a periodic ring that cannot be resident at once is refused, not deadlocked
+    big = binding.Fdtd((4096, 64, 8), (1, 1, 1), 0.1, (0, 1, 0))
+    with pytest.raises(binding.FdtdError) as e:
+        big.set_kernel(binding.KERNEL_SYSTOLIC, (7, 7, 7), 4)
+    assert e.value.code == binding.EINVAL
+    big.close()
+
+
+@pytest.mark.parametrize("variant", ["nofma"])
+def test_full_size_config2_systolic_vs_oracle_and_naive(cuda_device, variant):
+    """BASELINE configs[1] at its full 256^3 size in the launch configuration bench.py times (library defaults),
+    shortened to 3 launches (96 steps; the oracle needs ~10 s for them): bit-exact against the oracle."""
+    w = workloads.config(1)
+    steps = 96
+    want = oracle_run(w, steps)
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, variant=variant)
+    assert info["tiles"] > 148
+    compare((E, H), want, exact=True)
+    E2, H2, _ = gpu_run(w, steps, binding.KERNEL_NAIVE, variant=variant)
+    compare((E2, H2), want, exact=True)

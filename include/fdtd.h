@@ -17,6 +17,11 @@
  *                         subdomain on chip, slide it along the x-y-z-t diagonal, exchange only faces through
  *                         global memory and hand off with per-tile flags.  It performs "the exact same update
  *                         equations", so results are identical per cell to the naive schedule.
+ *                         Tile 31x15x7 runs the register-resident kernel (fields in registers, coefficients in
+ *                         shared memory, loader warps staging the faces with cp.async); other built tile
+ *                         shapes run the shared-memory kernel below.
+ *   FDTD_KERNEL_SYSTOLIC_SMEM  the same schedule with the whole subdomain in shared memory (the first,
+ *                         simpler implementation; kept as a cross-check and for other tile shapes).
  *
  * Layout contract.  Every field / coefficient component is ONE contiguous fp32 array of nx*ny*nz elements,
  * x fastest:  idx = i + nx*(j + ny*k).  Yee positions: E_x(i+1/2,j,k) E_y(i,j+1/2,k) E_z(i,j,k+1/2)
@@ -46,7 +51,7 @@ typedef struct fdtd_ctx fdtd_ctx; /* opaque; owned by the library */
 
 enum { FDTD_PEC = 0, FDTD_PERIODIC = 1 };
 enum { FDTD_OK = 0, FDTD_EINVAL = 1, FDTD_ENOMEM = 2, FDTD_ECUDA = 3, FDTD_ESTATE = 4, FDTD_ETIMEOUT = 5 };
-enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1 };
+enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1, FDTD_KERNEL_SYSTOLIC_SMEM = 2 };
 
 /* Create a context for an nx*ny*nz grid with cell sizes dx,dy,dz (> 0, finite), time step dt (> 0, finite)
  * and per-axis wall type boundary[3] (host array of FDTD_PEC | FDTD_PERIODIC).
@@ -100,7 +105,7 @@ int fdtd_sync(fdtd_ctx* ctx);
 int fdtd_set_time(fdtd_ctx* ctx, long long t);
 long long fdtd_get_time(const fdtd_ctx* ctx);
 
-/* Choose the schedule.  which = FDTD_KERNEL_NAIVE | FDTD_KERNEL_SYSTOLIC.
+/* Choose the schedule.  which = FDTD_KERNEL_NAIVE | FDTD_KERNEL_SYSTOLIC | FDTD_KERNEL_SYSTOLIC_SMEM.
  * For the systolic kernel (Nx,Ny,Nz) is the updated tile ("subdomain": 31x15x15 updated inside a
  * 32x16x16 cached block) and T the temporal depth (steps a tile stays resident per launch); 0 = library default.
  * FDTD_EINVAL if the shape is not one the kernel was built for or the grid cannot run it (see fdtd_last_error). */

@@ -25,7 +25,11 @@ struct fdtd_ctx {
     int which;
     int reqN[3];      // requested tile (0 = default)
     int reqT;         // requested temporal depth (0 = default)
-    int cfg_idx;      // resolved systolic configuration, -1 = unresolved
+    int cfg_idx;      // resolved shared-memory systolic configuration, -1 = unresolved / not used
+    bool use_reg;     // resolved: the register-resident kernel (tile 31x15x7) runs
+    bool resolved;
+    int N[3];         // resolved tile
+    size_t smem;      // resolved dynamic shared memory per CTA
     int T;            // resolved temporal depth
     int ctas;
     // systolic state
@@ -86,33 +90,44 @@ int resolve_systolic(fdtd_ctx* c)
 {
     if (coef_mixed(c)) return fail(c, FDTD_EINVAL, "systolic kernel needs ca and cb both bound or both NULL");
     const int want_coef = has_coef(c) ? 1 : 0;
+    const bool smem_only = c->which == FDTD_KERNEL_SYSTOLIC_SMEM;
     int N[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};
     if (N[0] == 0) {
-        if (want_coef) { N[0] = 31; N[1] = 15; N[2] = 7; }
-        else           { N[0] = 31; N[1] = 15; N[2] = 15; }
+        if (!smem_only || want_coef) { N[0] = 31; N[1] = 15; N[2] = 7; }
+        else                         { N[0] = 31; N[1] = 15; N[2] = 15; }
         if (const char* e = getenv("FDTD_TILE")) {
             int x, y, z;
             if (sscanf(e, "%dx%dx%d", &x, &y, &z) == 3) { N[0] = x; N[1] = y; N[2] = z; }
         }
     }
+    c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
     int found = -1;
-    for (int i = 0; i < systolic_num_configs(); ++i) {
-        const SysConfig* s = systolic_config(i);
-        if (s->Bx - 1 == N[0] && s->By - 1 == N[1] && s->Bz - 1 == N[2] && s->coef == want_coef) { found = i; break; }
+    int threads = 0;
+    if (c->use_reg) {
+        cudaError_t e = systolic_reg_prepare(want_coef);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+        c->smem = systolic_reg_smem(want_coef);
+        threads = systolic_reg_threads();
+    } else {
+        for (int i = 0; i < systolic_num_configs(); ++i) {
+            const SysConfig* s = systolic_config(i);
+            if (s->Bx - 1 == N[0] && s->By - 1 == N[1] && s->Bz - 1 == N[2] && s->coef == want_coef) { found = i; break; }
+        }
+        if (found < 0) {
+            char buf[160];
+            snprintf(buf, sizeof buf, "no systolic kernel built for tile %dx%dx%d %s coefficient arrays", N[0], N[1], N[2],
+                     want_coef ? "with" : "without");
+            return fail(c, FDTD_EINVAL, buf);
+        }
+        cudaError_t e = systolic_prepare(found);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+        c->smem = systolic_config(found)->smem;
+        threads = systolic_config(found)->threads;
     }
-    if (found < 0) {
-        char buf[160];
-        snprintf(buf, sizeof buf, "no systolic kernel built for tile %dx%dx%d %s coefficient arrays", N[0], N[1], N[2],
-                 want_coef ? "with" : "without");
-        return fail(c, FDTD_EINVAL, buf);
-    }
-    cudaError_t e = systolic_prepare(found);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
-    const SysConfig* s = systolic_config(found);
-    // persistent grid: every CTA resident at once (one per SM for the 192 KB boxes)
-    int per_sm = (int)((227u * 1024u) / (s->smem + 1024u));
+    // persistent grid: every CTA resident at once
+    int per_sm = (int)((227u * 1024u) / (c->smem + 1024u));
     if (per_sm < 1) per_sm = 1;
-    int by_threads = 2048 / s->threads;
+    int by_threads = 2048 / threads;
     if (per_sm > by_threads) per_sm = by_threads;
     if (per_sm > 4) per_sm = 4;
     c->ctas = c->num_sms * per_sm;
@@ -131,6 +146,8 @@ int resolve_systolic(fdtd_ctx* c)
         return fail(c, FDTD_EINVAL, buf);
     }
     c->cfg_idx = found;
+    for (int a = 0; a < 3; ++a) c->N[a] = N[a];
+    c->resolved = true;
     return FDTD_OK;
 }
 
@@ -173,12 +190,11 @@ int step_naive(fdtd_ctx* c, int n)
 
 int step_systolic(fdtd_ctx* c, int n)
 {
-    if (c->cfg_idx < 0) {
+    if (!c->resolved) {
         const int rc = resolve_systolic(c);
         if (rc != FDTD_OK) return rc;
     }
-    const SysConfig* s = systolic_config(c->cfg_idx);
-    const int N[3] = {s->Bx - 1, s->By - 1, s->Bz - 1};
+    const int N[3] = {c->N[0], c->N[1], c->N[2]};
     int left = n;
     while (left > 0) {
         const int T = left < c->T ? left : c->T;
@@ -211,7 +227,7 @@ int step_systolic(fdtd_ctx* c, int n)
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
-        e = launch_systolic(c->cfg_idx, P, ctas, c->stream);
+        e = c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream) : launch_systolic(c->cfg_idx, P, ctas, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "systolic launch");
         c->flag_base += T + 2;
         c->t += T;
@@ -284,6 +300,9 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->which = FDTD_KERNEL_SYSTOLIC;
     c->reqT = 0;
     c->cfg_idx = -1;
+    c->use_reg = false;
+    c->resolved = false;
+    c->smem = 0;
     c->T = 0;
     c->ctas = 0;
     c->d_flags = nullptr;
@@ -362,6 +381,7 @@ int fdtd_set_coeffs(fdtd_ctx* c, const float* const ca[3], const float* const cb
         c->g.db[a] = db ? db[a] : c->dt;
     }
     c->cfg_idx = -1;   // the coefficient-carrying kernels are separate instantiations
+    c->resolved = false;
     return FDTD_OK;
 }
 
@@ -457,7 +477,7 @@ long long fdtd_get_time(const fdtd_ctx* c) { return c ? c->t : -1; }
 int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
 {
     if (!c) return FDTD_EINVAL;
-    if (which != FDTD_KERNEL_NAIVE && which != FDTD_KERNEL_SYSTOLIC) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: unknown kernel");
+    if (which != FDTD_KERNEL_NAIVE && which != FDTD_KERNEL_SYSTOLIC && which != FDTD_KERNEL_SYSTOLIC_SMEM) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: unknown kernel");
     if (Nx < 0 || Ny < 0 || Nz < 0 || T < 0) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: negative argument");
     if ((Nx == 0) != (Ny == 0) || (Nx == 0) != (Nz == 0)) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: give all of Nx,Ny,Nz or none");
     const int oldN[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};
@@ -466,12 +486,14 @@ int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
     c->reqN[0] = Nx; c->reqN[1] = Ny; c->reqN[2] = Nz;
     c->reqT = T;
     c->cfg_idx = -1;
-    if (which == FDTD_KERNEL_SYSTOLIC) {
+    c->resolved = false;
+    if (which != FDTD_KERNEL_NAIVE) {
         const int rc = resolve_systolic(c);
         if (rc != FDTD_OK) {
             c->which = oldw; c->reqT = oldT;
             c->reqN[0] = oldN[0]; c->reqN[1] = oldN[1]; c->reqN[2] = oldN[2];
             c->cfg_idx = -1;
+            c->resolved = false;
             return rc;
         }
     }
@@ -484,20 +506,19 @@ int fdtd_get_kernel(const fdtd_ctx* cc, int out[8])
     if (!c || !out) return FDTD_EINVAL;
     memset(out, 0, 8 * sizeof(int));
     out[0] = c->which;
-    if (c->which == FDTD_KERNEL_SYSTOLIC) {
-        if (c->cfg_idx < 0) {
+    if (c->which != FDTD_KERNEL_NAIVE) {
+        if (!c->resolved) {
             const int rc = resolve_systolic(c);
             if (rc != FDTD_OK) return rc;
         }
-        const SysConfig* s = systolic_config(c->cfg_idx);
-        out[1] = s->Bx - 1; out[2] = s->By - 1; out[3] = s->Bz - 1;
+        out[1] = c->N[0]; out[2] = c->N[1]; out[3] = c->N[2];
         out[4] = c->T;
         long long nt = 1;
         const int N[3] = {out[1], out[2], out[3]};
         for (int a = 0; a < 3; ++a) nt *= make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T).nb;
         out[5] = (int)nt;
         out[6] = nt < c->ctas ? (int)nt : c->ctas;
-        out[7] = (int)s->smem;
+        out[7] = (int)c->smem;
     }
     return FDTD_OK;
 }

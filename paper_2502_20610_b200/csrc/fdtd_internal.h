@@ -16,3 +16,9 @@ const SysConfig* systolic_config(int idx);
 // returns cudaSuccess and launches `ctas` persistent CTAs of configuration cfg_idx
 cudaError_t launch_systolic(int cfg_idx, const SysParams& p, int ctas, cudaStream_t st);
 cudaError_t systolic_prepare(int cfg_idx);   // set max dynamic smem attribute
+
+// implemented in systolic_reg.cu: the register-resident systolic kernel, tile 31x15x7 in a 32x16x8 box
+size_t systolic_reg_smem(int coef);
+int systolic_reg_threads();
+cudaError_t systolic_reg_prepare(int coef);
+cudaError_t launch_systolic_reg(int coef, const SysParams& p, int ctas, cudaStream_t st);

@@ -99,6 +99,28 @@ def test_systolic_matches_oracle(cuda_device, oracle_results, name, tile, T, var
     compare((E, H), oracle_results(name), exact=(variant == "nofma"))
 
 
+# the register-resident kernel (tile 31x15x7) on every reduced config, several temporal depths, incl. T > tile width
+REG_RUNS = [("C1", 8), ("C1", 33), ("C2s", 5), ("C2s", 32), ("C3s", 16), ("C3s", 7), ("C4s", 40), ("C4s", 3),
+            ("C5s", 32), ("C5s", 1), ("ragged", 6), ("ragged", 50), ("allper", 5)]
+
+
+@pytest.mark.parametrize("name,T", REG_RUNS)
+def test_register_kernel_matches_oracle(cuda_device, oracle_results, name, T):
+    w, steps = CASES[name]
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=T, variant="nofma")
+    assert info["smem"] < 200 * 1024 and info["T"] == T
+    compare((E, H), oracle_results(name), exact=True)
+
+
+@pytest.mark.parametrize("name,T", [("C2s", 32), ("C3s", 16), ("C1", 8)])
+def test_shared_memory_kernel_same_tile(cuda_device, oracle_results, name, T):
+    """FDTD_KERNEL_SYSTOLIC_SMEM: the first implementation (whole subdomain in shared memory), same schedule."""
+    w, steps = CASES[name]
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC_SMEM, tile=(31, 15, 7), T=T, variant="nofma")
+    assert info["which"] == binding.KERNEL_SYSTOLIC_SMEM
+    compare((E, H), oracle_results(name), exact=True)
+
+
 def test_systolic_default_configuration(cuda_device, oracle_results):
     # whatever tile / depth the library picks by itself
     for name in ("C1", "C2s"):
@@ -114,6 +136,8 @@ def test_systolic_under_perturbed_cta_order(cuda_device, oracle_results, monkeyp
     for seed in (11, 12345):
         monkeypatch.setenv("FDTD_DEBUG_DELAY", str(seed))
         E, H, _ = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(7, 7, 7), T=10, variant="nofma")
+        compare((E, H), oracle_results("C2s"), exact=True)
+        E, H, _ = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=12, variant="nofma")
         compare((E, H), oracle_results("C2s"), exact=True)
 
 

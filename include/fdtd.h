@@ -51,7 +51,7 @@ typedef struct fdtd_ctx fdtd_ctx; /* opaque; owned by the library */
 
 enum { FDTD_PEC = 0, FDTD_PERIODIC = 1 };
 enum { FDTD_OK = 0, FDTD_EINVAL = 1, FDTD_ENOMEM = 2, FDTD_ECUDA = 3, FDTD_ESTATE = 4, FDTD_ETIMEOUT = 5 };
-enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1, FDTD_KERNEL_SYSTOLIC_SMEM = 2 };
+enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1, FDTD_KERNEL_SYSTOLIC_SMEM = 2, FDTD_KERNEL_SYSTOLIC_REG = 3 };
 
 /* Create a context for an nx*ny*nz grid with cell sizes dx,dy,dz (> 0, finite), time step dt (> 0, finite)
  * and per-axis wall type boundary[3] (host array of FDTD_PEC | FDTD_PERIODIC).

@@ -11,7 +11,7 @@ import os
 
 PEC, PERIODIC = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, ETIMEOUT = range(6)
-KERNEL_NAIVE, KERNEL_SYSTOLIC, KERNEL_SYSTOLIC_SMEM = 0, 1, 2
+KERNEL_NAIVE, KERNEL_SYSTOLIC, KERNEL_SYSTOLIC_SMEM, KERNEL_SYSTOLIC_REG = 0, 1, 2, 3
 _ERRNAME = {1: "FDTD_EINVAL", 2: "FDTD_ENOMEM", 3: "FDTD_ECUDA", 4: "FDTD_ESTATE", 5: "FDTD_ETIMEOUT"}
 
 HERE = os.path.dirname(os.path.abspath(__file__))

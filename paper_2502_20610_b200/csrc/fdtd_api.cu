@@ -9,6 +9,8 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
+
 #include "fdtd_internal.h"
 
 struct fdtd_ctx {
@@ -27,6 +29,9 @@ struct fdtd_ctx {
     int reqT;         // requested temporal depth (0 = default)
     int cfg_idx;      // resolved shared-memory systolic configuration, -1 = unresolved / not used
     bool use_reg;     // resolved: the register-resident kernel (tile 31x15x7) runs
+    bool use_tma;     // resolved: its TMA-staged version runs (PEC grids, nx % 4 == 0)
+    TmaMaps tmaps;    // 36 CUtensorMap: [E0..2 H0..2 ca0..2 cb0..2][z plane, y row, x column]
+    bool tmaps_valid;
     bool resolved;
     int N[3];         // resolved tile
     size_t smem;      // resolved dynamic shared memory per CTA
@@ -101,9 +106,16 @@ int resolve_systolic(fdtd_ctx* c)
         }
     }
     c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
+    c->use_tma = c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->g.per[0] && !c->g.per[1] && !c->g.per[2] &&
+                 c->g.n[0] % 4 == 0 && !getenv("FDTD_NO_TMA");
     int found = -1;
     int threads = 0;
-    if (c->use_reg) {
+    if (c->use_tma) {
+        cudaError_t e = systolic_tma_prepare(want_coef);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+        c->smem = systolic_tma_smem(want_coef);
+        threads = systolic_tma_threads();
+    } else if (c->use_reg) {
         cudaError_t e = systolic_reg_prepare(want_coef);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
         c->smem = systolic_reg_smem(want_coef);
@@ -168,6 +180,57 @@ int ensure_flags(fdtd_ctx* c, size_t ntiles)
     return FDTD_OK;
 }
 
+// Tensor maps of the TMA-staged kernel: each field / coefficient array is a rank-3 fp32 tensor (nx, ny, nz) with
+// byte strides (4 nx, 4 nx ny); one map per array and shell piece (the box extents are part of the map).
+// Elements outside the tensor are delivered as zeros: the PEC ghost of reading #5 and the empty part of clipped tiles.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int ensure_tmaps(fdtd_ctx* c)
+{
+    if (c->tmaps_valid) return FDTD_OK;
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) return fail(c, FDTD_ECUDA, "cuTensorMapEncodeTiled is not available in this driver");
+        encode = (EncodeTiledFn)fn;
+    }
+    int box[3][3];
+    systolic_tma_boxes(box);
+    const void* arr[12];
+    for (int a = 0; a < 3; ++a) {
+        arr[a] = c->g.E[a];
+        arr[3 + a] = c->g.H[a];
+        arr[6 + a] = c->g.ca[a];
+        arr[9 + a] = c->g.cb[a];
+    }
+    static_assert(sizeof(CUtensorMap) * 36 == sizeof(TmaMaps), "TmaMaps layout");
+    CUtensorMap* host = reinterpret_cast<CUtensorMap*>(c->tmaps.bytes);
+    memset(c->tmaps.bytes, 0, sizeof c->tmaps.bytes);
+    const cuuint64_t dims[3] = {(cuuint64_t)c->g.n[0], (cuuint64_t)c->g.n[1], (cuuint64_t)c->g.n[2]};
+    const cuuint64_t strides[2] = {(cuuint64_t)c->g.n[0] * 4u, (cuuint64_t)c->g.n[0] * c->g.n[1] * 4u};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    for (int a = 0; a < 12; ++a) {
+        if (!arr[a]) continue;
+        for (int f = 0; f < 3; ++f) {
+            const cuuint32_t b[3] = {(cuuint32_t)box[f][0], (cuuint32_t)box[f][1], (cuuint32_t)box[f][2]};
+            const CUresult r = encode(&host[a * 3 + f], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(arr[a]), dims, strides, b, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                char buf[96];
+                snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d) for array %d piece %d", (int)r, a, f);
+                return fail(c, FDTD_ECUDA, buf);
+            }
+        }
+    }
+    c->tmaps_valid = true;
+    return FDTD_OK;
+}
+
 int step_naive(fdtd_ctx* c, int n)
 {
     for (int s = 0; s < n; ++s) {
@@ -192,6 +255,10 @@ int step_systolic(fdtd_ctx* c, int n)
 {
     if (!c->resolved) {
         const int rc = resolve_systolic(c);
+        if (rc != FDTD_OK) return rc;
+    }
+    if (c->use_tma) {
+        const int rc = ensure_tmaps(c);
         if (rc != FDTD_OK) return rc;
     }
     const int N[3] = {c->N[0], c->N[1], c->N[2]};
@@ -224,10 +291,13 @@ int step_systolic(fdtd_ctx* c, int n)
         P.abort_flag = c->d_abort;
         P.spin_budget = c->spin_budget;
         P.delay_seed = c->delay_seed;
+        P.dbg = getenv("FDTD_DEBUG_SKIP") ? atoi(getenv("FDTD_DEBUG_SKIP")) : 0;
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
-        e = c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream) : launch_systolic(c->cfg_idx, P, ctas, c->stream);
+        e = c->use_tma   ? launch_systolic_tma(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
+            : c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream)
+                         : launch_systolic(c->cfg_idx, P, ctas, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "systolic launch");
         c->flag_base += T + 2;
         c->t += T;
@@ -301,6 +371,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->reqT = 0;
     c->cfg_idx = -1;
     c->use_reg = false;
+    c->use_tma = false;
+    c->tmaps_valid = false;
     c->resolved = false;
     c->smem = 0;
     c->T = 0;
@@ -346,6 +418,7 @@ int fdtd_set_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
         c->g.H[a] = H[a];
     }
     c->fields_set = true;
+    c->tmaps_valid = false;
     return FDTD_OK;
 }
 
@@ -382,6 +455,7 @@ int fdtd_set_coeffs(fdtd_ctx* c, const float* const ca[3], const float* const cb
     }
     c->cfg_idx = -1;   // the coefficient-carrying kernels are separate instantiations
     c->resolved = false;
+    c->tmaps_valid = false;
     return FDTD_OK;
 }
 
@@ -477,7 +551,7 @@ long long fdtd_get_time(const fdtd_ctx* c) { return c ? c->t : -1; }
 int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
 {
     if (!c) return FDTD_EINVAL;
-    if (which != FDTD_KERNEL_NAIVE && which != FDTD_KERNEL_SYSTOLIC && which != FDTD_KERNEL_SYSTOLIC_SMEM) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: unknown kernel");
+    if (which != FDTD_KERNEL_NAIVE && which != FDTD_KERNEL_SYSTOLIC && which != FDTD_KERNEL_SYSTOLIC_SMEM && which != FDTD_KERNEL_SYSTOLIC_REG) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: unknown kernel");
     if (Nx < 0 || Ny < 0 || Nz < 0 || T < 0) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: negative argument");
     if ((Nx == 0) != (Ny == 0) || (Nx == 0) != (Nz == 0)) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: give all of Nx,Ny,Nz or none");
     const int oldN[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};

@@ -22,3 +22,10 @@ size_t systolic_reg_smem(int coef);
 int systolic_reg_threads();
 cudaError_t systolic_reg_prepare(int coef);
 cudaError_t launch_systolic_reg(int coef, const SysParams& p, int ctas, cudaStream_t st);
+
+// implemented in systolic_tma.cu: the TMA-staged systolic kernel (PEC grids, nx % 4 == 0), tile 31x15x7
+size_t systolic_tma_smem(int coef);
+int systolic_tma_threads();
+void systolic_tma_boxes(int box[3][3]);   // TMA box extents (x,y,z) of the z-plane, y-row and x-column shell pieces
+cudaError_t systolic_tma_prepare(int coef);
+cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);

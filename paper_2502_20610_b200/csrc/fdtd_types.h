@@ -70,7 +70,14 @@ struct SysParams {
     unsigned int* counter; // tile claim counter, zeroed before the launch
     int* abort_flag;       // != 0: a watchdog fired; every CTA leaves
     long long spin_budget; // clock64 ticks a single wait may take
+    int dbg;               // debug timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes, 8 no fences
     unsigned int delay_seed; // debug: != 0 inserts pseudo-random sleeps to perturb the inter-CTA order
+};
+
+// 36 CUtensorMap (128 bytes each) passed to systolic_tma.cu as a __grid_constant__ kernel parameter:
+// [12 arrays: E0..2 H0..2 ca0..2 cb0..2][3 shell pieces: z plane, y row, x column]
+struct alignas(64) TmaMaps {
+    unsigned char bytes[36 * 128];
 };
 
 struct SysConfig {        // one compiled instantiation

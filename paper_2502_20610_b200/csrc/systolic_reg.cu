@@ -169,7 +169,7 @@ __device__ __forceinline__ void tile_init(const SysParams& P, int tile, TileGeom
 __device__ __forceinline__ void wait_upwind(const SysParams& P, const TileGeom& t, const int* flags, int target, Ctl* ctl)
 {
     const int lane = threadIdx.x & 31;
-    if (lane < 7 && *(volatile int*)&ctl->abort == 0) {
+    if (lane < 7 && *(volatile int*)&ctl->abort == 0 && !(P.dbg & 1)) {
         const int u = t.nbr[lane];
         if (u >= 0) {
             const long long t_start = clock64();
@@ -215,6 +215,7 @@ __device__ __forceinline__ void load_shell(const SysParams& P, const TileGeom& t
         int gx, gy, gz;
         const bool in = resolve(P, 0, o0 + lx, gx) & resolve(P, 1, o1 + ly, gy) & resolve(P, 2, o2 + lz, gz);
         const long long off = in ? gx + nx * (gy + ny * (long long)gz) : 0;
+        if (P.dbg & 2) return;
 #pragma unroll
         for (int c = 0; c < 3; ++c) cp_async4(d0 + c * dstride, fld[c] + off, in);
         if (COEF && WITH_COEF) {
@@ -398,7 +399,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exEx[(l + 1) * PLANE + slot] = ex[l + 1];
             }
             // publish E of R_k \ R_{k+1} (everything at the last step)                                  (a8, a6)
-            if (colE) {
+            if (colE && !(P.dbg & 4)) {
                 const bool whole = last || lx == w0 || ly == w1;
                 if (whole) {
 #pragma unroll
@@ -479,7 +480,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exHx[m * PLANE + slot] = hx[m];
             }
             // publish H of R_{k+1} \ R_{k+2}: frame-k planes l = w-1 (everything at the last step)       (a8, a6)
-            if (colH) {
+            if (colH && !(P.dbg & 4)) {
                 const bool whole = last || lx == w0 - 1 || ly == w1 - 1;
                 if (whole) {
 #pragma unroll
@@ -562,12 +563,12 @@ __global__ void __launch_bounds__(NT, 1) systolic_reg_kernel(const __grid_consta
             for (int k = 0; k < T; ++k) {
                 bar_sync(BAR_EDONE, N_EDONE);
                 if (lane == 0) {
-                    __threadfence();
+                    if (!(P.dbg & 8)) __threadfence();
                     st_release(P.flagE + tile, P.flag_base + k + 1);
                 }
                 bar_sync(BAR_HDONE, N_HDONE);
                 if (lane == 0) {
-                    __threadfence();
+                    if (!(P.dbg & 8)) __threadfence();
                     st_release(P.flagH + tile, P.flag_base + k + 1);
                 }
             }

@@ -1,0 +1,676 @@
+// systolic_tma.cu -- the systolic FDTD kernel for sm_100a, TMA-staged version (the product kernel on PEC grids).
+//
+// Schedule: exactly that of systolic_reg.cu / DESIGN.md section 4 (tile regions R_k = [a-k, a+w-k) sliding along
+// the x-y-z-t diagonal; one E phase and one H phase per step; minus-shell loads and
+// plus-shell publishes through global memory; per-tile acquire/release flags on the seven upwind
+// neighbours).  What differs is how a B200 SM executes it:
+//
+//   * box 32 x 16 x 8 cells (tile 31 x 15 x 7).  Compute thread (lane, warp) owns the (x,y) slot
+//     (gx mod 32, gy mod 16) and keeps the 8-cell z column of all six field components in REGISTERS; the slide
+//     in x/y is modular addressing, the slide in z a register renaming inside the unrolled z march.
+//   * the compute warps execute NO per-cell predicate: walls and the outside of the domain are data.  Cells
+//     outside the grid are zero-filled by TMA (fields and coefficients), so E stays 0 there (the PEC ghost,
+//     reading #5); frozen wall components get (ca, cb) = (1, 0) when their coefficients enter the chip; shell
+//     slots compute garbage that the next shell absorb overwrites.  Stores are predicated, arithmetic is not.
+//   * the minus shell of every step is fetched by TMA (cp.async.bulk.tensor.3d, three boxes per array: a z
+//     plane 36x16x1, a y row 36x1x7, an x column 4x15x7, each starting on a 16-byte boundary in x) into shared-memory staging, completing on mbarriers;
+//     auxiliary warps poll the upwind flags, issue the copies one step ahead of the compute warps, scatter
+//     the entering coefficients into the owner threads' private shared-memory slots and repack the x column
+//     so that its single owner lane absorbs it with 16-byte loads.
+//   * every hand-off inside the CTA is an mbarrier with one elected arrive per warp; the only CTA-wide
+//     barrier is the 512-thread named barrier between absorb and phase.
+//
+//   compute (warps 0-15)     H side (warps 16,17)            E side (warp 18)          signal (warp 19)
+//   --------------------     --------------------            ----------------          ----------------
+//   wait HREADY(k)           wait HFREE(k-1)                 wait EFREE(k-1), HDONE(k-1)
+//   absorb H shell  ->HFREE  poll flagH[u] >= base+k         poll flagE[u] >= base+k+1
+//   E phase k                TMA H (+ coefficient) shell     TMA E shell
+//   publish E       ->EDONE  wait EDONE(k-1), copies landed  wait copies landed        wait EDONE(k): fence,
+//   wait EREADY(k)           scatter coefficients, pack x    pack x column                  flagE = base+k+1
+//   absorb E shell  ->EFREE  ->HREADY(k)                     ->EREADY(k)
+//   H phase k
+//   publish H       ->HDONE                                                            wait HDONE(k): fence,
+//                                                                                           flagH = base+k+1
+//
+// Per-cell arithmetic is yee_update.h, unchanged: with -fmad=false the result is bit-identical to the oracle.
+// Scope: all three axes PEC and nx % 4 == 0 (TMA strides are multiples of 16 bytes); other grids run
+// systolic_reg.cu.
+#include <cuda.h>
+
+#include "fdtd_internal.h"
+#include "yee_update.h"
+
+namespace {
+
+constexpr int BX = 32, BY = 16, BZ = 8;
+constexpr int W0 = BX - 1, W1 = BY - 1, W2 = BZ - 1;   // tile widths (PEC axes: always full)
+constexpr int PLANE = BX * BY;                          // 512 (x,y) slots = compute threads
+constexpr int NCOMPUTE = PLANE;
+constexpr int NWARPS_C = NCOMPUTE / 32;
+constexpr int NT = NCOMPUTE + 128;
+constexpr int W_HPROD = 16, W_HAUX = 17, W_EPROD = 18;   // warp 19: signal
+
+// staging of one array's minus shell (floats); every TMA destination is 128-byte aligned
+// TMA needs the innermost start coordinate on a 16-byte boundary, the shell slides by one cell per step: every
+// box starts at q0 = o0 & ~3 and is RX = 36 cells wide; r0 = o0 & 3 is where the shell begins inside a staged row
+constexpr int RX = BX + 4;
+constexpr int ST_Z = RX * BY;                // box (36,16,1)   [y][x]      576 floats
+constexpr int ST_YRAW = RX * W2;             // box (36,1,7)    [z][x]      252 floats
+constexpr int ST_Y = 256;                    // padded to a multiple of 32 floats
+constexpr int ST_XRAW = 4 * W1 * W2;         // box (4,15,7)    [z][y][4]   (only x index r0 is used)
+constexpr int ST_X = 448;                    // ST_XRAW = 420 padded to a multiple of 32 floats
+constexpr int ST_ARR = ST_Z + ST_Y + ST_X;   // 1280 floats
+constexpr int XPK = BY * 3 * 8;              // packed x column [y slot][component][8]
+constexpr int EXP = 7 * PLANE;               // one exchange array: 7 planes of (x,y) slots
+constexpr unsigned BYTES_ARR = (ST_Z + ST_YRAW + ST_XRAW) * 4u;   // bytes TMA delivers per array and step
+
+template <bool COEF>
+struct Lay {
+    static constexpr int NC = COEF ? 6 : 3;            // resident coefficient arrays (no COEF: cb masks only)
+    static constexpr int stgh = 0;
+    static constexpr int stge = stgh + 3 * ST_ARR;
+    static constexpr int stgc = stge + 3 * ST_ARR;
+    static constexpr int xpkh = stgc + (COEF ? 6 * ST_ARR : 0);
+    static constexpr int xpke = xpkh + XPK;
+    static constexpr int exch = xpke + XPK;            // exHz, exHx, exEz, exEx
+    static constexpr int coef = exch + 4 * EXP;
+    static constexpr int total = coef + NC * BZ * PLANE;
+};
+
+enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_SIGACK, MB_COUNT };
+
+struct TileGeom {
+    int a[3];
+    int nbr[7];
+};
+
+struct Ctl {
+    int tile;
+    int abort;
+};
+
+// ---- PTX helpers --------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ int ld_acquire(const int* p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ int ld_volatile(const int* p)
+{
+    int v;
+    asm volatile("ld.volatile.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void bar_sync(int id, int count)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+// one elected arrive per warp, after every lane's earlier shared/global accesses
+__device__ __forceinline__ void warp_arrive(unsigned long long* bar)
+{
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+// TMA: box of the 3-D tensor `map` at element coordinates (c0,c1,c2) -> shared memory; out-of-bounds elements
+// are written as zeros; completes `bytes of the box` on the mbarrier
+__device__ __forceinline__ void tma_load_3d(float* dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(smem_u32(dst)),
+                 "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- geometry ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tile_init(const SysParams& P, int tile, TileGeom& t)
+{
+    const int nbx = P.ax[0].nb, nby = P.ax[1].nb;
+    int b[3];
+    b[0] = tile % nbx;
+    b[1] = (tile / nbx) % nby;
+    b[2] = tile / (nbx * nby);
+    t.a[0] = b[0] * W0;
+    t.a[1] = b[1] * W1;
+    t.a[2] = b[2] * W2;
+    for (int d = 1; d < 8; ++d) {
+        int idx[3];
+        bool ok = true;
+        for (int q = 0; q < 3; ++q) {
+            idx[q] = b[q] - ((d >> q) & 1);
+            if (idx[q] < 0) ok = false;
+        }
+        t.nbr[d - 1] = ok ? idx[0] + nbx * (idx[1] + nby * idx[2]) : -1;
+    }
+}
+
+// frozen tangential E on the low PEC walls (reading #5): component c of the cell at (gx,gy,gz)
+__device__ __forceinline__ bool frozen(int c, int gx, int gy, int gz)
+{
+    return c == 0 ? (gy == 0) | (gz == 0) : c == 1 ? (gz == 0) | (gx == 0) : (gx == 0) | (gy == 0);
+}
+
+// lanes 0..6 of the calling warp each watch one upwind neighbour (a9); watchdog as in systolic_reg.cu
+__device__ __forceinline__ void wait_upwind(const SysParams& P, const TileGeom& t, const int* flags, int target, Ctl* ctl)
+{
+    const int lane = threadIdx.x & 31;
+    if (lane < 7 && *(volatile int*)&ctl->abort == 0 && !(P.dbg & 1)) {
+        const int u = t.nbr[lane];
+        if (u >= 0 && ld_acquire(flags + u) < target) {
+            const long long t_start = clock64();
+            unsigned spins = 0;
+            while (ld_acquire(flags + u) < target) {
+                if ((++spins & 63u) == 0u) {
+                    if (ld_volatile(P.abort_flag) != 0) { *(volatile int*)&ctl->abort = 1; break; }
+                    if (clock64() - t_start > P.spin_budget) {
+                        atomicExch(P.abort_flag, 1);
+                        *(volatile int*)&ctl->abort = 1;
+                        break;
+                    }
+                }
+                __nanosleep(32);
+            }
+        }
+    }
+    __syncwarp();
+}
+
+__device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k, int phase)
+{
+    unsigned h = P.delay_seed ^ (unsigned)(tile * 2654435761u) ^ (unsigned)(k * 40503u + phase * 97u);
+    h ^= h >> 15; h *= 2246822519u; h ^= h >> 13; h *= 3266489917u; h ^= h >> 16;
+    if ((h & 3u) == 0u) __nanosleep((h >> 8) & 0x3fffu);   // up to ~16 us, one phase in four
+}
+
+// one lane issues the three boxes of `narr` consecutive tensor maps (maps[arr*3 + face]) for the box of step k
+__device__ __forceinline__ void issue_shell(const CUtensorMap* maps, int narr, float* stg, int o0, int o1, int o2, unsigned long long* bar)
+{
+    const int q0 = o0 & ~3;
+    mbar_expect_tx(bar, (unsigned)narr * BYTES_ARR);
+    for (int a = 0; a < narr; ++a) {
+        float* d = stg + a * ST_ARR;
+        tma_load_3d(d, maps + a * 3 + 0, q0, o1, o2, bar);                      // z plane l_z = 0
+        tma_load_3d(d + ST_Z, maps + a * 3 + 1, q0, o1, o2 + 1, bar);           // y row   l_y = 0, l_z = 1..7
+        tma_load_3d(d + ST_Z + ST_Y, maps + a * 3 + 2, q0, o1 + 1, o2 + 1, bar);   // x column l_x = 0, l_y = 1..15, l_z = 1..7
+    }
+}
+
+// ---- H-side auxiliary warps: coefficients of the entering cells -> the owner threads' private slots ----------
+// part / 2 splits the work between warps 16 and 17.  COEF: values come from the staged arrays (ca 0..2, cb 3..5)
+// and frozen wall components become (1, 0); no COEF: the three cb masks are generated (dt inside, 0 frozen/outside).
+template <bool COEF>
+__device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int o0, int o1, int o2, int part)
+{
+    constexpr int NC = Lay<COEF>::NC;
+    const int lane = threadIdx.x & 31;
+    const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
+    const float* stg = sm + Lay<COEF>::stgc;
+    float* coef = sm + Lay<COEF>::coef;
+    const bool walls = (o0 <= 0) | (o1 <= 0) | (o2 <= 0);   // the box touches a low wall: fix-ups needed
+    const int r0 = o0 & 3;
+    const float dt = P.g.cb_scalar;
+
+    auto put = [&](int c, int src, int lx, int ly, int l) {
+        const int gx = o0 + lx, gy = o1 + ly, gz = o2 + l;
+        float v;
+        if (COEF) {
+            v = stg[c * ST_ARR + src];
+            if (walls && frozen(c % 3, gx, gy, gz)) v = c < 3 ? 1.0f : 0.0f;
+        } else {
+            const bool in = ((unsigned)gx < (unsigned)nx) & ((unsigned)gy < (unsigned)ny) & ((unsigned)gz < (unsigned)nz);
+            v = (in && !frozen(c, gx, gy, gz)) ? dt : 0.0f;
+        }
+        coef[(c * BZ + (gz & (BZ - 1))) * PLANE + (gy & (BY - 1)) * BX + (gx & (BX - 1))] = v;
+    };
+
+    int task = part;
+    for (int c = 0; c < NC; ++c) {
+        for (int j = 0; j < BY; ++j, ++task)          // z plane: rows l_y = j
+            if (task & 1) put(c, j * RX + r0 + lane, lane, j, 0);
+        for (int l = 1; l < BZ; ++l, ++task)          // y row: l_z = l
+            if (task & 1) put(c, ST_Z + (l - 1) * RX + r0 + lane, lane, 0, l);
+        for (int r = 0; r < 4; ++r, ++task) {         // x column: 105 cells, (l_z-1)*15 + (l_y-1)
+            const int idx = r * 32 + lane;
+            if ((task & 1) && idx < W1 * W2) put(c, ST_Z + ST_Y + idx * 4 + r0, 0, 1 + idx % W1, 1 + idx / W1);
+        }
+    }
+}
+
+// x column of the three field arrays in `stg` -> xpk[(y slot*3 + c)*8 + l], l = 1..7 (16-byte rows for the owner lane)
+__device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, int o1, int part, int nparts)
+{
+    const int lane = threadIdx.x & 31;
+    int task = 0;
+    for (int c = 0; c < 3; ++c)
+        for (int r = 0; r < 4; ++r, ++task) {
+            const int idx = r * 32 + lane;
+            if (task % nparts == part && idx < W1 * W2) {
+                const int ly = 1 + idx % W1, l = 1 + idx / W1;
+                xpk[(((o1 + ly) & (BY - 1)) * 3 + c) * 8 + l] = stg[c * ST_ARR + ST_Z + ST_Y + idx * 4 + (o0 & 3)];
+            }
+        }
+}
+
+// ---- compute warps ---------------------------------------------------------------------------------------------
+struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
+    unsigned hready, eready, sigack;
+};
+
+template <bool COEF>
+__device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, float* sm, unsigned long long* mb, Phases& ph)
+{
+    const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
+    const int slot = wy * BX + lane;
+    const int slot_ym = ((wy - 1) & (BY - 1)) * BX + lane, slot_yp = ((wy + 1) & (BY - 1)) * BX + lane;
+    const int lane_m = (lane - 1) & 31, lane_p = (lane + 1) & 31;
+    const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
+    const long long plane = (long long)nx * ny;
+
+    const float* stgH = sm + Lay<COEF>::stgh;
+    const float* stgE = sm + Lay<COEF>::stge;
+    const float* xpkH = sm + Lay<COEF>::xpkh;
+    const float* xpkE = sm + Lay<COEF>::xpke;
+    float* exHz = sm + Lay<COEF>::exch;
+    float* exHx = exHz + EXP;
+    float* exEz = exHx + EXP;
+    float* exEx = exEz + EXP;
+    float* coef = sm + Lay<COEF>::coef + slot;   // this thread's private coefficient slots: [(c*BZ + z slot)*PLANE]
+
+    const float rdx = P.g.rd[0], rdy = P.g.rd[1], rdz = P.g.rd[2];
+    const float dbx = P.g.db[0], dby = P.g.db[1], dbz = P.g.db[2];
+    float* const Ex = P.g.E[0]; float* const Ey = P.g.E[1]; float* const Ez = P.g.E[2];
+    float* const Hx = P.g.H[0]; float* const Hy = P.g.H[1]; float* const Hz = P.g.H[2];
+
+    // frame k: local l <-> global z = o2 + l.  E(l) lives in e?[l] before the E phase and in e?[l+1] after it;
+    // H(l) lives in h?[l] before the H phase and in h?[l+1] (= frame k+1 index) after it.
+    float ex[BZ + 1], ey[BZ + 1], ez[BZ + 1], hx[BZ], hy[BZ], hz[BZ];
+#pragma unroll
+    for (int l = 0; l <= BZ; ++l) ex[l] = ey[l] = ez[l] = 0.0f;
+#pragma unroll
+    for (int l = 0; l < BZ; ++l) hx[l] = hy[l] = hz[l] = 0.0f;
+
+    const int T = P.T;
+    for (int k = 0; k < T; ++k) {
+        const bool last = (k == T - 1);
+        const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+        const int lx = (lane - o0) & (BX - 1), ly = (wy - o1) & (BY - 1);
+        const int gx = o0 + lx, gy = o1 + ly;
+        const bool col_in = ((unsigned)gx < (unsigned)nx) & ((unsigned)gy < (unsigned)ny);
+        const long long col_off = col_in ? gx + (long long)nx * gy : 0;
+
+        // ---------------- H (+ coefficient) minus shell ----------------------------------------------------
+        if (k == 0) {
+            // a6: the whole box straight from global memory; H and coefficients on [0,w]^3, E on R_0 = [1,w]^3
+#pragma unroll
+            for (int l = 0; l < BZ; ++l) {
+                const int gz = o2 + l;
+                const bool ok = col_in && (unsigned)gz < (unsigned)nz;
+                const long long off = ok ? col_off + plane * gz : 0;
+                hx[l] = ok ? __ldcg(Hx + off) : 0.0f;
+                hy[l] = ok ? __ldcg(Hy + off) : 0.0f;
+                hz[l] = ok ? __ldcg(Hz + off) : 0.0f;
+                const bool oke = ok && lx >= 1 && ly >= 1 && l >= 1;
+                ex[l] = oke ? __ldcg(Ex + off) : 0.0f;
+                ey[l] = oke ? __ldcg(Ey + off) : 0.0f;
+                ez[l] = oke ? __ldcg(Ez + off) : 0.0f;
+                float* cs = coef + (gz & (BZ - 1)) * PLANE;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const bool fr = frozen(c, gx, gy, gz);
+                    if (COEF) {
+                        const float a = ok ? __ldg(P.g.ca[c] + off) : 0.0f;
+                        const float b = ok ? __ldg(P.g.cb[c] + off) : 0.0f;
+                        cs[c * (BZ * PLANE)] = fr ? 1.0f : a;
+                        cs[(3 + c) * (BZ * PLANE)] = fr ? 0.0f : b;
+                    } else {
+                        cs[c * (BZ * PLANE)] = (ok && !fr) ? P.g.cb_scalar : 0.0f;
+                    }
+                }
+            }
+#pragma unroll
+            for (int l = 1; l < BZ; ++l) {
+                exHz[(l - 1) * PLANE + slot] = hz[l];
+                exHx[(l - 1) * PLANE + slot] = hx[l];
+            }
+        } else {
+            mbar_wait(mb + MB_HREADY, ph.hready & 1u);
+            ++ph.hready;
+            const int zi = ly * RX + (o0 & 3) + lx;
+            hx[0] = stgH[0 * ST_ARR + zi];
+            hy[0] = stgH[1 * ST_ARR + zi];
+            hz[0] = stgH[2 * ST_ARR + zi];
+            if (ly == 0) {            // warp-uniform: the entering row; its y+1 neighbours read it from the exchange
+                const float* sy = stgH + ST_Z + (o0 & 3) + lx;
+#pragma unroll
+                for (int l = 1; l < BZ; ++l) {
+                    hx[l] = sy[0 * ST_ARR + (l - 1) * RX];
+                    hy[l] = sy[1 * ST_ARR + (l - 1) * RX];
+                    hz[l] = sy[2 * ST_ARR + (l - 1) * RX];
+                    exHz[(l - 1) * PLANE + slot] = hz[l];
+                    exHx[(l - 1) * PLANE + slot] = hx[l];
+                }
+            } else if (lx == 0) {     // one lane per warp: the entering column, packed by the H-side warps
+                const float4* s4 = reinterpret_cast<const float4*>(xpkH + wy * 24);
+                const float4 a0 = s4[0], a1 = s4[1], b0 = s4[2], b1 = s4[3], c0 = s4[4], c1 = s4[5];
+                hx[1] = a0.y; hx[2] = a0.z; hx[3] = a0.w; hx[4] = a1.x; hx[5] = a1.y; hx[6] = a1.z; hx[7] = a1.w;
+                hy[1] = b0.y; hy[2] = b0.z; hy[3] = b0.w; hy[4] = b1.x; hy[5] = b1.y; hy[6] = b1.z; hy[7] = b1.w;
+                hz[1] = c0.y; hz[2] = c0.z; hz[3] = c0.w; hz[4] = c1.x; hz[5] = c1.y; hz[6] = c1.z; hz[7] = c1.w;
+            }
+            warp_arrive(mb + MB_HFREE);
+        }
+        bar_sync(1, NCOMPUTE);   // exchange rows of H (shell + last H phase) and the scattered coefficients are visible
+
+        // ---------------- E phase on R_k = [1,w]^3 (a1): every slot computes, shell slots produce garbage ----
+#pragma unroll
+        for (int l = BZ - 1; l >= 1; --l) {
+            const float hz_xm = __shfl_sync(0xffffffffu, hz[l], lane_m);
+            const float hy_xm = __shfl_sync(0xffffffffu, hy[l], lane_m);
+            const float hz_ym = exHz[(l - 1) * PLANE + slot_ym];
+            const float hx_ym = exHx[(l - 1) * PLANE + slot_ym];
+            const float* cs = coef + ((o2 + l) & (BZ - 1)) * PLANE;
+            float cax = 1.0f, cay = 1.0f, caz = 1.0f, cbx, cby, cbz;
+            if (COEF) {
+                cax = cs[0 * (BZ * PLANE)]; cay = cs[1 * (BZ * PLANE)]; caz = cs[2 * (BZ * PLANE)];
+                cbx = cs[3 * (BZ * PLANE)]; cby = cs[4 * (BZ * PLANE)]; cbz = cs[5 * (BZ * PLANE)];
+            } else {
+                cbx = cs[0 * (BZ * PLANE)]; cby = cs[1 * (BZ * PLANE)]; cbz = cs[2 * (BZ * PLANE)];
+            }
+            // E_x: (Hz - Hz[j-1])/dy - (Hy - Hy[k-1])/dz      eq. (1)
+            ex[l + 1] = yee_e_update<COEF>(ex[l], hz[l], hz_ym, hy[l], hy[l - 1], rdy, rdz, cax, cbx);
+            // E_y: (Hx - Hx[k-1])/dz - (Hz - Hz[i-1])/dx
+            ey[l + 1] = yee_e_update<COEF>(ey[l], hx[l], hx[l - 1], hz[l], hz_xm, rdz, rdx, cay, cby);
+            // E_z: (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy
+            ez[l + 1] = yee_e_update<COEF>(ez[l], hy[l], hy_xm, hx[l], hx_ym, rdx, rdy, caz, cbz);
+        }
+        const bool actE = (lx >= 1) & (ly >= 1);            // column belongs to R_k
+        // soft source after the E update of step t0 + k (a4): rare, CTA-uniform test first
+        {
+            const long long ts = P.t0 + k;
+            if (P.g.src_comp >= 0 && ts >= 0 && ts < P.g.src_nwave &&
+                P.g.src_box[0] <= o0 + W0 && P.g.src_box[0] + P.g.src_box[3] > o0 + 1 &&
+                P.g.src_box[1] <= o1 + W1 && P.g.src_box[1] + P.g.src_box[4] > o1 + 1 &&
+                P.g.src_box[2] <= o2 + W2 && P.g.src_box[2] + P.g.src_box[5] > o2 + 1) {
+                const int sx = gx - P.g.src_box[0], sy = gy - P.g.src_box[1];
+                if (actE && sx >= 0 && sx < P.g.src_box[3] && sy >= 0 && sy < P.g.src_box[4]) {
+                    const float wsrc = __ldg(P.g.src_wave + ts);
+#pragma unroll
+                    for (int l = 1; l < BZ; ++l) {
+                        const int sz = o2 + l - P.g.src_box[2];
+                        if (sz >= 0 && sz < P.g.src_box[5]) {
+                            const float amp = __ldg(P.g.src_amp + (sx + P.g.src_box[3] * (sy + (long long)P.g.src_box[4] * sz)));
+                            const float inj = amp * wsrc;
+                            if (P.g.src_comp == 0) ex[l + 1] = ex[l + 1] + inj;
+                            else if (P.g.src_comp == 1) ey[l + 1] = ey[l + 1] + inj;
+                            else ez[l + 1] = ez[l + 1] + inj;
+                        }
+                    }
+                }
+            }
+        }
+        // E of planes 1..6 for the y+1 readers of the H phase; the shell column lx = 0 is written by the E-side warp
+        if (lx != 0) {
+#pragma unroll
+            for (int l = 1; l < BZ - 1; ++l) {
+                exEz[l * PLANE + slot] = ez[l + 1];
+                exEx[l * PLANE + slot] = ex[l + 1];
+            }
+        }
+        // publish E of R_k \ R_{k+1} (everything at the last step)                                      (a8, a6)
+        if (actE && col_in && !(P.dbg & 4)) {
+            const bool whole = last | (lx == W0) | (ly == W1);
+#pragma unroll
+            for (int l = 1; l < BZ; ++l) {
+                const int gz = o2 + l;
+                if ((whole || l == W2) && (unsigned)gz < (unsigned)nz) {
+                    const long long off = col_off + plane * gz;
+                    __stcg(Ex + off, ex[l + 1]);
+                    __stcg(Ey + off, ey[l + 1]);
+                    __stcg(Ez + off, ez[l + 1]);
+                }
+            }
+        }
+        if (k > 0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it
+            mbar_wait(mb + MB_SIGACK, ph.sigack & 1u);
+            ++ph.sigack;
+        }
+        warp_arrive(mb + MB_EDONE);
+        if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);
+
+        // ---------------- E minus shell -------------------------------------------------------------------------
+        mbar_wait(mb + MB_EREADY, ph.eready & 1u);
+        ++ph.eready;
+        {
+            const int zi = ly * RX + (o0 & 3) + lx;
+            ex[1] = stgE[0 * ST_ARR + zi];
+            ey[1] = stgE[1 * ST_ARR + zi];
+            ez[1] = stgE[2 * ST_ARR + zi];
+            exEz[slot] = ez[1];
+            exEx[slot] = ex[1];
+            if (ly == 0) {
+                const float* sy = stgE + ST_Z + (o0 & 3) + lx;
+#pragma unroll
+                for (int l = 1; l < BZ; ++l) {
+                    ex[l + 1] = sy[0 * ST_ARR + (l - 1) * RX];
+                    ey[l + 1] = sy[1 * ST_ARR + (l - 1) * RX];
+                    ez[l + 1] = sy[2 * ST_ARR + (l - 1) * RX];
+                }
+            } else if (lx == 0) {
+                const float4* s4 = reinterpret_cast<const float4*>(xpkE + wy * 24);
+                const float4 a0 = s4[0], a1 = s4[1], b0 = s4[2], b1 = s4[3], c0 = s4[4], c1 = s4[5];
+                ex[2] = a0.y; ex[3] = a0.z; ex[4] = a0.w; ex[5] = a1.x; ex[6] = a1.y; ex[7] = a1.z; ex[8] = a1.w;
+                ey[2] = b0.y; ey[3] = b0.z; ey[4] = b0.w; ey[5] = b1.x; ey[6] = b1.y; ey[7] = b1.z; ey[8] = b1.w;
+                ez[2] = c0.y; ez[3] = c0.z; ez[4] = c0.w; ez[5] = c1.x; ez[6] = c1.y; ez[7] = c1.z; ez[8] = c1.w;
+            }
+        }
+        warp_arrive(mb + MB_EFREE);
+        bar_sync(1, NCOMPUTE);   // exchange rows of E are visible
+
+        // ---------------- H phase on R_{k+1} = [0,w-1]^3 (a2): every slot computes ----------------------------
+#pragma unroll
+        for (int l = BZ - 2; l >= 0; --l) {
+            const float ey_xp = __shfl_sync(0xffffffffu, ey[l + 1], lane_p);
+            const float ez_xp = __shfl_sync(0xffffffffu, ez[l + 1], lane_p);
+            const float ez_yp = exEz[l * PLANE + slot_yp];
+            const float ex_yp = exEx[l * PLANE + slot_yp];
+            hx[l + 1] = yee_h_update(hx[l], ez_yp, ez[l + 1], ey[l + 2], ey[l + 1], rdy, rdz, dbx);   // (Ez[j+1]-Ez)/dy - (Ey[k+1]-Ey)/dz
+            hy[l + 1] = yee_h_update(hy[l], ex[l + 2], ex[l + 1], ez_xp, ez[l + 1], rdz, rdx, dby);   // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
+            hz[l + 1] = yee_h_update(hz[l], ey_xp, ey[l + 1], ex_yp, ex[l + 1], rdx, rdy, dbz);       // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
+            exHz[l * PLANE + slot] = hz[l + 1];
+            exHx[l * PLANE + slot] = hx[l + 1];
+        }
+        // publish H of R_{k+1} \ R_{k+2} (everything at the last step)                                  (a8, a6)
+        if ((lx <= W0 - 1) & (ly <= W1 - 1) && col_in && !(P.dbg & 4)) {
+            const bool whole = last | (lx == W0 - 1) | (ly == W1 - 1);
+#pragma unroll
+            for (int l = 0; l < BZ - 1; ++l) {
+                const int gz = o2 + l;
+                if ((whole || l == W2 - 1) && (unsigned)gz < (unsigned)nz) {
+                    const long long off = col_off + plane * gz;
+                    __stcg(Hx + off, hx[l + 1]);
+                    __stcg(Hy + off, hy[l + 1]);
+                    __stcg(Hz + off, hz[l + 1]);
+                }
+            }
+        }
+        warp_arrive(mb + MB_HDONE);
+        if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);
+    }
+    // the signal warp's last ack of this tile is covered by the CTA barrier at the tile boundary
+    ++ph.sigack;
+}
+
+template <bool COEF>
+__global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_constant__ SysParams P, const __grid_constant__ TmaMaps M)
+{
+    extern __shared__ __align__(128) float sm[];
+    __shared__ __align__(8) unsigned long long mb[MB_COUNT];
+    __shared__ Ctl ctl;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        ctl.abort = 0;
+        mbar_init(mb + MB_HFULL, 1);
+        mbar_init(mb + MB_CFULL, 1);
+        mbar_init(mb + MB_EFULL, 1);
+        mbar_init(mb + MB_HREADY, 2);
+        mbar_init(mb + MB_EREADY, 1);
+        mbar_init(mb + MB_HFREE, NWARPS_C);
+        mbar_init(mb + MB_EFREE, NWARPS_C);
+        mbar_init(mb + MB_EDONE, NWARPS_C);
+        mbar_init(mb + MB_HDONE, NWARPS_C);
+        mbar_init(mb + MB_SIGACK, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(M.bytes);   // [E0 E1 E2 H0 H1 H2 ca0..2 cb0..2][3 faces]
+    Phases ph = {0u, 0u, 0u};
+    // completed phases of every mbarrier an auxiliary role waits on (each role counts only what it uses)
+    unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) {
+            ctl.tile = (int)atomicAdd(P.counter, 1u);
+            if (ld_volatile(P.abort_flag) != 0) ctl.abort = 1;
+        }
+        __syncthreads();
+        const int tile = ctl.tile;
+        if (tile >= P.ntiles || ctl.abort) break;
+        TileGeom t;
+        tile_init(P, tile, t);
+        const int T = P.T;
+
+        if (warp < NWARPS_C) {
+            compute_tile<COEF>(P, t, tile, sm, mb, ph);
+        } else if (warp == W_HPROD || warp == W_HAUX) {
+            // H side: shell of step k needs the staging of step k-1 absorbed (HFREE), the upwind tiles' H of
+            // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
+            for (int k = 1; k < T; ++k) {
+                const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                if (warp == W_HPROD) {
+                    if (k >= 2) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
+                    wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
+                    if (lane == 0 && !(P.dbg & 2)) {
+                        fence_proxy_async();
+                        issue_shell(maps + 3 * 3, 3, sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
+                        if (COEF) issue_shell(maps + 6 * 3, 6, sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                    }
+                    __syncwarp();
+                }
+                mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
+                if (!(P.dbg & 2)) {
+                    mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull;
+                    if (COEF) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
+                }
+                scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
+                pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1, warp - W_HPROD, 2);
+                warp_arrive(mb + MB_HREADY);
+            }
+            if (T >= 2) ++n_hfree;        // the last absorb's HFREE phase: covered by the CTA barrier at the tile boundary
+            ++n_edone;                    // EDONE(T-1) likewise
+        } else if (warp == W_EPROD) {
+            for (int k = 0; k < T; ++k) {
+                const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                if (k >= 1) {
+                    mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
+                    mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;     // H phase k-1 has read the E exchange rows
+                }
+                wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
+                if (!(P.dbg & 2)) {
+                    if (lane == 0) {
+                        fence_proxy_async();
+                        issue_shell(maps, 3, sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
+                    }
+                    __syncwarp();
+                    mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull;
+                }
+                const float* stg = sm + Lay<COEF>::stge;
+                pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1, 0, 1);
+                // the shell column's Ez, Ex of planes 1..6 for its y-1 readers in the H phase
+                float* exEz = sm + Lay<COEF>::exch + 2 * EXP;
+                float* exEx = exEz + EXP;
+                for (int r = 0; r < 3; ++r) {
+                    const int idx = r * 32 + lane;            // (l-1)*15 + (ly-1), l = 1..6
+                    if (idx < W1 * (W2 - 1)) {
+                        const int ly = 1 + idx % W1, l = 1 + idx / W1;
+                        const int s = ((o1 + ly) & (BY - 1)) * BX + (o0 & (BX - 1));
+                        exEz[l * PLANE + s] = stg[2 * ST_ARR + ST_Z + ST_Y + idx * 4 + (o0 & 3)];
+                        exEx[l * PLANE + s] = stg[0 * ST_ARR + ST_Z + ST_Y + idx * 4 + (o0 & 3)];
+                    }
+                }
+                warp_arrive(mb + MB_EREADY);
+            }
+            ++n_efree; ++n_hdone;         // phases of step T-1: covered by the CTA barrier at the tile boundary
+        } else {
+            // signal warp: every publish of the phase has been issued before its warp arrived; make them visible
+            // at gpu scope, then raise the flag                                                              (a9)
+            for (int k = 0; k < T; ++k) {
+                mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
+                if (lane == 0) {
+                    if (!(P.dbg & 8)) __threadfence();
+                    st_release(P.flagE + tile, P.flag_base + k + 1);
+                }
+                mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
+                if (lane == 0) {
+                    if (!(P.dbg & 8)) __threadfence();
+                    st_release(P.flagH + tile, P.flag_base + k + 1);
+                    mbar_arrive(mb + MB_SIGACK);
+                }
+                __syncwarp();
+            }
+        }
+    }
+}
+
+}  // namespace
+
+size_t systolic_tma_smem(int coef) { return (size_t)(coef ? Lay<true>::total : Lay<false>::total) * sizeof(float); }
+int systolic_tma_threads() { return NT; }
+void systolic_tma_boxes(int box[3][3])
+{
+    const int b[3][3] = {{RX, BY, 1}, {RX, 1, W2}, {4, W1, W2}};
+    for (int f = 0; f < 3; ++f)
+        for (int q = 0; q < 3; ++q) box[f][q] = b[f][q];
+}
+
+cudaError_t systolic_tma_prepare(int coef)
+{
+    const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
+    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)systolic_tma_smem(coef));
+}
+
+cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st)
+{
+    static_assert(sizeof(CUtensorMap) == 128, "TmaMaps layout");
+    const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
+    void* args[] = {(void*)&p, (void*)&maps};
+    return cudaLaunchKernel(fn, dim3((unsigned)ctas), dim3((unsigned)NT), args, systolic_tma_smem(coef), st);
+}

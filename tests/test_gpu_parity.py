@@ -106,10 +106,27 @@ REG_RUNS = [("C1", 8), ("C1", 33), ("C2s", 5), ("C2s", 32), ("C3s", 16), ("C3s",
 
 @pytest.mark.parametrize("name,T", REG_RUNS)
 def test_register_kernel_matches_oracle(cuda_device, oracle_results, name, T):
+    """FDTD_KERNEL_SYSTOLIC_REG: the cp.async-staged register kernel (any wall type, any nx)."""
     w, steps = CASES[name]
-    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=T, variant="nofma")
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC_REG, tile=(31, 15, 7), T=T, variant="nofma")
     assert info["smem"] < 200 * 1024 and info["T"] == T
     compare((E, H), oracle_results(name), exact=True)
+
+
+# the TMA-staged kernel (what FDTD_KERNEL_SYSTOLIC runs on PEC grids with nx % 4 == 0): every PEC config, several
+# temporal depths incl. T = 1, T > tile width and T > grid size; both builds
+TMA_RUNS = [("C1", 8), ("C1", 33), ("C1", 100), ("C2s", 5), ("C2s", 32), ("C2s", 1), ("C4s", 40), ("C4s", 3), ("C5s", 32), ("C5s", 2),
+            ("C5s", 90)]
+
+
+@pytest.mark.parametrize("variant", ["nofma", "fma"])
+@pytest.mark.parametrize("name,T", TMA_RUNS)
+def test_tma_kernel_matches_oracle(cuda_device, oracle_results, name, T, variant):
+    w, steps = CASES[name]
+    assert all(b == PEC for b in w.boundary) and w.n[0] % 4 == 0
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=T, variant=variant)
+    assert info["smem"] in (220160, 140288) and info["T"] == T     # the TMA kernel, not the cp.async kernel
+    compare((E, H), oracle_results(name), exact=(variant == "nofma"))
 
 
 @pytest.mark.parametrize("name,T", [("C2s", 32), ("C3s", 16), ("C1", 8)])

@@ -38,7 +38,7 @@ def parse():
     ap.add_argument("--size", type=int, default=0, help="cube size for the configs[3] sweep")
     ap.add_argument("--tile", default="", help="NXxNYxNZ systolic tile (default: library choice)")
     ap.add_argument("--T", type=int, default=0, help="temporal depth (default: library choice)")
-    ap.add_argument("--variant", default="fma", choices=["fma", "nofma"])
+    ap.add_argument("--variant", default="fma", choices=["fma", "nofma", "prof"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()

@@ -14,6 +14,8 @@ HEADERS = ["fdtd_internal.h", "fdtd_types.h", "yee_update.h", "systolic_tile.cuh
 LIBS = {
     "fma": (os.path.join(HERE, "libfdtd_b200.so"), []),
     "nofma": (os.path.join(HERE, "libfdtd_b200_nofma.so"), ["-fmad=false", "-DFDTD_NOFMA"]),
+    # developer build: clock64 section timers inside the systolic kernel, dumped to stderr by fdtd_destroy
+    "prof": (os.path.join(HERE, "libfdtd_b200_prof.so"), ["-DFDTD_PROFILE"]),
 }
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

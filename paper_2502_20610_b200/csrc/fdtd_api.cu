@@ -42,6 +42,7 @@ struct fdtd_ctx {
     size_t flags_cap;
     unsigned int* d_counter;
     int* d_abort;
+    long long* d_prof;   // FDTD_PROFILE build only
     int flag_base;
     long long spin_budget;
     unsigned int delay_seed;
@@ -291,6 +292,7 @@ int step_systolic(fdtd_ctx* c, int n)
         P.abort_flag = c->d_abort;
         P.spin_budget = c->spin_budget;
         P.delay_seed = c->delay_seed;
+        P.prof = c->d_prof;
         P.dbg = getenv("FDTD_DEBUG_SKIP") ? atoi(getenv("FDTD_DEBUG_SKIP")) : 0;
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
@@ -381,6 +383,7 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->flags_cap = 0;
     c->d_counter = nullptr;
     c->d_abort = nullptr;
+    c->d_prof = nullptr;
     c->flag_base = 0;
     c->delay_seed = 0;
     c->device = dev;
@@ -395,6 +398,10 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     e = cudaMalloc(&c->d_counter, sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_abort, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(c->d_abort, 0, sizeof(int));
+#ifdef FDTD_PROFILE
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_prof, 32 * sizeof(long long));
+    if (e == cudaSuccess) e = cudaMemset(c->d_prof, 0, 32 * sizeof(long long));
+#endif
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
     if (e != cudaSuccess) {
@@ -664,6 +671,15 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->d_flags) cudaFree(c->d_flags);
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);
+    if (c->d_prof) {
+        long long h[32];
+        if (cudaMemcpy(h, c->d_prof, sizeof h, cudaMemcpyDeviceToHost) == cudaSuccess) {
+            fprintf(stderr, "fdtd profile (clock64 ticks summed over CTAs):");
+            for (int i = 0; i < 32; ++i) fprintf(stderr, "%s%lld", i % 8 == 0 ? "\n  " : " ", h[i]);
+            fprintf(stderr, "\n");
+        }
+        cudaFree(c->d_prof);
+    }
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     delete c;

@@ -282,6 +282,19 @@ __device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, 
 }
 
 // ---- compute warps ---------------------------------------------------------------------------------------------
+// FDTD_PROFILE build only: lane 0 of compute warp 0 accumulates clock64 ticks per section of the step into
+// P.prof[0..7] (wait HREADY+absorb, barrier, E phase+publish, wait SIGACK, wait EREADY, absorb+barrier, H phase+publish,
+// steps); aux warps add theirs to P.prof[8..].
+#ifdef FDTD_PROFILE
+#define PROF_DECL long long pt_ = clock64(), pacc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
+#define PROF_MARK(i) do { const long long n_ = clock64(); pacc_[i] += n_ - pt_; pt_ = n_; } while (0)
+#define PROF_FLUSH(base) do { if ((threadIdx.x & 31) == 0 && P.prof) for (int i_ = 0; i_ < 8; ++i_) atomicAdd((unsigned long long*)P.prof + (base) + i_, (unsigned long long)pacc_[i_]); } while (0)
+#else
+#define PROF_DECL
+#define PROF_MARK(i)
+#define PROF_FLUSH(base)
+#endif
+
 struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
     unsigned hready, eready, sigack;
 };
@@ -320,8 +333,10 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     for (int l = 0; l < BZ; ++l) hx[l] = hy[l] = hz[l] = 0.0f;
 
     const int T = P.T;
+    PROF_DECL;
     for (int k = 0; k < T; ++k) {
         const bool last = (k == T - 1);
+        PROF_MARK(7);
         const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
         const int lx = (lane - o0) & (BX - 1), ly = (wy - o1) & (BY - 1);
         const int gx = o0 + lx, gy = o1 + ly;
@@ -388,8 +403,10 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
             warp_arrive(mb + MB_HFREE);
         }
+        PROF_MARK(0);
         bar_sync(1, NCOMPUTE);   // exchange rows of H (shell + last H phase) and the scattered coefficients are visible
 
+        PROF_MARK(1);
         // ---------------- E phase on R_k = [1,w]^3 (a1): every slot computes, shell slots produce garbage ----
 #pragma unroll
         for (int l = BZ - 1; l >= 1; --l) {
@@ -459,6 +476,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 }
             }
         }
+        PROF_MARK(2);
         if (k > 0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it
             mbar_wait(mb + MB_SIGACK, ph.sigack & 1u);
             ++ph.sigack;
@@ -467,8 +485,10 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);
 
         // ---------------- E minus shell -------------------------------------------------------------------------
+        PROF_MARK(3);
         mbar_wait(mb + MB_EREADY, ph.eready & 1u);
         ++ph.eready;
+        PROF_MARK(4);
         {
             const int zi = ly * RX + (o0 & 3) + lx;
             ex[1] = stgE[0 * ST_ARR + zi];
@@ -494,6 +514,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         }
         warp_arrive(mb + MB_EFREE);
         bar_sync(1, NCOMPUTE);   // exchange rows of E are visible
+        PROF_MARK(5);
 
         // ---------------- H phase on R_{k+1} = [0,w-1]^3 (a2): every slot computes ----------------------------
 #pragma unroll
@@ -524,7 +545,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         }
         warp_arrive(mb + MB_HDONE);
         if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);
+        PROF_MARK(6);
     }
+    if (threadIdx.x < 32) PROF_FLUSH(0);
     // the signal warp's last ack of this tile is covered by the CTA barrier at the tile boundary
     ++ph.sigack;
 }
@@ -573,11 +596,15 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         } else if (warp == W_HPROD || warp == W_HAUX) {
             // H side: shell of step k needs the staging of step k-1 absorbed (HFREE), the upwind tiles' H of
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
+            PROF_DECL;
             for (int k = 1; k < T; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                PROF_MARK(7);
                 if (warp == W_HPROD) {
                     if (k >= 2) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
+                    PROF_MARK(0);
                     wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
+                    PROF_MARK(1);
                     if (lane == 0 && !(P.dbg & 2)) {
                         fence_proxy_async();
                         issue_shell(maps + 3 * 3, 3, sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
@@ -585,15 +612,21 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     }
                     __syncwarp();
                 }
+                PROF_MARK(2);
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
+                PROF_MARK(3);
                 if (!(P.dbg & 2)) {
                     mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull;
                     if (COEF) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
                 }
-                scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
+                PROF_MARK(4);
+                if (!(P.dbg & 16)) scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
+                PROF_MARK(5);
                 pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1, warp - W_HPROD, 2);
                 warp_arrive(mb + MB_HREADY);
+                PROF_MARK(6);
             }
+            if (warp == W_HPROD) PROF_FLUSH(8);
             if (T >= 2) ++n_hfree;        // the last absorb's HFREE phase: covered by the CTA barrier at the tile boundary
             ++n_edone;                    // EDONE(T-1) likewise
         } else if (warp == W_EPROD) {

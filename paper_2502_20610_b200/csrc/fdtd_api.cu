@@ -31,6 +31,7 @@ struct fdtd_ctx {
     bool use_reg;     // resolved: the register-resident kernel (tile 31x15x7) runs
     bool use_tma;     // resolved: its TMA-staged version runs (PEC grids, nx % 4 == 0)
     TmaMaps tmaps;    // 36 CUtensorMap: [E0..2 H0..2 ca0..2 cb0..2][z plane, y row, x column]
+    int tma_group[3]; // per group (E, H, coefficients): 0 per-array maps, 1 one 4-D map per piece, 2 two triples
     bool tmaps_valid;
     bool resolved;
     int N[3];         // resolved tile
@@ -211,22 +212,56 @@ int ensure_tmaps(fdtd_ctx* c)
     static_assert(sizeof(CUtensorMap) * 36 == sizeof(TmaMaps), "TmaMaps layout");
     CUtensorMap* host = reinterpret_cast<CUtensorMap*>(c->tmaps.bytes);
     memset(c->tmaps.bytes, 0, sizeof c->tmaps.bytes);
-    const cuuint64_t dims[3] = {(cuuint64_t)c->g.n[0], (cuuint64_t)c->g.n[1], (cuuint64_t)c->g.n[2]};
-    const cuuint64_t strides[2] = {(cuuint64_t)c->g.n[0] * 4u, (cuuint64_t)c->g.n[0] * c->g.n[1] * 4u};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    for (int a = 0; a < 12; ++a) {
-        if (!arr[a]) continue;
+    const cuuint64_t nbytes = (cuuint64_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * 4u;
+    // arrays first..first+count-1 at one positive stride (multiple of 16 bytes, no overlap)? -> the stride, else 0
+    auto uniform_stride = [&](int first, int count) -> cuuint64_t {
+        if (!arr[first] || getenv("FDTD_TMA_NO_GROUP")) return 0;
+        const char* b0 = (const char*)arr[first];
+        const char* b1 = (const char*)arr[first + 1];
+        if (b1 <= b0) return 0;
+        const cuuint64_t d = (cuuint64_t)(b1 - b0);
+        if (d < nbytes || (d & 15u) || d >= (1ull << 40)) return 0;
+        for (int a = 2; a < count; ++a)
+            if ((const char*)arr[first + a] != b0 + d * a) return 0;
+        return d;
+    };
+    auto encode_maps = [&](CUtensorMap* dst, const void* base, int narr, cuuint64_t astride) -> int {
+        const cuuint64_t dims[4] = {(cuuint64_t)c->g.n[0], (cuuint64_t)c->g.n[1], (cuuint64_t)c->g.n[2], (cuuint64_t)narr};
+        const cuuint64_t strides[3] = {(cuuint64_t)c->g.n[0] * 4u, (cuuint64_t)c->g.n[0] * c->g.n[1] * 4u, astride};
+        const cuuint32_t estr[4] = {1, 1, 1, 1};
         for (int f = 0; f < 3; ++f) {
-            const cuuint32_t b[3] = {(cuuint32_t)box[f][0], (cuuint32_t)box[f][1], (cuuint32_t)box[f][2]};
-            const CUresult r = encode(&host[a * 3 + f], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<void*>(arr[a]), dims, strides, b, estr,
+            const cuuint32_t b[4] = {(cuuint32_t)box[f][0], (cuuint32_t)box[f][1], (cuuint32_t)box[f][2], (cuuint32_t)narr};
+            const CUresult r = encode(dst + f, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, narr > 1 ? 4 : 3, const_cast<void*>(base), dims, strides, b, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) {
                 char buf[96];
-                snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d) for array %d piece %d", (int)r, a, f);
+                snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (CUresult %d), %d array(s), piece %d", (int)r, narr, f);
                 return fail(c, FDTD_ECUDA, buf);
             }
         }
+        return FDTD_OK;
+    };
+    // groups: E = arrays 0..2 (slot 0), H = 3..5 (slot 9), coefficients = 6..11 (slot 18)
+    const int first[3] = {0, 3, 6}, count[3] = {3, 3, 6};
+    for (int g = 0; g < 3; ++g) {
+        c->tma_group[g] = 0;
+        if (!arr[first[g]]) continue;
+        CUtensorMap* dst = host + first[g] * 3;
+        int rc = FDTD_OK;
+        cuuint64_t d = uniform_stride(first[g], count[g]);
+        cuuint64_t da = 0, db = 0;
+        if (d) {
+            c->tma_group[g] = 1;
+            rc = encode_maps(dst, arr[first[g]], count[g], d);
+        } else if (g == 2 && (da = uniform_stride(6, 3)) && (db = uniform_stride(9, 3))) {
+            c->tma_group[g] = 2;
+            rc = encode_maps(dst, arr[6], 3, da);
+            if (rc == FDTD_OK) rc = encode_maps(dst + 9, arr[9], 3, db);
+        } else {
+            for (int a = 0; a < count[g] && rc == FDTD_OK; ++a) rc = encode_maps(dst + a * 3, arr[first[g] + a], 1, 0);
+        }
+        if (rc != FDTD_OK) return rc;
     }
     c->tmaps_valid = true;
     return FDTD_OK;
@@ -293,6 +328,7 @@ int step_systolic(fdtd_ctx* c, int n)
         P.spin_budget = c->spin_budget;
         P.delay_seed = c->delay_seed;
         P.prof = c->d_prof;
+        for (int g = 0; g < 3; ++g) P.tma_group[g] = c->tma_group[g];
         P.dbg = getenv("FDTD_DEBUG_SKIP") ? atoi(getenv("FDTD_DEBUG_SKIP")) : 0;
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");

@@ -53,24 +53,28 @@ constexpr int W_HPROD = 16, W_HAUX = 17, W_EPROD = 18;   // warp 19: signal
 // staging of one array's minus shell (floats); every TMA destination is 128-byte aligned
 // TMA needs the innermost start coordinate on a 16-byte boundary, the shell slides by one cell per step: every
 // box starts at q0 = o0 & ~3 and is RX = 36 cells wide; r0 = o0 & 3 is where the shell begins inside a staged row
+// Box extents are chosen so that every piece is a multiple of 128 bytes: a group of arrays at uniform stride can
+// then be fetched by ONE 4-D box per piece and lands exactly where per-array 3-D boxes would put it.
 constexpr int RX = BX + 4;
-constexpr int ST_Z = RX * BY;                // box (36,16,1)   [y][x]      576 floats
-constexpr int ST_YRAW = RX * W2;             // box (36,1,7)    [z][x]      252 floats
-constexpr int ST_Y = 256;                    // padded to a multiple of 32 floats
-constexpr int ST_XRAW = 4 * W1 * W2;         // box (4,15,7)    [z][y][4]   (only x index r0 is used)
-constexpr int ST_X = 448;                    // ST_XRAW = 420 padded to a multiple of 32 floats
-constexpr int ST_ARR = ST_Z + ST_Y + ST_X;   // 1280 floats
+constexpr int FZ = RX * BY;                  // box (36,16,1)   [y][x]      576 floats: plane l_z = 0
+constexpr int FY = RX * BZ;                  // box (36,1,8)    [z][x]      288 floats: row l_y = 0, l_z = 1..8 (8 unused)
+constexpr int FX = 4 * BY * W2;              // box (4,16,7)    [z][y][4]   448 floats: column l_x = 0 (x index r0), l_y = 0..15, l_z = 1..7
+constexpr int F_ARR = FZ + FY + FX;          // 1312 floats per array and step
+// a staged group of NA arrays: [NA][FZ] [NA][FY] [NA][FX]
+template <int NA> __device__ __forceinline__ int zidx(int a, int ly, int x) { return a * FZ + ly * RX + x; }
+template <int NA> __device__ __forceinline__ int yidx(int a, int l, int x) { return NA * FZ + a * FY + (l - 1) * RX + x; }
+template <int NA> __device__ __forceinline__ int xidx(int a, int ly, int l) { return NA * (FZ + FY) + a * FX + ((l - 1) * BY + ly) * 4; }
 constexpr int XPK = BY * 3 * 8;              // packed x column [y slot][component][8]
 constexpr int EXP = 7 * PLANE;               // one exchange array: 7 planes of (x,y) slots
-constexpr unsigned BYTES_ARR = (ST_Z + ST_YRAW + ST_XRAW) * 4u;   // bytes TMA delivers per array and step
+constexpr unsigned BYTES_ARR = F_ARR * 4u;   // bytes TMA delivers per array and step
 
 template <bool COEF>
 struct Lay {
     static constexpr int NC = COEF ? 6 : 3;            // resident coefficient arrays (no COEF: cb masks only)
     static constexpr int stgh = 0;
-    static constexpr int stge = stgh + 3 * ST_ARR;
-    static constexpr int stgc = stge + 3 * ST_ARR;
-    static constexpr int xpkh = stgc + (COEF ? 6 * ST_ARR : 0);
+    static constexpr int stge = stgh + 3 * F_ARR;
+    static constexpr int stgc = stge + 3 * F_ARR;
+    static constexpr int xpkh = stgc + (COEF ? 6 * F_ARR : 0);
     static constexpr int xpke = xpkh + XPK;
     static constexpr int exch = xpke + XPK;            // exHz, exHx, exEz, exEx
     static constexpr int coef = exch + 4 * EXP;
@@ -212,73 +216,116 @@ __device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k,
     if ((h & 3u) == 0u) __nanosleep((h >> 8) & 0x3fffu);   // up to ~16 us, one phase in four
 }
 
-// one lane issues the three boxes of `narr` consecutive tensor maps (maps[arr*3 + face]) for the box of step k
-__device__ __forceinline__ void issue_shell(const CUtensorMap* maps, int narr, float* stg, int o0, int o1, int o2, unsigned long long* bar)
+__device__ __forceinline__ void tma_load_4d(float* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(smem_u32(dst)),
+                 "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// One lane issues the minus shell of step k for a group of NA arrays into stg = [NA][FZ] [NA][FY] [NA][FX].
+// grouped == 1: the arrays sit at a uniform stride and maps[0..2] are 4-D (x, y, z, array) maps, one box per piece;
+// grouped == 2 (NA = 6): two such triples (maps[0..2], maps[9..11]); grouped == 0: per-array 3-D maps maps[a*3 + piece].
+template <int NA>
+__device__ __forceinline__ void issue_shell(const CUtensorMap* maps, int grouped, float* stg, int o0, int o1, int o2, unsigned long long* bar)
 {
     const int q0 = o0 & ~3;
-    mbar_expect_tx(bar, (unsigned)narr * BYTES_ARR);
-    for (int a = 0; a < narr; ++a) {
-        float* d = stg + a * ST_ARR;
-        tma_load_3d(d, maps + a * 3 + 0, q0, o1, o2, bar);                      // z plane l_z = 0
-        tma_load_3d(d + ST_Z, maps + a * 3 + 1, q0, o1, o2 + 1, bar);           // y row   l_y = 0, l_z = 1..7
-        tma_load_3d(d + ST_Z + ST_Y, maps + a * 3 + 2, q0, o1 + 1, o2 + 1, bar);   // x column l_x = 0, l_y = 1..15, l_z = 1..7
+    mbar_expect_tx(bar, (unsigned)NA * BYTES_ARR);
+    float* dz = stg;
+    float* dy = stg + NA * FZ;
+    float* dx = stg + NA * (FZ + FY);
+    if (grouped == 1) {
+        tma_load_4d(dz, maps + 0, q0, o1, o2, 0, bar);
+        tma_load_4d(dy, maps + 1, q0, o1, o2 + 1, 0, bar);
+        tma_load_4d(dx, maps + 2, q0, o1, o2 + 1, 0, bar);
+    } else if (grouped == 2) {
+        for (int h = 0; h < 2; ++h) {
+            tma_load_4d(dz + h * 3 * FZ, maps + h * 9 + 0, q0, o1, o2, 0, bar);
+            tma_load_4d(dy + h * 3 * FY, maps + h * 9 + 1, q0, o1, o2 + 1, 0, bar);
+            tma_load_4d(dx + h * 3 * FX, maps + h * 9 + 2, q0, o1, o2 + 1, 0, bar);
+        }
+    } else {
+        for (int a = 0; a < NA; ++a) {
+            tma_load_3d(dz + a * FZ, maps + a * 3 + 0, q0, o1, o2, bar);          // z plane  l_z = 0
+            tma_load_3d(dy + a * FY, maps + a * 3 + 1, q0, o1, o2 + 1, bar);      // y row    l_y = 0, l_z = 1..
+            tma_load_3d(dx + a * FX, maps + a * 3 + 2, q0, o1, o2 + 1, bar);      // x column l_x = 0, l_y = 0.., l_z = 1..7
+        }
     }
 }
 
-// ---- H-side auxiliary warps: coefficients of the entering cells -> the owner threads' private slots ----------
-// part / 2 splits the work between warps 16 and 17.  COEF: values come from the staged arrays (ca 0..2, cb 3..5)
-// and frozen wall components become (1, 0); no COEF: the three cb masks are generated (dt inside, 0 frozen/outside).
+// coefficient value of component slot c (COEF: ca 0..2, cb 3..5; else cb masks 0..2) for the cell at (gx,gy,gz):
+// staged value v, except frozen wall components -> (ca, cb) = (1, 0); no COEF: dt inside the grid, else 0
+template <bool COEF>
+__device__ __forceinline__ float coef_value(const SysParams& P, int c, float v, int gx, int gy, int gz)
+{
+    if (COEF) return frozen(c % 3, gx, gy, gz) ? (c < 3 ? 1.0f : 0.0f) : v;
+    const bool in = ((unsigned)gx < (unsigned)P.g.n[0]) & ((unsigned)gy < (unsigned)P.g.n[1]) & ((unsigned)gz < (unsigned)P.g.n[2]);
+    return (in && !frozen(c, gx, gy, gz)) ? P.g.cb_scalar : 0.0f;
+}
+
+// ---- H-side auxiliary warps: coefficients of the entering row and column -> the owner threads' private slots ----
+// (the entering plane l_z = 0 is absorbed by the compute threads themselves).  Warp part 0 takes the row l_y = 0,
+// part 1 the column l_x = 0; loads of a batch are issued before its stores.
 template <bool COEF>
 __device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int o0, int o1, int o2, int part)
 {
     constexpr int NC = Lay<COEF>::NC;
     const int lane = threadIdx.x & 31;
-    const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
     const float* stg = sm + Lay<COEF>::stgc;
     float* coef = sm + Lay<COEF>::coef;
-    const bool walls = (o0 <= 0) | (o1 <= 0) | (o2 <= 0);   // the box touches a low wall: fix-ups needed
     const int r0 = o0 & 3;
-    const float dt = P.g.cb_scalar;
-
-    auto put = [&](int c, int src, int lx, int ly, int l) {
-        const int gx = o0 + lx, gy = o1 + ly, gz = o2 + l;
-        float v;
-        if (COEF) {
-            v = stg[c * ST_ARR + src];
-            if (walls && frozen(c % 3, gx, gy, gz)) v = c < 3 ? 1.0f : 0.0f;
-        } else {
-            const bool in = ((unsigned)gx < (unsigned)nx) & ((unsigned)gy < (unsigned)ny) & ((unsigned)gz < (unsigned)nz);
-            v = (in && !frozen(c, gx, gy, gz)) ? dt : 0.0f;
+    if (part == 0) {
+        const int gx = o0 + lane, gy = o1;
+        float* dst = coef + (gy & (BY - 1)) * BX + (gx & (BX - 1));
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            float v[BZ];
+#pragma unroll
+            for (int l = 1; l < BZ; ++l) v[l] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
+#pragma unroll
+            for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_value<COEF>(P, c, v[l], gx, gy, o2 + l);
         }
-        coef[(c * BZ + (gz & (BZ - 1))) * PLANE + (gy & (BY - 1)) * BX + (gx & (BX - 1))] = v;
-    };
-
-    int task = part;
-    for (int c = 0; c < NC; ++c) {
-        for (int j = 0; j < BY; ++j, ++task)          // z plane: rows l_y = j
-            if (task & 1) put(c, j * RX + r0 + lane, lane, j, 0);
-        for (int l = 1; l < BZ; ++l, ++task)          // y row: l_z = l
-            if (task & 1) put(c, ST_Z + (l - 1) * RX + r0 + lane, lane, 0, l);
-        for (int r = 0; r < 4; ++r, ++task) {         // x column: 105 cells, (l_z-1)*15 + (l_y-1)
-            const int idx = r * 32 + lane;
-            if ((task & 1) && idx < W1 * W2) put(c, ST_Z + ST_Y + idx * 4 + r0, 0, 1 + idx % W1, 1 + idx / W1);
+    } else {
+        const int xs = o0 & (BX - 1);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            float v[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {            // 105 cells: idx = (l-1)*15 + (ly-1)
+                const int idx = r * 32 + lane;
+                const int ly = 1 + idx % W1, l = 1 + idx / W1;
+                v[r] = (COEF && idx < W1 * W2) ? stg[xidx<6>(c, ly, l) + r0] : 0.0f;
+            }
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int idx = r * 32 + lane;
+                const int ly = 1 + idx % W1, l = 1 + idx / W1;
+                if (idx < W1 * W2)
+                    coef[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE + ((o1 + ly) & (BY - 1)) * BX + xs] = coef_value<COEF>(P, c, v[r], o0, o1 + ly, o2 + l);
+            }
         }
     }
 }
 
 // x column of the three field arrays in `stg` -> xpk[(y slot*3 + c)*8 + l], l = 1..7 (16-byte rows for the owner lane)
-__device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, int o1, int part, int nparts)
+__device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, int o1)
 {
     const int lane = threadIdx.x & 31;
-    int task = 0;
-    for (int c = 0; c < 3; ++c)
-        for (int r = 0; r < 4; ++r, ++task) {
+    const int r0 = o0 & 3;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        float v[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
             const int idx = r * 32 + lane;
-            if (task % nparts == part && idx < W1 * W2) {
-                const int ly = 1 + idx % W1, l = 1 + idx / W1;
-                xpk[(((o1 + ly) & (BY - 1)) * 3 + c) * 8 + l] = stg[c * ST_ARR + ST_Z + ST_Y + idx * 4 + (o0 & 3)];
-            }
+            v[r] = idx < W1 * W2 ? stg[xidx<3>(c, 1 + idx % W1, 1 + idx / W1) + r0] : 0.0f;
         }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int idx = r * 32 + lane;
+            if (idx < W1 * W2) xpk[(((o1 + 1 + idx % W1) & (BY - 1)) * 3 + c) * 8 + 1 + idx / W1] = v[r];
+        }
+    }
 }
 
 // ---- compute warps ---------------------------------------------------------------------------------------------
@@ -380,17 +427,34 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         } else {
             mbar_wait(mb + MB_HREADY, ph.hready & 1u);
             ++ph.hready;
-            const int zi = ly * RX + (o0 & 3) + lx;
-            hx[0] = stgH[0 * ST_ARR + zi];
-            hy[0] = stgH[1 * ST_ARR + zi];
-            hz[0] = stgH[2 * ST_ARR + zi];
+            const int xs = (o0 & 3) + lx;     // position inside a staged row
+            hx[0] = stgH[zidx<3>(0, ly, xs)];
+            hy[0] = stgH[zidx<3>(1, ly, xs)];
+            hz[0] = stgH[zidx<3>(2, ly, xs)];
+            {   // coefficients of the entering plane l_z = 0 -> this thread's private slots
+                float* cs = coef + (o2 & (BZ - 1)) * PLANE;
+                if (COEF) {
+                    const float* sc = sm + Lay<COEF>::stgc;
+                    float v[6];
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) v[c] = sc[zidx<6>(c, ly, xs)];
+                    if ((o0 <= 0) | (o1 <= 0) | (o2 <= 0)) {   // CTA-uniform: the box touches a low wall
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) v[c] = coef_value<COEF>(P, c, v[c], gx, gy, o2);
+                    }
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) cs[c * (BZ * PLANE)] = v[c];
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) cs[c * (BZ * PLANE)] = coef_value<COEF>(P, c, 0.0f, gx, gy, o2);
+                }
+            }
             if (ly == 0) {            // warp-uniform: the entering row; its y+1 neighbours read it from the exchange
-                const float* sy = stgH + ST_Z + (o0 & 3) + lx;
 #pragma unroll
                 for (int l = 1; l < BZ; ++l) {
-                    hx[l] = sy[0 * ST_ARR + (l - 1) * RX];
-                    hy[l] = sy[1 * ST_ARR + (l - 1) * RX];
-                    hz[l] = sy[2 * ST_ARR + (l - 1) * RX];
+                    hx[l] = stgH[yidx<3>(0, l, xs)];
+                    hy[l] = stgH[yidx<3>(1, l, xs)];
+                    hz[l] = stgH[yidx<3>(2, l, xs)];
                     exHz[(l - 1) * PLANE + slot] = hz[l];
                     exHx[(l - 1) * PLANE + slot] = hx[l];
                 }
@@ -464,15 +528,22 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         }
         // publish E of R_k \ R_{k+1} (everything at the last step)                                      (a8, a6)
         if (actE && col_in && !(P.dbg & 4)) {
-            const bool whole = last | (lx == W0) | (ly == W1);
+            if ((unsigned)(o2 + W2) < (unsigned)nz) {            // the leaving plane l = 7: every column
+                const long long off = col_off + plane * (o2 + W2);
+                __stcg(Ex + off, ex[W2 + 1]);
+                __stcg(Ey + off, ey[W2 + 1]);
+                __stcg(Ez + off, ez[W2 + 1]);
+            }
+            if (last | (lx == W0) | (ly == W1)) {                // leaving column / row: planes 1..6 as well
+                long long off = col_off + plane * (o2 + 1);
 #pragma unroll
-            for (int l = 1; l < BZ; ++l) {
-                const int gz = o2 + l;
-                if ((whole || l == W2) && (unsigned)gz < (unsigned)nz) {
-                    const long long off = col_off + plane * gz;
-                    __stcg(Ex + off, ex[l + 1]);
-                    __stcg(Ey + off, ey[l + 1]);
-                    __stcg(Ez + off, ez[l + 1]);
+                for (int l = 1; l < W2; ++l) {
+                    if ((unsigned)(o2 + l) < (unsigned)nz) {
+                        __stcg(Ex + off, ex[l + 1]);
+                        __stcg(Ey + off, ey[l + 1]);
+                        __stcg(Ez + off, ez[l + 1]);
+                    }
+                    off += plane;
                 }
             }
         }
@@ -490,19 +561,18 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         ++ph.eready;
         PROF_MARK(4);
         {
-            const int zi = ly * RX + (o0 & 3) + lx;
-            ex[1] = stgE[0 * ST_ARR + zi];
-            ey[1] = stgE[1 * ST_ARR + zi];
-            ez[1] = stgE[2 * ST_ARR + zi];
+            const int xs = (o0 & 3) + lx;
+            ex[1] = stgE[zidx<3>(0, ly, xs)];
+            ey[1] = stgE[zidx<3>(1, ly, xs)];
+            ez[1] = stgE[zidx<3>(2, ly, xs)];
             exEz[slot] = ez[1];
             exEx[slot] = ex[1];
             if (ly == 0) {
-                const float* sy = stgE + ST_Z + (o0 & 3) + lx;
 #pragma unroll
                 for (int l = 1; l < BZ; ++l) {
-                    ex[l + 1] = sy[0 * ST_ARR + (l - 1) * RX];
-                    ey[l + 1] = sy[1 * ST_ARR + (l - 1) * RX];
-                    ez[l + 1] = sy[2 * ST_ARR + (l - 1) * RX];
+                    ex[l + 1] = stgE[yidx<3>(0, l, xs)];
+                    ey[l + 1] = stgE[yidx<3>(1, l, xs)];
+                    ez[l + 1] = stgE[yidx<3>(2, l, xs)];
                 }
             } else if (lx == 0) {
                 const float4* s4 = reinterpret_cast<const float4*>(xpkE + wy * 24);
@@ -531,15 +601,22 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         }
         // publish H of R_{k+1} \ R_{k+2} (everything at the last step)                                  (a8, a6)
         if ((lx <= W0 - 1) & (ly <= W1 - 1) && col_in && !(P.dbg & 4)) {
-            const bool whole = last | (lx == W0 - 1) | (ly == W1 - 1);
+            if ((unsigned)(o2 + W2 - 1) < (unsigned)nz) {        // the leaving plane l = 6: every column
+                const long long off = col_off + plane * (o2 + W2 - 1);
+                __stcg(Hx + off, hx[W2]);
+                __stcg(Hy + off, hy[W2]);
+                __stcg(Hz + off, hz[W2]);
+            }
+            if (last | (lx == W0 - 1) | (ly == W1 - 1)) {        // leaving column / row: planes 0..5 as well
+                long long off = col_off + plane * o2;
 #pragma unroll
-            for (int l = 0; l < BZ - 1; ++l) {
-                const int gz = o2 + l;
-                if ((whole || l == W2 - 1) && (unsigned)gz < (unsigned)nz) {
-                    const long long off = col_off + plane * gz;
-                    __stcg(Hx + off, hx[l + 1]);
-                    __stcg(Hy + off, hy[l + 1]);
-                    __stcg(Hz + off, hz[l + 1]);
+                for (int l = 0; l < W2 - 1; ++l) {
+                    if ((unsigned)(o2 + l) < (unsigned)nz) {
+                        __stcg(Hx + off, hx[l + 1]);
+                        __stcg(Hy + off, hy[l + 1]);
+                        __stcg(Hz + off, hz[l + 1]);
+                    }
+                    off += plane;
                 }
             }
         }
@@ -607,8 +684,8 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     PROF_MARK(1);
                     if (lane == 0 && !(P.dbg & 2)) {
                         fence_proxy_async();
-                        issue_shell(maps + 3 * 3, 3, sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
-                        if (COEF) issue_shell(maps + 6 * 3, 6, sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
+                        if (COEF) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                     }
                     __syncwarp();
                 }
@@ -622,7 +699,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 PROF_MARK(4);
                 if (!(P.dbg & 16)) scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
                 PROF_MARK(5);
-                pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1, warp - W_HPROD, 2);
+                if (warp == W_HAUX) pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
                 warp_arrive(mb + MB_HREADY);
                 PROF_MARK(6);
             }
@@ -634,19 +711,19 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                 if (k >= 1) {
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
-                    mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;     // H phase k-1 has read the E exchange rows
                 }
                 wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
                 if (!(P.dbg & 2)) {
                     if (lane == 0) {
                         fence_proxy_async();
-                        issue_shell(maps, 3, sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
+                        issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
                     }
                     __syncwarp();
                     mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull;
                 }
                 const float* stg = sm + Lay<COEF>::stge;
-                pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1, 0, 1);
+                pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
+                if (k >= 1) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
                 // the shell column's Ez, Ex of planes 1..6 for its y-1 readers in the H phase
                 float* exEz = sm + Lay<COEF>::exch + 2 * EXP;
                 float* exEx = exEz + EXP;
@@ -655,8 +732,8 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     if (idx < W1 * (W2 - 1)) {
                         const int ly = 1 + idx % W1, l = 1 + idx / W1;
                         const int s = ((o1 + ly) & (BY - 1)) * BX + (o0 & (BX - 1));
-                        exEz[l * PLANE + s] = stg[2 * ST_ARR + ST_Z + ST_Y + idx * 4 + (o0 & 3)];
-                        exEx[l * PLANE + s] = stg[0 * ST_ARR + ST_Z + ST_Y + idx * 4 + (o0 & 3)];
+                        exEz[l * PLANE + s] = stg[xidx<3>(2, ly, l) + (o0 & 3)];
+                        exEx[l * PLANE + s] = stg[xidx<3>(0, ly, l) + (o0 & 3)];
                     }
                 }
                 warp_arrive(mb + MB_EREADY);
@@ -689,7 +766,7 @@ size_t systolic_tma_smem(int coef) { return (size_t)(coef ? Lay<true>::total : L
 int systolic_tma_threads() { return NT; }
 void systolic_tma_boxes(int box[3][3])
 {
-    const int b[3][3] = {{RX, BY, 1}, {RX, 1, W2}, {4, W1, W2}};
+    const int b[3][3] = {{RX, BY, 1}, {RX, 1, BZ}, {4, BY, W2}};
     for (int f = 0; f < 3; ++f)
         for (int q = 0; q < 3; ++q) box[f][q] = b[f][q];
 }

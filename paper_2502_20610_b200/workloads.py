@@ -148,6 +148,18 @@ C4_SIZES = (64, 128, 256, 512, 768, 1024)
 # ----------------------------------------------------------------------------------------------
 # fields
 # ----------------------------------------------------------------------------------------------
+def _grouped(ts):
+    """Device tensors only: the same values as views of ONE contiguous block [len(ts), nk, nj, ni].  The C ABI still
+    receives one pointer per component; at a uniform stride between them the library fetches all components of
+    a shell piece with a single 4-D TMA box (include/fdtd.h, fdtd_set_fields / fdtd_set_coeffs)."""
+    import torch
+    block = torch.empty((len(ts),) + tuple(ts[0].shape), dtype=ts[0].dtype, device=ts[0].device)
+    for q in range(len(ts)):
+        block[q].copy_(ts[q])
+        ts[q] = None
+    return [block[q] for q in range(block.shape[0])]
+
+
 def make_fields(w: Workload, window=None, device=None):
     """-> (E, H): two lists of three float32 arrays of shape (nk, nj, ni) for `window` (default whole grid).
     device=None: numpy; else torch tensors on that device (bit-identical values)."""
@@ -157,8 +169,8 @@ def make_fields(w: Workload, window=None, device=None):
         if device is None:
             return ([np.zeros(shape, np.float32) for _ in range(3)], [np.zeros(shape, np.float32) for _ in range(3)])
         import torch
-        return ([torch.zeros(shape, dtype=torch.float32, device=device) for _ in range(3)],
-                [torch.zeros(shape, dtype=torch.float32, device=device) for _ in range(3)])
+        return (list(torch.zeros((3,) + shape, dtype=torch.float32, device=device)),
+                list(torch.zeros((3,) + shape, dtype=torch.float32, device=device)))
     assert w.fields == "uniform"
     coords = (i, j, k)
     E, H = [], []
@@ -172,6 +184,8 @@ def make_fields(w: Workload, window=None, device=None):
         E.append(_to_f32(v))
         m = hash24(w.seed, AID_H[a], idx)
         H.append(_to_f32(_to_f32(m) * np.float32(2.0 ** -23) - np.float32(1.0)))
+    if device is not None:
+        E, H = _grouped(E), _grouped(H)
     return E, H
 
 
@@ -229,6 +243,9 @@ def make_coeffs(w: Workload, window=None, device=None):
         cb64 = dt * (1.0 + ca64) / (2.0 * eps[a])
         ca.append(_to_f32(ca64))
         cb.append(_to_f32(cb64))
+    if device is not None:
+        g = _grouped(ca + cb)
+        ca, cb = g[:3], g[3:]
     return ca, cb
 
 

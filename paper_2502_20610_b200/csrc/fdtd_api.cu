@@ -44,6 +44,8 @@ struct fdtd_ctx {
     unsigned int* d_counter;
     int* d_abort;
     long long* d_prof;   // FDTD_PROFILE build only
+    int* d_order;        // wavefront claim order of the TMA kernel, for order_nb[] tiles per axis
+    int order_nb[3];
     int flag_base;
     long long spin_budget;
     unsigned int delay_seed;
@@ -267,6 +269,36 @@ int ensure_tmaps(fdtd_ctx* c)
     return FDTD_OK;
 }
 
+// Claim order of the TMA kernel: tiles sorted by wavefront index bx+by+bz (ties: z, y, x).  Every upwind neighbour
+// of a tile has a smaller index, so it is claimed earlier (forward progress as with the lexicographic order), and the
+// tiles in flight at one time are mutually independent once a wavefront holds more tiles than there are CTAs.
+int ensure_order(fdtd_ctx* c, const int nb[3])
+{
+    if (c->d_order && c->order_nb[0] == nb[0] && c->order_nb[1] == nb[1] && c->order_nb[2] == nb[2]) return FDTD_OK;
+    const size_t nt = (size_t)nb[0] * nb[1] * nb[2];
+    std::vector<int> h;
+    h.reserve(nt);
+    for (int d = 0; d <= nb[0] + nb[1] + nb[2] - 3; ++d)
+        for (int z = 0; z < nb[2]; ++z) {
+            if (d - z < 0) break;
+            for (int y = 0; y < nb[1]; ++y) {
+                const int x = d - z - y;
+                if (x < 0) break;
+                if (x < nb[0]) h.push_back(x + nb[0] * (y + nb[1] * z));
+            }
+        }
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    if (c->d_order) cudaFree(c->d_order);
+    c->d_order = nullptr;
+    e = cudaMalloc(&c->d_order, nt * sizeof(int));
+    if (e != cudaSuccess) return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(order): ") + cudaGetErrorString(e));
+    e = cudaMemcpy(c->d_order, h.data(), nt * sizeof(int), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(order)");
+    for (int a = 0; a < 3; ++a) c->order_nb[a] = nb[a];
+    return FDTD_OK;
+}
+
 int step_naive(fdtd_ctx* c, int n)
 {
     for (int s = 0; s < n; ++s) {
@@ -316,6 +348,13 @@ int step_systolic(fdtd_ctx* c, int n)
             cudaError_t e = cudaMemsetAsync(c->d_flags, 0, 2 * c->flags_cap * sizeof(int), c->stream);
             if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(flags)");
             c->flag_base = 0;
+        }
+        P.order = nullptr;
+        if (c->use_tma && !getenv("FDTD_LEX_ORDER")) {
+            const int nb[3] = {P.ax[0].nb, P.ax[1].nb, P.ax[2].nb};
+            const int rc2 = ensure_order(c, nb);
+            if (rc2 != FDTD_OK) return rc2;
+            P.order = c->d_order;
         }
         P.T = T;
         P.t0 = c->t;
@@ -420,6 +459,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->d_counter = nullptr;
     c->d_abort = nullptr;
     c->d_prof = nullptr;
+    c->d_order = nullptr;
+    c->order_nb[0] = c->order_nb[1] = c->order_nb[2] = 0;
     c->flag_base = 0;
     c->delay_seed = 0;
     c->device = dev;
@@ -707,6 +748,7 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->d_flags) cudaFree(c->d_flags);
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);
+    if (c->d_order) cudaFree(c->d_order);
     if (c->d_prof) {
         long long h[32];
         if (cudaMemcpy(h, c->d_prof, sizeof h, cudaMemcpyDeviceToHost) == cudaSuccess) {

@@ -70,6 +70,7 @@ struct SysParams {
     unsigned int* counter; // tile claim counter, zeroed before the launch
     int* abort_flag;       // != 0: a watchdog fired; every CTA leaves
     long long spin_budget; // clock64 ticks a single wait may take
+    const int* order;      // systolic_tma.cu: claim index -> tile, sorted by wavefront bx+by+bz (NULL: identity)
     int tma_group[3];      // systolic_tma.cu, per group (E, H, coefficients): 0 per-array 3-D maps, 1 one 4-D map per piece, 2 two triples
     long long* prof;       // FDTD_PROFILE build: 32 tick accumulators (NULL otherwise)
     int dbg;               // debug timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes, 8 no fences

@@ -44,8 +44,9 @@ namespace {
 
 constexpr int BX = 32, BY = 16, BZ = 8;
 constexpr int W0 = BX - 1, W1 = BY - 1, W2 = BZ - 1;   // tile widths (PEC axes: always full)
-constexpr int PLANE = BX * BY;                          // 512 (x,y) slots = compute threads
-constexpr int NCOMPUTE = PLANE;
+constexpr int NCOMPUTE = BX * BY;                       // 512 (x,y) slots = compute threads
+constexpr int SX = BX + 1;                              // row stride of the slot-indexed shared arrays: a column of
+constexpr int PLANE = SX * BY;                          // slots (the entering x column) then spans 16 banks, not one
 constexpr int NWARPS_C = NCOMPUTE / 32;
 constexpr int NT = NCOMPUTE + 128;
 constexpr int W_HPROD = 16, W_HAUX = 17, W_EPROD = 18;   // warp 19: signal
@@ -276,7 +277,7 @@ __device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int 
     const int r0 = o0 & 3;
     if (part == 0) {
         const int gx = o0 + lane, gy = o1;
-        float* dst = coef + (gy & (BY - 1)) * BX + (gx & (BX - 1));
+        float* dst = coef + (gy & (BY - 1)) * SX + (gx & (BX - 1));
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             float v[BZ];
@@ -301,7 +302,7 @@ __device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int 
                 const int idx = r * 32 + lane;
                 const int ly = 1 + idx % W1, l = 1 + idx / W1;
                 if (idx < W1 * W2)
-                    coef[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE + ((o1 + ly) & (BY - 1)) * BX + xs] = coef_value<COEF>(P, c, v[r], o0, o1 + ly, o2 + l);
+                    coef[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE + ((o1 + ly) & (BY - 1)) * SX + xs] = coef_value<COEF>(P, c, v[r], o0, o1 + ly, o2 + l);
             }
         }
     }
@@ -350,8 +351,8 @@ template <bool COEF>
 __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, float* sm, unsigned long long* mb, Phases& ph)
 {
     const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
-    const int slot = wy * BX + lane;
-    const int slot_ym = ((wy - 1) & (BY - 1)) * BX + lane, slot_yp = ((wy + 1) & (BY - 1)) * BX + lane;
+    const int slot = wy * SX + lane;
+    const int slot_ym = ((wy - 1) & (BY - 1)) * SX + lane, slot_yp = ((wy + 1) & (BY - 1)) * SX + lane;
     const int lane_m = (lane - 1) & 31, lane_p = (lane + 1) & 31;
     const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
     const long long plane = (long long)nx * ny;
@@ -662,8 +663,11 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             if (ld_volatile(P.abort_flag) != 0) ctl.abort = 1;
         }
         __syncthreads();
-        const int tile = ctl.tile;
-        if (tile >= P.ntiles || ctl.abort) break;
+        if (ctl.tile >= P.ntiles || ctl.abort) break;
+        // claim order = wavefront order (P.order sorts the tiles by bx+by+bz): the tiles in flight at any time lie on
+        // one or two anti-diagonal planes and do not depend on each other, their upwind tiles were claimed a whole
+        // tile lifetime earlier -- the hand-off latency then never stalls a step
+        const int tile = P.order ? P.order[ctl.tile] : ctl.tile;
         TileGeom t;
         tile_init(P, tile, t);
         const int T = P.T;
@@ -683,7 +687,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
                     PROF_MARK(1);
                     if (lane == 0 && !(P.dbg & 2)) {
-                        fence_proxy_async();
+                        if (!(P.dbg & 32)) fence_proxy_async();
                         issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         if (COEF) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                     }
@@ -715,7 +719,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
                 if (!(P.dbg & 2)) {
                     if (lane == 0) {
-                        fence_proxy_async();
+                        if (!(P.dbg & 32)) fence_proxy_async();
                         issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
                     }
                     __syncwarp();
@@ -731,7 +735,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     const int idx = r * 32 + lane;            // (l-1)*15 + (ly-1), l = 1..6
                     if (idx < W1 * (W2 - 1)) {
                         const int ly = 1 + idx % W1, l = 1 + idx / W1;
-                        const int s = ((o1 + ly) & (BY - 1)) * BX + (o0 & (BX - 1));
+                        const int s = ((o1 + ly) & (BY - 1)) * SX + (o0 & (BX - 1));
                         exEz[l * PLANE + s] = stg[xidx<3>(2, ly, l) + (o0 & 3)];
                         exEx[l * PLANE + s] = stg[xidx<3>(0, ly, l) + (o0 & 3)];
                     }
@@ -744,13 +748,10 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             // at gpu scope, then raise the flag                                                              (a9)
             for (int k = 0; k < T; ++k) {
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
-                if (lane == 0) {
-                    if (!(P.dbg & 8)) __threadfence();
-                    st_release(P.flagE + tile, P.flag_base + k + 1);
-                }
+                // every publish of the phase happens-before its warp's arrive on EDONE; the release store is cumulative
+                if (lane == 0) st_release(P.flagE + tile, P.flag_base + k + 1);
                 mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
                 if (lane == 0) {
-                    if (!(P.dbg & 8)) __threadfence();
                     st_release(P.flagH + tile, P.flag_base + k + 1);
                     mbar_arrive(mb + MB_SIGACK);
                 }

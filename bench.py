@@ -24,6 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "TCUPS (6-component Yee cell updates/s, fp32) vs grid size; HBM GB/s"
+TMA_SMEM = (226560, 144384)     # dynamic shared memory of systolic_tma.cu with / without coefficient arrays
 
 
 def parse():
@@ -285,10 +286,15 @@ def main():
     achieved = bpc * cell_updates / (kernel_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy)" if "hbm_gbs" in peaks else "fallback 6.65 TB/s",
-                "algorithmic_bytes_per_cell_update": bpc, "kernel": "systolic_kernel" if args.kernel == "systolic" else "e_half_naive+h_half_naive",
+                "algorithmic_bytes_per_cell_update": bpc,
+                "kernel": ("systolic_tma_kernel" if info["smem"] in TMA_SMEM else "systolic_reg_kernel") if args.kernel == "systolic" else "e_half_naive+h_half_naive",
                 "launches_in_region": launches, "avg_launch_ms": kernel_ms / max(launches, 1),
                 "roof_tcups": peak * 1e9 / bpc / 1e12,
-                "fp32_roof_tcups": 148 * 128 * 2 * 1.965e9 / 45 / 1e12}
+                # explanatory ceilings of the systolic kernel: arithmetic-only issue floor (33 FMA-contracted
+                # instructions per cell), the kernel's own instruction mix at 100 % issue, the shared-memory pipe
+                "fp32_roof_tcups": 148 * 128 * 1.965e9 / 33 / 1e12,
+                "issue_roof_tcups": 148 * 128 * 1.965e9 / 118 / 1e12,
+                "smem_roof_tcups": 148 * 1.965e9 * 3255 / 2300 / 1e12}
     prof = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(prof):
         try:

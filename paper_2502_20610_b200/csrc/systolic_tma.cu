@@ -348,7 +348,7 @@ struct Phases {   // completed phases of each mbarrier as seen by this thread's 
 };
 
 template <bool COEF>
-__device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, float* sm, unsigned long long* mb, Phases& ph)
+__device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, int k0, int k1, float* sm, unsigned long long* mb, Phases& ph)
 {
     const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
     const int slot = wy * SX + lane;
@@ -382,7 +382,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 
     const int T = P.T;
     PROF_DECL;
-    for (int k = 0; k < T; ++k) {
+    for (int k = k0; k < k1; ++k) {
         const bool last = (k == T - 1);
         PROF_MARK(7);
         const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
@@ -549,7 +549,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         PROF_MARK(2);
-        if (k > 0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it
+        if (k > k0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it
             mbar_wait(mb + MB_SIGACK, ph.sigack & 1u);
             ++ph.sigack;
         }
@@ -627,7 +627,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     }
     if (threadIdx.x < 32) PROF_FLUSH(0);
     // the signal warp's last ack of this tile is covered by the CTA barrier at the tile boundary
-    ++ph.sigack;
+    if (k1 > k0) ++ph.sigack;
 }
 
 template <bool COEF>
@@ -671,18 +671,37 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         TileGeom t;
         tile_init(P, tile, t);
         const int T = P.T;
+        // a11: steps at which the tile's region lies wholly outside the grid do nothing and publish nothing.  The region
+        // [a-k, a+w-k) meets [0,n) on every axis for k in [kin, kout); the tile runs [k0, k1) = [kin-1, kout) -- one step
+        // early, because the cells of R_kin enter as the minus shell of step kin-1 -- and its flags jump over the rest.
+        int k0 = 0, k1 = T;
+        for (int q = 0; q < 3; ++q) {
+            const int wq = q == 0 ? W0 : q == 1 ? W1 : W2;
+            k0 = max(k0, t.a[q] - P.g.n[q]);          // kin - 1 = a - n
+            k1 = min(k1, t.a[q] + wq);
+        }
+        if (k1 < k0) k1 = k0;
+        if (P.dbg & 64) { k0 = 0; k1 = T; }
+        if (k0 > 0 && warp < NWARPS_C) {
+            // started late: nothing is loaded from the grid; the box holds zero fields (registers) and zero coefficients
+            float* cs = sm + Lay<COEF>::coef + (tid >> 5) * SX + lane;
+#pragma unroll
+            for (int c = 0; c < Lay<COEF>::NC * BZ; ++c) cs[c * PLANE] = 0.0f;
+        }
+        __syncthreads();
 
         if (warp < NWARPS_C) {
-            compute_tile<COEF>(P, t, tile, sm, mb, ph);
+            compute_tile<COEF>(P, t, tile, k0, k1, sm, mb, ph);
         } else if (warp == W_HPROD || warp == W_HAUX) {
             // H side: shell of step k needs the staging of step k-1 absorbed (HFREE), the upwind tiles' H of
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
             PROF_DECL;
-            for (int k = 1; k < T; ++k) {
+            const int hk0 = max(k0, 1);       // step 0 loads its whole box itself
+            for (int k = hk0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                 PROF_MARK(7);
                 if (warp == W_HPROD) {
-                    if (k >= 2) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
+                    if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                     PROF_MARK(0);
                     wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
                     PROF_MARK(1);
@@ -694,7 +713,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     __syncwarp();
                 }
                 PROF_MARK(2);
-                mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
+                if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
                 PROF_MARK(3);
                 if (!(P.dbg & 2)) {
                     mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull;
@@ -708,12 +727,12 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 PROF_MARK(6);
             }
             if (warp == W_HPROD) PROF_FLUSH(8);
-            if (T >= 2) ++n_hfree;        // the last absorb's HFREE phase: covered by the CTA barrier at the tile boundary
-            ++n_edone;                    // EDONE(T-1) likewise
+            if (k1 > hk0) ++n_hfree;      // the last absorb's HFREE phase: covered by the CTA barrier at the tile boundary
+            if (k1 > k0) ++n_edone;       // EDONE of the last step likewise
         } else if (warp == W_EPROD) {
-            for (int k = 0; k < T; ++k) {
+            for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
-                if (k >= 1) {
+                if (k > k0) {
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
                 }
                 wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
@@ -727,7 +746,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 }
                 const float* stg = sm + Lay<COEF>::stge;
                 pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
-                if (k >= 1) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
+                if (k > k0) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
                 // the shell column's Ez, Ex of planes 1..6 for its y-1 readers in the H phase
                 float* exEz = sm + Lay<COEF>::exch + 2 * EXP;
                 float* exEx = exEz + EXP;
@@ -742,11 +761,16 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 }
                 warp_arrive(mb + MB_EREADY);
             }
-            ++n_efree; ++n_hdone;         // phases of step T-1: covered by the CTA barrier at the tile boundary
+            if (k1 > k0) { ++n_efree; ++n_hdone; }   // phases of the last step: covered by the CTA barrier at the tile boundary
         } else {
             // signal warp: every publish of the phase has been issued before its warp arrived; make them visible
             // at gpu scope, then raise the flag                                                              (a9)
-            for (int k = 0; k < T; ++k) {
+            // steps before k0 publish nothing: their flags are raised at once
+            if (k0 > 0 && lane == 0) {
+                st_release(P.flagE + tile, P.flag_base + k0);
+                st_release(P.flagH + tile, P.flag_base + k0);
+            }
+            for (int k = k0; k < k1; ++k) {
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
                 // every publish of the phase happens-before its warp's arrive on EDONE; the release store is cumulative
                 if (lane == 0) st_release(P.flagE + tile, P.flag_base + k + 1);
@@ -756,6 +780,11 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     mbar_arrive(mb + MB_SIGACK);
                 }
                 __syncwarp();
+            }
+            // ... and so do the steps after the region has left the grid
+            if (k1 < T && lane == 0) {
+                st_release(P.flagE + tile, P.flag_base + T);
+                st_release(P.flagH + tile, P.flag_base + T);
             }
         }
     }

@@ -24,7 +24,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "TCUPS (6-component Yee cell updates/s, fp32) vs grid size; HBM GB/s"
-TMA_SMEM = (226560, 144384)     # dynamic shared memory of systolic_tma.cu with / without coefficient arrays
+TMA_SMEM = (229632, 147456)     # dynamic shared memory of systolic_tma.cu with / without coefficient arrays
 
 
 def parse():

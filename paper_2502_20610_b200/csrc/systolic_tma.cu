@@ -77,7 +77,9 @@ struct Lay {
     static constexpr int stgc = stge + 3 * F_ARR;
     static constexpr int xpkh = stgc + (COEF ? 6 * F_ARR : 0);
     static constexpr int xpke = xpkh + XPK;
-    static constexpr int exch = xpke + XPK;            // exHz, exHx, exEz, exEx
+    static constexpr int xoute = xpke + XPK;           // leaving x column of E, [y slot][component][8], stored by the signal warp
+    static constexpr int xouth = xoute + XPK;
+    static constexpr int exch = xouth + XPK;           // exHz, exHx, exEz, exEx
     static constexpr int coef = exch + 4 * EXP;
     static constexpr int total = coef + NC * BZ * PLANE;
 };
@@ -329,6 +331,29 @@ __device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, 
     }
 }
 
+// signal warp: the leaving x column (global x = gx) of three field arrays, rows ly = ly_lo..ly_hi, six planes starting
+// at local plane l_lo, from xo[(y slot*3 + c)*8 + l] to global memory                                    (a8)
+__device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld, const float* xo, int gx, int o1, int o2, int ly_lo, int ly_hi, int l_lo)
+{
+    const int lane = threadIdx.x & 31;
+    if ((unsigned)gx >= (unsigned)P.g.n[0]) return;
+    const long long nx = P.g.n[0], plane = nx * P.g.n[1];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        const int item = r * 32 + lane;            // y slot * 6 + plane
+        const int ys = item / 6, l = l_lo + item % 6;
+        const int ly = (ys - o1) & (BY - 1);
+        const int gy = o1 + ly, gz = o2 + l;
+        if (ly >= ly_lo && ly <= ly_hi && (unsigned)gy < (unsigned)P.g.n[1] && (unsigned)gz < (unsigned)P.g.n[2]) {
+            const long long off = gx + nx * gy + plane * gz;
+            const float* v = xo + ys * 24 + l;
+            __stcg(fld[0] + off, v[0]);
+            __stcg(fld[1] + off, v[8]);
+            __stcg(fld[2] + off, v[16]);
+        }
+    }
+}
+
 // ---- compute warps ---------------------------------------------------------------------------------------------
 // FDTD_PROFILE build only: lane 0 of compute warp 0 accumulates clock64 ticks per section of the step into
 // P.prof[0..7] (wait HREADY+absorb, barrier, E phase+publish, wait SIGACK, wait EREADY, absorb+barrier, H phase+publish,
@@ -527,6 +552,11 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exEx[l * PLANE + slot] = ex[l + 1];
             }
         }
+        PROF_MARK(2);
+        if (k > k0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it, the x-out rows are free
+            mbar_wait(mb + MB_SIGACK, ph.sigack & 1u);
+            ++ph.sigack;
+        }
         // publish E of R_k \ R_{k+1} (everything at the last step)                                      (a8, a6)
         if (actE && col_in && !(P.dbg & 4)) {
             if ((unsigned)(o2 + W2) < (unsigned)nz) {            // the leaving plane l = 7: every column
@@ -535,7 +565,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 __stcg(Ey + off, ey[W2 + 1]);
                 __stcg(Ez + off, ez[W2 + 1]);
             }
-            if (last | (lx == W0) | (ly == W1)) {                // leaving column / row: planes 1..6 as well
+            if (last | (ly == W1)) {                             // warp-uniform: the leaving row (or the whole tile), planes 1..6
                 long long off = col_off + plane * (o2 + 1);
 #pragma unroll
                 for (int l = 1; l < W2; ++l) {
@@ -546,12 +576,15 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     }
                     off += plane;
                 }
+            } else if (lx == W0) {                               // one lane per warp: the leaving column goes out through
+                float* xo = sm + Lay<COEF>::xoute + wy * 24;     // shared memory; the signal warp stores it
+#pragma unroll
+                for (int l = 1; l < W2; ++l) {
+                    xo[l] = ex[l + 1];
+                    xo[8 + l] = ey[l + 1];
+                    xo[16 + l] = ez[l + 1];
+                }
             }
-        }
-        PROF_MARK(2);
-        if (k > k0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it
-            mbar_wait(mb + MB_SIGACK, ph.sigack & 1u);
-            ++ph.sigack;
         }
         warp_arrive(mb + MB_EDONE);
         if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);
@@ -608,7 +641,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 __stcg(Hy + off, hy[W2]);
                 __stcg(Hz + off, hz[W2]);
             }
-            if (last | (lx == W0 - 1) | (ly == W1 - 1)) {        // leaving column / row: planes 0..5 as well
+            if (last | (ly == W1 - 1)) {                         // warp-uniform: leaving row (or whole tile), planes 0..5
                 long long off = col_off + plane * o2;
 #pragma unroll
                 for (int l = 0; l < W2 - 1; ++l) {
@@ -618,6 +651,14 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                         __stcg(Hz + off, hz[l + 1]);
                     }
                     off += plane;
+                }
+            } else if (lx == W0 - 1) {                           // the leaving column: out through shared memory
+                float* xo = sm + Lay<COEF>::xouth + wy * 24;
+#pragma unroll
+                for (int l = 0; l < W2 - 1; ++l) {
+                    xo[l] = hx[l + 1];
+                    xo[8 + l] = hy[l + 1];
+                    xo[16 + l] = hz[l + 1];
                 }
             }
         }
@@ -701,12 +742,13 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                 PROF_MARK(7);
                 if (warp == W_HPROD) {
-                    if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
-                    PROF_MARK(0);
+                    // acquire the upwind flags and order the async proxy after them while the staging is still in use
                     wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
+                    if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                    PROF_MARK(0);
+                    if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                     PROF_MARK(1);
                     if (lane == 0 && !(P.dbg & 2)) {
-                        if (!(P.dbg & 32)) fence_proxy_async();
                         issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         if (COEF) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                     }
@@ -732,13 +774,13 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         } else if (warp == W_EPROD) {
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
+                if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
                 if (k > k0) {
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
                 }
-                wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
                 if (!(P.dbg & 2)) {
                     if (lane == 0) {
-                        if (!(P.dbg & 32)) fence_proxy_async();
                         issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
                     }
                     __syncwarp();
@@ -771,10 +813,17 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 st_release(P.flagH + tile, P.flag_base + k0);
             }
             for (int k = k0; k < k1; ++k) {
+                const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                const bool xout = (k != T - 1) && !(P.dbg & 4);      // at the last step the compute warps store everything
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
-                // every publish of the phase happens-before its warp's arrive on EDONE; the release store is cumulative
+                if (xout) store_xcol(P, P.g.E, sm + Lay<COEF>::xoute, o0 + W0, o1, o2, 1, W1 - 1, 1);
+                __syncwarp();
+                // every publish of the phase happens-before its warp's arrive on EDONE (or is this warp's own store);
+                // the release store is cumulative over them
                 if (lane == 0) st_release(P.flagE + tile, P.flag_base + k + 1);
                 mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
+                if (xout) store_xcol(P, P.g.H, sm + Lay<COEF>::xouth, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
+                __syncwarp();
                 if (lane == 0) {
                     st_release(P.flagH + tile, P.flag_base + k + 1);
                     mbar_arrive(mb + MB_SIGACK);

@@ -73,7 +73,8 @@ struct SysParams {
     const int* order;      // systolic_tma.cu: claim index -> tile, sorted by wavefront bx+by+bz (NULL: identity)
     int tma_group[3];      // systolic_tma.cu, per group (E, H, coefficients): 0 per-array 3-D maps, 1 one 4-D map per piece, 2 two triples
     long long* prof;       // FDTD_PROFILE build: 32 tick accumulators (NULL otherwise)
-    int dbg;               // debug timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes, 8 no fences
+    int dbg;               // FDTD_DEBUG_SKIP timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes,
+                           // 16 no coefficient scatter, 32 no proxy fence, 64 no skipping of empty tile steps
     unsigned int delay_seed; // debug: != 0 inserts pseudo-random sleeps to perturb the inter-CTA order
 };
 

@@ -84,7 +84,7 @@ struct Lay {
     static constexpr int total = coef + NC * BZ * PLANE;
 };
 
-enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_SIGACK, MB_COUNT };
+enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_ACKE, MB_ACKH, MB_COUNT };
 
 struct TileGeom {
     int a[3];
@@ -369,7 +369,7 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
 #endif
 
 struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
-    unsigned hready, eready, sigack;
+    unsigned hready, eready, acke, ackh;
 };
 
 template <bool COEF>
@@ -554,8 +554,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         }
         PROF_MARK(2);
         if (k > k0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it, the x-out rows are free
-            mbar_wait(mb + MB_SIGACK, ph.sigack & 1u);
-            ++ph.sigack;
+            mbar_wait(mb + MB_ACKE, ph.acke & 1u);
+            ++ph.acke;
         }
         // publish E of R_k \ R_{k+1} (everything at the last step)                                      (a8, a6)
         if (actE && col_in && !(P.dbg & 4)) {
@@ -633,6 +633,10 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             exHz[l * PLANE + slot] = hz[l + 1];
             exHx[l * PLANE + slot] = hx[l + 1];
         }
+        if (k > k0) {   // the H signal duty of step k-1 is done (its x-out rows are free, HDONE cannot lap its waiter)
+            mbar_wait(mb + MB_ACKH, ph.ackh & 1u);
+            ++ph.ackh;
+        }
         // publish H of R_{k+1} \ R_{k+2} (everything at the last step)                                  (a8, a6)
         if ((lx <= W0 - 1) & (ly <= W1 - 1) && col_in && !(P.dbg & 4)) {
             if ((unsigned)(o2 + W2 - 1) < (unsigned)nz) {        // the leaving plane l = 6: every column
@@ -668,7 +672,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     }
     if (threadIdx.x < 32) PROF_FLUSH(0);
     // the signal warp's last ack of this tile is covered by the CTA barrier at the tile boundary
-    if (k1 > k0) ++ph.sigack;
+    if (k1 > k0) { ++ph.acke; ++ph.ackh; }
 }
 
 template <bool COEF>
@@ -689,11 +693,16 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         mbar_init(mb + MB_EFREE, NWARPS_C);
         mbar_init(mb + MB_EDONE, NWARPS_C);
         mbar_init(mb + MB_HDONE, NWARPS_C);
-        mbar_init(mb + MB_SIGACK, 1);
+        mbar_init(mb + MB_ACKE, 1);
+        mbar_init(mb + MB_ACKH, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // Shell slots and cells outside the grid compute on whatever the shared arrays hold and rely on 0 * garbage = 0:
+    // the garbage must be finite.  Shared memory keeps the bits of earlier kernels (possibly NaN patterns), so it is
+    // cleared once per CTA; from then on every value in it derives from finite data.
+    for (int i = tid; i < Lay<COEF>::total; i += NT) sm[i] = 0.0f;
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(M.bytes);   // [E0 E1 E2 H0 H1 H2 ca0..2 cb0..2][3 faces]
-    Phases ph = {0u, 0u, 0u};
+    Phases ph = {0u, 0u, 0u, 0u};
     // completed phases of every mbarrier an auxiliary role waits on (each role counts only what it uses)
     unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
 
@@ -738,37 +747,59 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
             PROF_DECL;
             const int hk0 = max(k0, 1);       // step 0 loads its whole box itself
-            for (int k = hk0; k < k1; ++k) {
-                const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
-                PROF_MARK(7);
-                if (warp == W_HPROD) {
-                    // acquire the upwind flags and order the async proxy after them while the staging is still in use
-                    wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
-                    if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
-                    PROF_MARK(0);
-                    if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
-                    PROF_MARK(1);
-                    if (lane == 0 && !(P.dbg & 2)) {
-                        issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
-                        if (COEF) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+            // Warp 17 also raises flagH: its duties alternate in time -- scatter for step j is triggered by EDONE(j-1)
+            // (mid step j-1), the H flag of step j-1 by HDONE(j-1) (end of step j-1) -- so the ~1-2 us a release store
+            // waits for the SM's outstanding stores overlap the E flag's (warp 19) instead of adding to it.
+            const bool hsig = (warp == W_HAUX);
+            if (hsig && k0 > 0 && lane == 0) st_release(P.flagH + tile, P.flag_base + k0);
+            for (int j = k0; j <= k1; ++j) {
+                if (j >= hk0 && j < k1) {
+                    const int k = j;
+                    const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                    PROF_MARK(7);
+                    if (warp == W_HPROD) {
+                        // acquire the upwind flags and order the async proxy after them while the staging is still in use
+                        wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
+                        if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                        PROF_MARK(0);
+                        if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
+                        PROF_MARK(1);
+                        if (lane == 0 && !(P.dbg & 2)) {
+                            issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
+                            if (COEF) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        }
+                        __syncwarp();
+                    }
+                    PROF_MARK(2);
+                    if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
+                    PROF_MARK(3);
+                    if (!(P.dbg & 2)) {
+                        mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull;
+                        if (COEF) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
+                    }
+                    PROF_MARK(4);
+                    if (!(P.dbg & 16)) scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
+                    PROF_MARK(5);
+                    if (warp == W_HAUX) pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
+                    warp_arrive(mb + MB_HREADY);
+                    PROF_MARK(6);
+                }
+                if (hsig && j > k0) {
+                    const int k = j - 1;       // H flag of step k                                                (a9)
+                    const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                    mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
+                    if (k != T - 1 && !(P.dbg & 4)) store_xcol(P, P.g.H, sm + Lay<COEF>::xouth, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
+                    __syncwarp();
+                    if (lane == 0) {
+                        st_release(P.flagH + tile, P.flag_base + k + 1);
+                        mbar_arrive(mb + MB_ACKH);
                     }
                     __syncwarp();
                 }
-                PROF_MARK(2);
-                if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
-                PROF_MARK(3);
-                if (!(P.dbg & 2)) {
-                    mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull;
-                    if (COEF) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
-                }
-                PROF_MARK(4);
-                if (!(P.dbg & 16)) scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
-                PROF_MARK(5);
-                if (warp == W_HAUX) pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
-                warp_arrive(mb + MB_HREADY);
-                PROF_MARK(6);
             }
+            if (hsig && k1 < T && lane == 0) st_release(P.flagH + tile, P.flag_base + T);
             if (warp == W_HPROD) PROF_FLUSH(8);
+            if (warp == W_HAUX) PROF_FLUSH(16);
             if (k1 > hk0) ++n_hfree;      // the last absorb's HFREE phase: covered by the CTA barrier at the tile boundary
             if (k1 > k0) ++n_edone;       // EDONE of the last step likewise
         } else if (warp == W_EPROD) {
@@ -805,36 +836,22 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             }
             if (k1 > k0) { ++n_efree; ++n_hdone; }   // phases of the last step: covered by the CTA barrier at the tile boundary
         } else {
-            // signal warp: every publish of the phase has been issued before its warp arrived; make them visible
-            // at gpu scope, then raise the flag                                                              (a9)
-            // steps before k0 publish nothing: their flags are raised at once
-            if (k0 > 0 && lane == 0) {
-                st_release(P.flagE + tile, P.flag_base + k0);
-                st_release(P.flagH + tile, P.flag_base + k0);
-            }
+            // E signal warp: every publish of the E phase has been issued before its warp arrived on EDONE (or is this warp's
+            // own store of the leaving x column); the release store of the tile flag is cumulative over them           (a9)
+            // steps outside [k0, k1) publish nothing: their flags are raised at once
+            if (k0 > 0 && lane == 0) st_release(P.flagE + tile, P.flag_base + k0);
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
-                const bool xout = (k != T - 1) && !(P.dbg & 4);      // at the last step the compute warps store everything
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
-                if (xout) store_xcol(P, P.g.E, sm + Lay<COEF>::xoute, o0 + W0, o1, o2, 1, W1 - 1, 1);
-                __syncwarp();
-                // every publish of the phase happens-before its warp's arrive on EDONE (or is this warp's own store);
-                // the release store is cumulative over them
-                if (lane == 0) st_release(P.flagE + tile, P.flag_base + k + 1);
-                mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
-                if (xout) store_xcol(P, P.g.H, sm + Lay<COEF>::xouth, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
+                if (k != T - 1 && !(P.dbg & 4)) store_xcol(P, P.g.E, sm + Lay<COEF>::xoute, o0 + W0, o1, o2, 1, W1 - 1, 1);
                 __syncwarp();
                 if (lane == 0) {
-                    st_release(P.flagH + tile, P.flag_base + k + 1);
-                    mbar_arrive(mb + MB_SIGACK);
+                    st_release(P.flagE + tile, P.flag_base + k + 1);
+                    mbar_arrive(mb + MB_ACKE);
                 }
                 __syncwarp();
             }
-            // ... and so do the steps after the region has left the grid
-            if (k1 < T && lane == 0) {
-                st_release(P.flagE + tile, P.flag_base + T);
-                st_release(P.flagH + tile, P.flag_base + T);
-            }
+            if (k1 < T && lane == 0) st_release(P.flagE + tile, P.flag_base + T);
         }
     }
 }

@@ -149,15 +149,20 @@ C4_SIZES = (64, 128, 256, 512, 768, 1024)
 # fields
 # ----------------------------------------------------------------------------------------------
 def _grouped(ts):
-    """Device tensors only: the same values as views of ONE contiguous block [len(ts), nk, nj, ni].  The C ABI still
+    """Device tensors only: the same values as views into ONE block, at a uniform 256-byte aligned stride.  The C ABI still
     receives one pointer per component; at a uniform stride between them the library fetches all components of
     a shell piece with a single 4-D TMA box (include/fdtd.h, fdtd_set_fields / fdtd_set_coeffs)."""
     import torch
-    block = torch.empty((len(ts),) + tuple(ts[0].shape), dtype=ts[0].dtype, device=ts[0].device)
+    shape, cells = tuple(ts[0].shape), ts[0].numel()
+    stride = (cells + 63) // 64 * 64              # every component stays 256-byte aligned
+    block = torch.empty(len(ts) * stride, dtype=ts[0].dtype, device=ts[0].device)
+    out = []
     for q in range(len(ts)):
-        block[q].copy_(ts[q])
+        v = block[q * stride:q * stride + cells].view(shape)
+        v.copy_(ts[q])
         ts[q] = None
-    return [block[q] for q in range(block.shape[0])]
+        out.append(v)
+    return out
 
 
 def make_fields(w: Workload, window=None, device=None):
@@ -169,8 +174,8 @@ def make_fields(w: Workload, window=None, device=None):
         if device is None:
             return ([np.zeros(shape, np.float32) for _ in range(3)], [np.zeros(shape, np.float32) for _ in range(3)])
         import torch
-        return (list(torch.zeros((3,) + shape, dtype=torch.float32, device=device)),
-                list(torch.zeros((3,) + shape, dtype=torch.float32, device=device)))
+        return (_grouped([torch.zeros(shape, dtype=torch.float32, device=device) for _ in range(3)]),
+                _grouped([torch.zeros(shape, dtype=torch.float32, device=device) for _ in range(3)]))
     assert w.fields == "uniform"
     coords = (i, j, k)
     E, H = [], []

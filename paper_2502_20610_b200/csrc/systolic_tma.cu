@@ -84,7 +84,7 @@ struct Lay {
     static constexpr int total = coef + NC * BZ * PLANE;
 };
 
-enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_ACKE, MB_ACKH, MB_COUNT };
+enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_ACKE, MB_ACKH, MB_CREADY, MB_CFREE, MB_COUNT };
 
 struct TileGeom {
     int a[3];
@@ -280,31 +280,33 @@ __device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int 
     if (part == 0) {
         const int gx = o0 + lane, gy = o1;
         float* dst = coef + (gy & (BY - 1)) * SX + (gx & (BX - 1));
+        float v[NC][BZ];      // all loads first: staging and slots are the same array to the compiler
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            float v[BZ];
+        for (int c = 0; c < NC; ++c)
 #pragma unroll
-            for (int l = 1; l < BZ; ++l) v[l] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
+            for (int l = 1; l < BZ; ++l) v[c][l] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
 #pragma unroll
-            for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_value<COEF>(P, c, v[l], gx, gy, o2 + l);
-        }
+        for (int c = 0; c < NC; ++c)
+#pragma unroll
+            for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_value<COEF>(P, c, v[c][l], gx, gy, o2 + l);
     } else {
         const int xs = o0 & (BX - 1);
+        float v[NC][4];
 #pragma unroll
-        for (int c = 0; c < NC; ++c) {
-            float v[4];
+        for (int r = 0; r < 4; ++r) {            // 105 cells: idx = (l-1)*15 + (ly-1)
+            const int idx = r * 32 + lane;
+            const int ly = 1 + idx % W1, l = 1 + idx / W1;
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {            // 105 cells: idx = (l-1)*15 + (ly-1)
-                const int idx = r * 32 + lane;
-                const int ly = 1 + idx % W1, l = 1 + idx / W1;
-                v[r] = (COEF && idx < W1 * W2) ? stg[xidx<6>(c, ly, l) + r0] : 0.0f;
-            }
+            for (int c = 0; c < NC; ++c) v[c][r] = (COEF && idx < W1 * W2) ? stg[xidx<6>(c, ly, l) + r0] : 0.0f;
+        }
 #pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const int idx = r * 32 + lane;
-                const int ly = 1 + idx % W1, l = 1 + idx / W1;
-                if (idx < W1 * W2)
-                    coef[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE + ((o1 + ly) & (BY - 1)) * SX + xs] = coef_value<COEF>(P, c, v[r], o0, o1 + ly, o2 + l);
+        for (int r = 0; r < 4; ++r) {
+            const int idx = r * 32 + lane;
+            const int ly = 1 + idx % W1, l = 1 + idx / W1;
+            if (idx < W1 * W2) {
+                float* d = coef + ((o2 + l) & (BZ - 1)) * PLANE + ((o1 + ly) & (BY - 1)) * SX + xs;
+#pragma unroll
+                for (int c = 0; c < NC; ++c) d[c * BZ * PLANE] = coef_value<COEF>(P, c, v[c][r], o0, o1 + ly, o2 + l);
             }
         }
     }
@@ -369,7 +371,7 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
 #endif
 
 struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
-    unsigned hready, eready, acke, ackh;
+    unsigned hready, eready, acke, ackh, cready;
 };
 
 template <bool COEF>
@@ -457,24 +459,6 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             hx[0] = stgH[zidx<3>(0, ly, xs)];
             hy[0] = stgH[zidx<3>(1, ly, xs)];
             hz[0] = stgH[zidx<3>(2, ly, xs)];
-            {   // coefficients of the entering plane l_z = 0 -> this thread's private slots
-                float* cs = coef + (o2 & (BZ - 1)) * PLANE;
-                if (COEF) {
-                    const float* sc = sm + Lay<COEF>::stgc;
-                    float v[6];
-#pragma unroll
-                    for (int c = 0; c < 6; ++c) v[c] = sc[zidx<6>(c, ly, xs)];
-                    if ((o0 <= 0) | (o1 <= 0) | (o2 <= 0)) {   // CTA-uniform: the box touches a low wall
-#pragma unroll
-                        for (int c = 0; c < 6; ++c) v[c] = coef_value<COEF>(P, c, v[c], gx, gy, o2);
-                    }
-#pragma unroll
-                    for (int c = 0; c < 6; ++c) cs[c * (BZ * PLANE)] = v[c];
-                } else {
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) cs[c * (BZ * PLANE)] = coef_value<COEF>(P, c, 0.0f, gx, gy, o2);
-                }
-            }
             if (ly == 0) {            // warp-uniform: the entering row; its y+1 neighbours read it from the exchange
 #pragma unroll
                 for (int l = 1; l < BZ; ++l) {
@@ -551,6 +535,33 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exEz[l * PLANE + slot] = ez[l + 1];
                 exEx[l * PLANE + slot] = ex[l + 1];
             }
+        }
+        // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
+        // They are first used by E phase k+1 (shell cells are not in R_k), so their copy and scatter run a phase behind
+        // the field shell: the compute warps wait for them here, after E phase k, not at the top of the step.
+        if (k >= 1) {
+            mbar_wait(mb + MB_CREADY, ph.cready & 1u);
+            ++ph.cready;
+            const int xs = (o0 & 3) + lx;
+            {   // the entering plane l_z = 0 -> this thread's private slots (row and column: auxiliary warp 17)
+                float* cs = coef + (o2 & (BZ - 1)) * PLANE;
+                if (COEF) {
+                    const float* sc = sm + Lay<COEF>::stgc;
+                    float v[6];
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) v[c] = sc[zidx<6>(c, ly, xs)];
+                    if ((o0 <= 0) | (o1 <= 0) | (o2 <= 0)) {   // CTA-uniform: the box touches a low wall
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) v[c] = coef_value<COEF>(P, c, v[c], gx, gy, o2);
+                    }
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) cs[c * (BZ * PLANE)] = v[c];
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) cs[c * (BZ * PLANE)] = coef_value<COEF>(P, c, 0.0f, gx, gy, o2);
+                }
+            }
+            warp_arrive(mb + MB_CFREE);
         }
         PROF_MARK(2);
         if (k > k0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it, the x-out rows are free
@@ -687,7 +698,9 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         mbar_init(mb + MB_HFULL, 1);
         mbar_init(mb + MB_CFULL, 1);
         mbar_init(mb + MB_EFULL, 1);
-        mbar_init(mb + MB_HREADY, 2);
+        mbar_init(mb + MB_HREADY, 1);
+        mbar_init(mb + MB_CREADY, 1);
+        mbar_init(mb + MB_CFREE, NWARPS_C);
         mbar_init(mb + MB_EREADY, 1);
         mbar_init(mb + MB_HFREE, NWARPS_C);
         mbar_init(mb + MB_EFREE, NWARPS_C);
@@ -702,9 +715,9 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
     // cleared once per CTA; from then on every value in it derives from finite data.
     for (int i = tid; i < Lay<COEF>::total; i += NT) sm[i] = 0.0f;
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(M.bytes);   // [E0 E1 E2 H0 H1 H2 ca0..2 cb0..2][3 faces]
-    Phases ph = {0u, 0u, 0u, 0u};
+    Phases ph = {0u, 0u, 0u, 0u, 0u};
     // completed phases of every mbarrier an auxiliary role waits on (each role counts only what it uses)
-    unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
+    unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_cfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
 
     for (;;) {
         __syncthreads();
@@ -747,10 +760,10 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
             PROF_DECL;
             const int hk0 = max(k0, 1);       // step 0 loads its whole box itself
-            // Warp 17 also raises flagH: its duties alternate in time -- scatter for step j is triggered by EDONE(j-1)
-            // (mid step j-1), the H flag of step j-1 by HDONE(j-1) (end of step j-1) -- so the ~1-2 us a release store
-            // waits for the SM's outstanding stores overlap the E flag's (warp 19) instead of adding to it.
-            const bool hsig = (warp == W_HAUX);
+            // Who raises flagH.  A release store waits ~1-2 us for the SM's outstanding stores; two per step in one warp
+            // (19) lengthen the ACK round trip.  Without coefficient arrays warp 17 is nearly idle and takes the H flag
+            // (measured +7 % at 768^3); with them it carries the coefficient pipeline and warp 19 keeps both flags.
+            const bool hsig = !COEF && warp == W_HAUX;
             if (hsig && k0 > 0 && lane == 0) st_release(P.flagH + tile, P.flag_base + k0);
             for (int j = k0; j <= k1; ++j) {
                 if (j >= hk0 && j < k1) {
@@ -758,31 +771,41 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                     PROF_MARK(7);
                     if (warp == W_HPROD) {
-                        // acquire the upwind flags and order the async proxy after them while the staging is still in use
+                        // field shell: acquire the upwind flags and order the async proxy after them while the staging is
+                        // still in use, copy, repack the entering column -> HREADY(k)
                         wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
                         if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
                         PROF_MARK(0);
                         if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                         PROF_MARK(1);
-                        if (lane == 0 && !(P.dbg & 2)) {
-                            issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
-                            if (COEF) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
-                        }
+                        if (lane == 0 && !(P.dbg & 2)) issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         __syncwarp();
+                        PROF_MARK(2);
+                        if (!(P.dbg & 2)) { mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull; }
+                        PROF_MARK(3);
+                        pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
+                        warp_arrive(mb + MB_HREADY);
+                        PROF_MARK(4);
+                    } else {
+                        // coefficient shell (constants of the run: no flag, no proxy fence): copy once the compute warps have
+                        // absorbed the previous plane, scatter row and column once E phase k-1 has read the leaving
+                        // cells' slots -> CREADY(k), awaited after E phase k
+                        if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
+                        PROF_MARK(0);
+                        if (COEF && lane == 0 && !(P.dbg & 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        __syncwarp();
+                        PROF_MARK(1);
+                        if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
+                        PROF_MARK(2);
+                        if (COEF && !(P.dbg & 2)) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
+                        PROF_MARK(3);
+                        if (!(P.dbg & 16)) {
+                            scatter_coef<COEF>(P, sm, o0, o1, o2, 0);
+                            scatter_coef<COEF>(P, sm, o0, o1, o2, 1);
+                        }
+                        warp_arrive(mb + MB_CREADY);
+                        PROF_MARK(4);
                     }
-                    PROF_MARK(2);
-                    if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
-                    PROF_MARK(3);
-                    if (!(P.dbg & 2)) {
-                        mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull;
-                        if (COEF) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
-                    }
-                    PROF_MARK(4);
-                    if (!(P.dbg & 16)) scatter_coef<COEF>(P, sm, o0, o1, o2, warp - W_HPROD);
-                    PROF_MARK(5);
-                    if (warp == W_HAUX) pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
-                    warp_arrive(mb + MB_HREADY);
-                    PROF_MARK(6);
                 }
                 if (hsig && j > k0) {
                     const int k = j - 1;       // H flag of step k                                                (a9)
@@ -797,11 +820,12 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     __syncwarp();
                 }
             }
-            if (hsig && k1 < T && lane == 0) st_release(P.flagH + tile, P.flag_base + T);
             if (warp == W_HPROD) PROF_FLUSH(8);
             if (warp == W_HAUX) PROF_FLUSH(16);
-            if (k1 > hk0) ++n_hfree;      // the last absorb's HFREE phase: covered by the CTA barrier at the tile boundary
-            if (k1 > k0) ++n_edone;       // EDONE of the last step likewise
+            if (hsig && k1 < T && lane == 0) st_release(P.flagH + tile, P.flag_base + T);
+            // phases of the last step that this warp does not wait for: covered by the CTA barrier at the tile boundary
+            if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else ++n_cfree; }
+            if (k1 > k0 && warp == W_HAUX) ++n_edone;
         } else if (warp == W_EPROD) {
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
@@ -836,10 +860,13 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             }
             if (k1 > k0) { ++n_efree; ++n_hdone; }   // phases of the last step: covered by the CTA barrier at the tile boundary
         } else {
-            // E signal warp: every publish of the E phase has been issued before its warp arrived on EDONE (or is this warp's
-            // own store of the leaving x column); the release store of the tile flag is cumulative over them           (a9)
+            // signal warp: every publish of a phase has been issued before its warp arrived on the DONE barrier (or is this
+            // warp's own store of the leaving x column); the release store of the tile flag is cumulative over them   (a9)
             // steps outside [k0, k1) publish nothing: their flags are raised at once
-            if (k0 > 0 && lane == 0) st_release(P.flagE + tile, P.flag_base + k0);
+            if (k0 > 0 && lane == 0) {
+                st_release(P.flagE + tile, P.flag_base + k0);
+                if (COEF) st_release(P.flagH + tile, P.flag_base + k0);
+            }
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
@@ -850,8 +877,21 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     mbar_arrive(mb + MB_ACKE);
                 }
                 __syncwarp();
+                if (COEF) {
+                    mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
+                    if (k != T - 1 && !(P.dbg & 4)) store_xcol(P, P.g.H, sm + Lay<COEF>::xouth, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
+                    __syncwarp();
+                    if (lane == 0) {
+                        st_release(P.flagH + tile, P.flag_base + k + 1);
+                        mbar_arrive(mb + MB_ACKH);
+                    }
+                    __syncwarp();
+                }
             }
-            if (k1 < T && lane == 0) st_release(P.flagE + tile, P.flag_base + T);
+            if (k1 < T && lane == 0) {
+                st_release(P.flagE + tile, P.flag_base + T);
+                if (COEF) st_release(P.flagH + tile, P.flag_base + T);
+            }
         }
     }
 }

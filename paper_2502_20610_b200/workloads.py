@@ -165,9 +165,35 @@ def _grouped(ts):
     return out
 
 
+_SLAB_CELLS = 1 << 26      # device arrays larger than this are generated slab by slab (the generators' int64 temporaries
+                           # are several times the size of a component: 81 GiB config 5 would not fit beside them)
+
+
+def _slabwise(gen, w, device, ncomp):
+    """Run `gen(w, window, device)` (-> list of ncomp tensors for the window) over z slabs of the whole grid and return
+    ncomp views of one block at a uniform 256-byte aligned stride (see _grouped); None entries pass through."""
+    import torch
+    nx, ny, nz = w.n
+    cells = nx * ny * nz
+    stride = (cells + 63) // 64 * 64
+    block = torch.empty(ncomp * stride, dtype=torch.float32, device=device)
+    out = [block[q * stride:q * stride + cells].view(nz, ny, nx) for q in range(ncomp)]
+    nk = max(1, _SLAB_CELLS // (nx * ny))
+    for k0 in range(0, nz, nk):
+        kk = min(nk, nz - k0)
+        part = gen(w, (0, 0, k0, nx, ny, kk), device)
+        for q in range(ncomp):
+            out[q][k0:k0 + kk].copy_(part[q])
+        del part
+    return out
+
+
 def make_fields(w: Workload, window=None, device=None):
     """-> (E, H): two lists of three float32 arrays of shape (nk, nj, ni) for `window` (default whole grid).
     device=None: numpy; else torch tensors on that device (bit-identical values)."""
+    if device is not None and window is None and w.cells > _SLAB_CELLS:
+        g = _slabwise(lambda ww, win, dev: sum(make_fields(ww, win, dev), []), w, device, 6)
+        return g[:3], g[3:]
     i, j, k, idx = _lin_index(w.n, window, like=device)
     shape = tuple(idx.shape)
     if w.fields == "zero":
@@ -234,6 +260,9 @@ def make_eps(w: Workload, window=None, device=None):
 def make_coeffs(w: Workload, window=None, device=None):
     """-> (ca, cb): lists of three float32 per-cell arrays, or (None, None) when the workload has uniform
     coefficients (ca = 1, cb = dt).  All six arrays are materialised and read even where ca == 1."""
+    if device is not None and window is None and w.cells > _SLAB_CELLS and w.has_coeff_arrays:
+        g = _slabwise(lambda ww, win, dev: sum(make_coeffs(ww, win, dev), []), w, device, 6)
+        return g[:3], g[3:]
     eps = make_eps(w, window, device)
     if eps is None:
         return None, None

@@ -108,6 +108,23 @@ def algorithmic_bytes_per_cell_update(kernel, info, has_coef):
     return 4.0 * (loads + stores) / (V * T)
 
 
+def max_over_ranks(dist, value, device):
+    """Replicas only: the one cross-rank step of the bench is the MAX of a per-rank time.
+    dist is torch.distributed (already initialised) or None for a single process."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_tcups(world, cell_updates_per_rank, seconds):
+    """Whole-job throughput of `world` independent replicas that each advanced cell_updates_per_rank in `seconds`
+    (the max over ranks): weak scaling, no data-path collective."""
+    return world * cell_updates_per_rank / seconds / 1e12
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle as it stands, on the host cores, same config / metric / unit."""
     import numpy as np
@@ -230,12 +247,9 @@ def main():
     sampler.stop_flag = True
     sampler.join()
     launches = c1["launches"] - c0["launches"]
-    if dist is not None:
-        t = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(dist, total_ms, dev)
     cell_updates = w.cells * S * K
-    value = world * cell_updates / (total_ms * 1e-3) / 1e12
+    value = job_tcups(world, cell_updates, total_ms * 1e-3)
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     e2e = None
@@ -260,12 +274,9 @@ def main():
             one()
         barrier()
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dist, dt, dev)
         nbytes = 6 * w.cells * 4
-        e2e = {"value": world * w.cells * S * ke / dt / 1e12, "unit": "TCUPS", "h2d_bytes_per_step": nbytes,
+        e2e = {"value": job_tcups(world, w.cells * S * ke, dt), "unit": "TCUPS", "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": ke,
                "note": "six field arrays pinned host->device, S time steps, six arrays device->host, per bench step; "
                        "the six coefficient arrays are problem constants bound once"}

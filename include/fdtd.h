@@ -56,7 +56,8 @@ enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1, FDTD_KERNEL_SYSTOLIC_SME
 /* Create a context for an nx*ny*nz grid with cell sizes dx,dy,dz (> 0, finite), time step dt (> 0, finite)
  * and per-axis wall type boundary[3] (host array of FDTD_PEC | FDTD_PERIODIC).
  * cuda_stream: a cudaStream_t (as void*) on which all work is enqueued; NULL = the legacy default stream.
- * The default kernel is FDTD_KERNEL_SYSTOLIC with library-chosen tile shape and temporal depth.
+ * Default schedule (no fdtd_set_kernel call): FDTD_KERNEL_SYSTOLIC with library-chosen tile shape and temporal depth
+ * where its TMA-staged kernel applies (all axes PEC, nx % 4 == 0), FDTD_KERNEL_NAIVE otherwise; fdtd_get_kernel tells.
  * *out is written only on FDTD_OK.  FDTD_EINVAL: bad dims (each 1..2^15, product < 2^40), spacings, dt, boundary.
  * FDTD_ECUDA: no usable sm_100 device / CUDA failure.   (problem statement: PAPER.md:35-37) */
 int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, float dt,

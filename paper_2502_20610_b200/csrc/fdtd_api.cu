@@ -25,6 +25,7 @@ struct fdtd_ctx {
     long long t;
     // schedule
     int which;
+    bool which_explicit;   // fdtd_set_kernel was called: no automatic choice
     int reqN[3];      // requested tile (0 = default)
     int reqT;         // requested temporal depth (0 = default)
     int cfg_idx;      // resolved shared-memory systolic configuration, -1 = unresolved / not used
@@ -299,6 +300,20 @@ int ensure_order(fdtd_ctx* c, const int nb[3])
     return FDTD_OK;
 }
 
+// Library default (no fdtd_set_kernel call): the systolic schedule where its TMA-staged kernel applies (all axes PEC,
+// nx % 4 == 0); grids with a periodic axis or another nx run the naive kernel, which is ~4x faster there than the
+// cp.async systolic kernel (a ring of tiles advances in lock step: 0.015 vs 0.070 TCUPS on config 3).
+bool tma_eligible(const fdtd_ctx* c)
+{
+    return !c->g.per[0] && !c->g.per[1] && !c->g.per[2] && c->g.n[0] % 4 == 0 && !coef_mixed(c) && !getenv("FDTD_NO_TMA");
+}
+
+int effective_kernel(const fdtd_ctx* c)
+{
+    if (!c->which_explicit && c->which == FDTD_KERNEL_SYSTOLIC && !tma_eligible(c)) return FDTD_KERNEL_NAIVE;
+    return c->which;
+}
+
 int step_naive(fdtd_ctx* c, int n)
 {
     for (int s = 0; s < n; ++s) {
@@ -445,6 +460,7 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->d_amp = c->d_wave = nullptr;
     c->t = 0;
     c->which = FDTD_KERNEL_SYSTOLIC;
+    c->which_explicit = false;
     c->reqT = 0;
     c->cfg_idx = -1;
     c->use_reg = false;
@@ -587,7 +603,7 @@ int fdtd_step(fdtd_ctx* c, int n)
     if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_step before fdtd_set_fields");
     cudaError_t e = cudaEventRecord(c->ev0, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
-    const int rc = (c->which == FDTD_KERNEL_NAIVE) ? step_naive(c, n) : step_systolic(c, n);
+    const int rc = (effective_kernel(c) == FDTD_KERNEL_NAIVE) ? step_naive(c, n) : step_systolic(c, n);
     e = cudaEventRecord(c->ev1, c->stream);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
     c->ev_valid = true;
@@ -641,6 +657,7 @@ int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
     const int oldN[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};
     const int oldT = c->reqT, oldw = c->which;
     c->which = which;
+    c->which_explicit = true;
     c->reqN[0] = Nx; c->reqN[1] = Ny; c->reqN[2] = Nz;
     c->reqT = T;
     c->cfg_idx = -1;
@@ -663,8 +680,8 @@ int fdtd_get_kernel(const fdtd_ctx* cc, int out[8])
     fdtd_ctx* c = const_cast<fdtd_ctx*>(cc);
     if (!c || !out) return FDTD_EINVAL;
     memset(out, 0, 8 * sizeof(int));
-    out[0] = c->which;
-    if (c->which != FDTD_KERNEL_NAIVE) {
+    out[0] = effective_kernel(c);
+    if (out[0] != FDTD_KERNEL_NAIVE) {
         if (!c->resolved) {
             const int rc = resolve_systolic(c);
             if (rc != FDTD_OK) return rc;

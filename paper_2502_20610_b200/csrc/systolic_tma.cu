@@ -12,25 +12,29 @@
 //     outside the grid are zero-filled by TMA (fields and coefficients), so E stays 0 there (the PEC ghost,
 //     reading #5); frozen wall components get (ca, cb) = (1, 0) when their coefficients enter the chip; shell
 //     slots compute garbage that the next shell absorb overwrites.  Stores are predicated, arithmetic is not.
-//   * the minus shell of every step is fetched by TMA (cp.async.bulk.tensor.3d, three boxes per array: a z
-//     plane 36x16x1, a y row 36x1x7, an x column 4x15x7, each starting on a 16-byte boundary in x) into shared-memory staging, completing on mbarriers;
-//     auxiliary warps poll the upwind flags, issue the copies one step ahead of the compute warps, scatter
-//     the entering coefficients into the owner threads' private shared-memory slots and repack the x column
+//   * the minus shell of every step is fetched by TMA (cp.async.bulk.tensor, three boxes per array or -- when the
+//     component arrays sit at a uniform stride -- per group of arrays: a z plane 36x16x1, a y row 36x1x8, an x column
+//     4x16x7, each starting on a 16-byte boundary in x) into shared-memory staging, completing on mbarriers;
+//     auxiliary warps poll the upwind flags, issue the copies one step ahead of the compute warps, scatter the
+//     entering row/column coefficients into the owner threads' private shared-memory slots and repack the x column
 //     so that its single owner lane absorbs it with 16-byte loads.
-//   * every hand-off inside the CTA is an mbarrier with one elected arrive per warp; the only CTA-wide
-//     barrier is the 512-thread named barrier between absorb and phase.
+//   * every hand-off inside the CTA is an mbarrier with one elected arrive per warp; the only CTA-wide barrier is the
+//     512-thread named barrier between absorb and phase.
+//   * tiles are claimed in wavefront order (bx+by+bz) and skip the steps at which their region lies outside the grid.
 //
-//   compute (warps 0-15)     H side (warps 16,17)            E side (warp 18)          signal (warp 19)
-//   --------------------     --------------------            ----------------          ----------------
-//   wait HREADY(k)           wait HFREE(k-1)                 wait EFREE(k-1), HDONE(k-1)
-//   absorb H shell  ->HFREE  poll flagH[u] >= base+k         poll flagE[u] >= base+k+1
-//   E phase k                TMA H (+ coefficient) shell     TMA E shell
-//   publish E       ->EDONE  wait EDONE(k-1), copies landed  wait copies landed        wait EDONE(k): fence,
-//   wait EREADY(k)           scatter coefficients, pack x    pack x column                  flagE = base+k+1
-//   absorb E shell  ->EFREE  ->HREADY(k)                     ->EREADY(k)
+//   compute (warps 0-15)         warp 16: field H shell      warp 17: coefficient shell   warp 18: field E shell     warp 19: flags
+//   --------------------         ------------------------    -------------------------    -----------------------    ---------------
+//   wait HREADY(k), absorb H     poll flagH[u] >= base+k     wait CFREE(k-1)              poll flagE[u] >= base+k+1
+//     -> HFREE                   fence.proxy.async           TMA coefficient shell k      fence.proxy.async
+//   E phase k                    wait HFREE(k-1)             wait EDONE(k-1), landed      wait EFREE(k-1)
+//   wait CREADY(k), absorb       TMA H shell k               scatter row + column         TMA E shell k, landed
+//     coefficient plane -> CFREE wait landed, pack x column  -> CREADY(k)                 pack x column
+//   wait ACKE(k-1), publish E    -> HREADY(k)                (no coefficient arrays: also wait HDONE(k-1)            wait EDONE(k): x column,
+//     -> EDONE                                                raises flagH, see below)    write E exchange column      flagE = base+k+1 -> ACKE
+//   wait EREADY(k), absorb E                                                              -> EREADY(k)               wait HDONE(k): x column,
+//     -> EFREE                                                                                                         flagH = base+k+1 -> ACKH
 //   H phase k
-//   publish H       ->HDONE                                                            wait HDONE(k): fence,
-//                                                                                           flagH = base+k+1
+//   wait ACKH(k-1), publish H -> HDONE
 //
 // Per-cell arithmetic is yee_update.h, unchanged: with -fmad=false the result is bit-identical to the oracle.
 // Scope: all three axes PEC and nx % 4 == 0 (TMA strides are multiples of 16 bytes); other grids run

@@ -719,6 +719,10 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
     // cleared once per CTA; from then on every value in it derives from finite data.
     for (int i = tid; i < Lay<COEF>::total; i += NT) sm[i] = 0.0f;
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(M.bytes);   // [E0 E1 E2 H0 H1 H2 ca0..2 cb0..2][3 faces]
+    // Acquire the flags of step k+1 (and run the ~0.7 us proxy fence) while the copy of step k is in flight, instead of
+    // at the top of iteration k+1.  Measured: +5 % at 768^3 without coefficient arrays, -2 % on config 2 with them (the
+    // field copies then queue earlier against the coefficient copies), hence per instantiation.
+    constexpr bool EARLY = !COEF;
     Phases ph = {0u, 0u, 0u, 0u, 0u};
     // completed phases of every mbarrier an auxiliary role waits on (each role counts only what it uses)
     unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_cfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
@@ -777,13 +781,19 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     if (warp == W_HPROD) {
                         // field shell: acquire the upwind flags and order the async proxy after them while the staging is
                         // still in use, copy, repack the entering column -> HREADY(k)
-                        wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
-                        if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                        if (k == hk0 || !EARLY) {      // later steps: acquired while the previous copy was in flight
+                            wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
+                            if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                        }
                         PROF_MARK(0);
                         if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                         PROF_MARK(1);
                         if (lane == 0 && !(P.dbg & 2)) issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         __syncwarp();
+                        if (k + 1 < k1 && EARLY) {
+                            wait_upwind(P, t, P.flagH, P.flag_base + k + 1, &ctl);
+                            if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                        }
                         PROF_MARK(2);
                         if (!(P.dbg & 2)) { mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull; }
                         PROF_MARK(3);
@@ -831,20 +841,28 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else ++n_cfree; }
             if (k1 > k0 && warp == W_HAUX) ++n_edone;
         } else if (warp == W_EPROD) {
+            // the flags of step k are acquired (and the async proxy ordered after them) while the copy of step k-1 is in
+            // flight: the ~0.7 us proxy fence is off the EFREE -> EREADY chain
+            if (k0 < k1) {
+                wait_upwind(P, t, P.flagE, P.flag_base + k0 + 1, &ctl);
+                if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+            }
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
-                wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
-                if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                if (k > k0 && !EARLY) {
+                    wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
+                    if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                }
                 if (k > k0) {
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
                 }
-                if (!(P.dbg & 2)) {
-                    if (lane == 0) {
-                        issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
-                    }
-                    __syncwarp();
-                    mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull;
+                if (lane == 0 && !(P.dbg & 2)) issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
+                __syncwarp();
+                if (k + 1 < k1 && EARLY) {
+                    wait_upwind(P, t, P.flagE, P.flag_base + k + 2, &ctl);
+                    if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
                 }
+                if (!(P.dbg & 2)) { mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull; }
                 const float* stg = sm + Lay<COEF>::stge;
                 pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
                 if (k > k0) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows

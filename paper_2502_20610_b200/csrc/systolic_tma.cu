@@ -41,6 +41,8 @@
 // systolic_reg.cu.
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "fdtd_internal.h"
 #include "yee_update.h"
 
@@ -379,7 +381,7 @@ struct Phases {   // completed phases of each mbarrier as seen by this thread's 
 };
 
 template <bool COEF>
-__device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, int k0, int k1, float* sm, unsigned long long* mb, Phases& ph)
+__device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, int k0, int k1, bool fast, float* sm, unsigned long long* mb, Phases& ph)
 {
     const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
     const int slot = wy * SX + lane;
@@ -486,6 +488,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 
         PROF_MARK(1);
         // ---------------- E phase on R_k = [1,w]^3 (a1): every slot computes, shell slots produce garbage ----
+        // fast (no coefficient arrays, box never touches a wall or the outside): cb is the scalar dt, no mask loads
+        auto e_phase = [&](auto fastc) {
+        constexpr bool FAST = decltype(fastc)::value;
 #pragma unroll
         for (int l = BZ - 1; l >= 1; --l) {
             const float hz_xm = __shfl_sync(0xffffffffu, hz[l], lane_m);
@@ -497,6 +502,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             if (COEF) {
                 cax = cs[0 * (BZ * PLANE)]; cay = cs[1 * (BZ * PLANE)]; caz = cs[2 * (BZ * PLANE)];
                 cbx = cs[3 * (BZ * PLANE)]; cby = cs[4 * (BZ * PLANE)]; cbz = cs[5 * (BZ * PLANE)];
+            } else if (FAST) {
+                cbx = cby = cbz = P.g.cb_scalar;
             } else {
                 cbx = cs[0 * (BZ * PLANE)]; cby = cs[1 * (BZ * PLANE)]; cbz = cs[2 * (BZ * PLANE)];
             }
@@ -507,6 +514,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             // E_z: (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy
             ez[l + 1] = yee_e_update<COEF>(ez[l], hy[l], hy_xm, hx[l], hx_ym, rdx, rdy, caz, cbz);
         }
+        };
+        if (!COEF && fast) e_phase(std::true_type{});
+        else e_phase(std::false_type{});
         const bool actE = (lx >= 1) & (ly >= 1);            // column belongs to R_k
         // soft source after the E update of step t0 + k (a4): rare, CTA-uniform test first
         {
@@ -543,7 +553,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
         // They are first used by E phase k+1 (shell cells are not in R_k), so their copy and scatter run a phase behind
         // the field shell: the compute warps wait for them here, after E phase k, not at the top of the step.
-        if (k >= 1) {
+        if (k >= 1 && !fast) {
             mbar_wait(mb + MB_CREADY, ph.cready & 1u);
             ++ph.cready;
             const int xs = (o0 & 3) + lx;
@@ -753,6 +763,13 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         }
         if (k1 < k0) k1 = k0;
         if (P.dbg & 64) { k0 = 0; k1 = T; }
+        // no coefficient arrays and the box stays strictly inside the grid (never index 0, never outside) for the whole
+        // launch: every cb mask would be dt -- the tile runs without masks, without their scatter and without CREADY/CFREE
+        bool fast = !COEF && !(P.dbg & 256);
+        for (int q = 0; q < 3; ++q) {
+            const int wq = q == 0 ? W0 : q == 1 ? W1 : W2;
+            fast = fast && (t.a[q] - k1 >= 1) && (t.a[q] - k0 + wq <= P.g.n[q]);
+        }
         if (k0 > 0 && warp < NWARPS_C) {
             // started late: nothing is loaded from the grid; the box holds zero fields (registers) and zero coefficients
             float* cs = sm + Lay<COEF>::coef + (tid >> 5) * SX + lane;
@@ -762,7 +779,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         __syncthreads();
 
         if (warp < NWARPS_C) {
-            compute_tile<COEF>(P, t, tile, k0, k1, sm, mb, ph);
+            compute_tile<COEF>(P, t, tile, k0, k1, fast, sm, mb, ph);
         } else if (warp == W_HPROD || warp == W_HAUX) {
             // H side: shell of step k needs the staging of step k-1 absorbed (HFREE), the upwind tiles' H of
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
@@ -804,6 +821,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                         // coefficient shell (constants of the run: no flag, no proxy fence): copy once the compute warps have
                         // absorbed the previous plane, scatter row and column once E phase k-1 has read the leaving
                         // cells' slots -> CREADY(k), awaited after E phase k
+                        if (!fast) {                 // (a uniform interior tile has no coefficient pipeline)
                         if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
                         PROF_MARK(0);
                         if (COEF && lane == 0 && !(P.dbg & 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
@@ -819,6 +837,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                         }
                         warp_arrive(mb + MB_CREADY);
                         PROF_MARK(4);
+                        }
                     }
                 }
                 if (hsig && j > k0) {
@@ -838,8 +857,8 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             if (warp == W_HAUX) PROF_FLUSH(16);
             if (hsig && k1 < T && lane == 0) st_release(P.flagH + tile, P.flag_base + T);
             // phases of the last step that this warp does not wait for: covered by the CTA barrier at the tile boundary
-            if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else ++n_cfree; }
-            if (k1 > k0 && warp == W_HAUX) ++n_edone;
+            if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else if (!fast) ++n_cfree; }
+            if (k1 > k0 && warp == W_HAUX) n_edone += fast ? (unsigned)(k1 - k0) : 1u;
         } else if (warp == W_EPROD) {
             // the flags of step k are acquired (and the async proxy ordered after them) while the copy of step k-1 is in
             // flight: the ~0.7 us proxy fence is off the EFREE -> EREADY chain

@@ -55,6 +55,7 @@ constexpr int SX = BX + 1;                              // row stride of the slo
 constexpr int PLANE = SX * BY;                          // slots (the entering x column) then spans 16 banks, not one
 constexpr int NWARPS_C = NCOMPUTE / 32;
 constexpr int NT = NCOMPUTE + 128;
+constexpr int REGS_COMPUTE = 104, REGS_AUX = 64;     // 512*104 + 128*64 = 61440 = 640*96; (112, 32) spills in the aux warps and is 10 % slower
 constexpr int W_HPROD = 16, W_HAUX = 17, W_EPROD = 18;   // warp 19: signal
 
 // staging of one array's minus shell (floats); every TMA destination is 128-byte aligned
@@ -95,6 +96,12 @@ enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFRE
 struct TileGeom {
     int a[3];
     int nbr[7];
+};
+
+struct TileJob {
+    int tile, k0, k1;
+    bool fast;
+    TileGeom t;
 };
 
 struct Ctl {
@@ -286,15 +293,20 @@ __device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int 
     if (part == 0) {
         const int gx = o0 + lane, gy = o1;
         float* dst = coef + (gy & (BY - 1)) * SX + (gx & (BX - 1));
-        float v[NC][BZ];      // all loads first: staging and slots are the same array to the compiler
+        // loads of a batch first (staging and slots are the same array to the compiler); three components per batch keep
+        // the auxiliary warps inside their 64-register budget
 #pragma unroll
-        for (int c = 0; c < NC; ++c)
+        for (int c0 = 0; c0 < NC; c0 += 3) {
+            float v[3][BZ];
 #pragma unroll
-            for (int l = 1; l < BZ; ++l) v[c][l] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
+            for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int c = 0; c < NC; ++c)
+                for (int l = 1; l < BZ; ++l) v[c][l] = COEF ? stg[yidx<6>(c0 + c, l, r0 + lane)] : 0.0f;
 #pragma unroll
-            for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_value<COEF>(P, c, v[c][l], gx, gy, o2 + l);
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int l = 1; l < BZ; ++l) dst[((c0 + c) * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_value<COEF>(P, c0 + c, v[c][l], gx, gy, o2 + l);
+        }
     } else {
         const int xs = o0 & (BX - 1);
         float v[NC][4];
@@ -737,19 +749,21 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
     // completed phases of every mbarrier an auxiliary role waits on (each role counts only what it uses)
     unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_cfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
 
-    for (;;) {
-        __syncthreads();
+    // One tile claim: CTA-wide barriers around the claim and around the late-start clearing.  Both role loops below call
+    // it the same number of times, so the barriers match although they are executed from two places.
+    auto next_tile = [&](TileJob& J) -> bool {
+        bar_sync(0, NT);
         if (tid == 0) {
             ctl.tile = (int)atomicAdd(P.counter, 1u);
             if (ld_volatile(P.abort_flag) != 0) ctl.abort = 1;
         }
-        __syncthreads();
-        if (ctl.tile >= P.ntiles || ctl.abort) break;
+        bar_sync(0, NT);
+        if (ctl.tile >= P.ntiles || ctl.abort) return false;
         // claim order = wavefront order (P.order sorts the tiles by bx+by+bz): the tiles in flight at any time lie on
         // one or two anti-diagonal planes and do not depend on each other, their upwind tiles were claimed a whole
         // tile lifetime earlier -- the hand-off latency then never stalls a step
         const int tile = P.order ? P.order[ctl.tile] : ctl.tile;
-        TileGeom t;
+        TileGeom& t = J.t;
         tile_init(P, tile, t);
         const int T = P.T;
         // a11: steps at which the tile's region lies wholly outside the grid do nothing and publish nothing.  The region
@@ -776,11 +790,27 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
 #pragma unroll
             for (int c = 0; c < Lay<COEF>::NC * BZ; ++c) cs[c * PLANE] = 0.0f;
         }
-        __syncthreads();
+        bar_sync(0, NT);
+        J.tile = tile; J.k0 = k0; J.k1 = k1; J.fast = fast;
+        return true;
+    };
 
-        if (warp < NWARPS_C) {
-            compute_tile<COEF>(P, t, tile, k0, k1, fast, sm, mb, ph);
-        } else if (warp == W_HPROD || warp == W_HAUX) {
+    // Register split (setmaxnreg): the launch gives each of the 640 threads 96 registers; uncapped the compute code wants
+    // ~140 (deeper load hoisting in the phases), the auxiliary warps need few.  Each role has its own tile loop so that
+    // the register budget of a region is the one set at its head.
+    if (warp < NWARPS_C) {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_COMPUTE));
+        TileJob J;
+        while (next_tile(J)) compute_tile<COEF>(P, J.t, J.tile, J.k0, J.k1, J.fast, sm, mb, ph);
+        return;
+    }
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_AUX));
+    TileJob J;
+    while (next_tile(J)) {
+        const TileGeom& t = J.t;
+        const int tile = J.tile, k0 = J.k0, k1 = J.k1, T = P.T;
+        const bool fast = J.fast;
+        if (warp == W_HPROD || warp == W_HAUX) {
             // H side: shell of step k needs the staging of step k-1 absorbed (HFREE), the upwind tiles' H of
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
             PROF_DECL;

@@ -746,8 +746,6 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
     // field copies then queue earlier against the coefficient copies), hence per instantiation.
     constexpr bool EARLY = !COEF;
     Phases ph = {0u, 0u, 0u, 0u, 0u};
-    // completed phases of every mbarrier an auxiliary role waits on (each role counts only what it uses)
-    unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_cfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
 
     // One tile claim: CTA-wide barriers around the claim and around the late-start clearing.  Both role loops below call
     // it the same number of times, so the barriers match although they are executed from two places.
@@ -805,6 +803,12 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         return;
     }
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_AUX));
+    // one instantiation of the auxiliary tile loop per role (the role is a compile-time constant inside): each keeps only
+    // its own phase counters and geometry alive
+    auto aux_loop = [&](auto rolec) {
+    constexpr int warp = decltype(rolec)::value;      // shadows the run-time warp index
+    // completed phases of every mbarrier this role waits on (each role counts only what it uses)
+    unsigned n_hfull = 0, n_cfull = 0, n_efull = 0, n_hfree = 0, n_cfree = 0, n_efree = 0, n_edone = 0, n_hdone = 0;
     TileJob J;
     while (next_tile(J)) {
         const TileGeom& t = J.t;
@@ -965,6 +969,11 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             }
         }
     }
+    };
+    if (warp == W_HPROD) aux_loop(std::integral_constant<int, W_HPROD>{});
+    else if (warp == W_HAUX) aux_loop(std::integral_constant<int, W_HAUX>{});
+    else if (warp == W_EPROD) aux_loop(std::integral_constant<int, W_EPROD>{});
+    else aux_loop(std::integral_constant<int, W_EPROD + 1>{});
 }
 
 }  // namespace

@@ -45,8 +45,9 @@ struct fdtd_ctx {
     unsigned int* d_counter;
     int* d_abort;
     long long* d_prof;   // FDTD_PROFILE build only
-    int* d_order;        // wavefront claim order of the TMA kernel, for order_nb[] tiles per axis
-    int order_nb[3];
+    int* d_order;        // wavefront claim order of the TMA kernel for the launch being enqueued
+    struct OrderEntry { int nb[3]; int* d; };
+    std::vector<OrderEntry> orders;   // one per tile-grid shape seen (fdtd_step(n) ends with a shorter launch: n = qT + r)
     int flag_base;
     long long spin_budget;
     unsigned int delay_seed;
@@ -275,7 +276,11 @@ int ensure_tmaps(fdtd_ctx* c)
 // tiles in flight at one time are mutually independent once a wavefront holds more tiles than there are CTAs.
 int ensure_order(fdtd_ctx* c, const int nb[3])
 {
-    if (c->d_order && c->order_nb[0] == nb[0] && c->order_nb[1] == nb[1] && c->order_nb[2] == nb[2]) return FDTD_OK;
+    for (const auto& o : c->orders)
+        if (o.nb[0] == nb[0] && o.nb[1] == nb[1] && o.nb[2] == nb[2]) {
+            c->d_order = o.d;
+            return FDTD_OK;
+        }
     const size_t nt = (size_t)nb[0] * nb[1] * nb[2];
     std::vector<int> h;
     h.reserve(nt);
@@ -288,15 +293,22 @@ int ensure_order(fdtd_ctx* c, const int nb[3])
                 if (x < nb[0]) h.push_back(x + nb[0] * (y + nb[1] * z));
             }
         }
-    cudaError_t e = cudaStreamSynchronize(c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
-    if (c->d_order) cudaFree(c->d_order);
-    c->d_order = nullptr;
-    e = cudaMalloc(&c->d_order, nt * sizeof(int));
+    if (c->orders.size() >= 8) {       // launches still in flight may read the oldest table: drain before freeing it
+        cudaError_t e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+        cudaFree(c->orders.front().d);
+        c->orders.erase(c->orders.begin());
+    }
+    fdtd_ctx::OrderEntry o;
+    for (int a = 0; a < 3; ++a) o.nb[a] = nb[a];
+    o.d = nullptr;
+    cudaError_t e = cudaMalloc(&o.d, nt * sizeof(int));
     if (e != cudaSuccess) return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(order): ") + cudaGetErrorString(e));
-    e = cudaMemcpy(c->d_order, h.data(), nt * sizeof(int), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(order)");
-    for (int a = 0; a < 3; ++a) c->order_nb[a] = nb[a];
+    e = cudaMemcpyAsync(o.d, h.data(), nt * sizeof(int), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);     // h is a local; once per tile-grid shape
+    if (e != cudaSuccess) { cudaFree(o.d); return cuda_fail(c, e, "cudaMemcpy(order)"); }
+    c->orders.push_back(o);
+    c->d_order = o.d;
     return FDTD_OK;
 }
 
@@ -476,7 +488,6 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->d_abort = nullptr;
     c->d_prof = nullptr;
     c->d_order = nullptr;
-    c->order_nb[0] = c->order_nb[1] = c->order_nb[2] = 0;
     c->flag_base = 0;
     c->delay_seed = 0;
     c->device = dev;
@@ -765,7 +776,7 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->d_flags) cudaFree(c->d_flags);
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);
-    if (c->d_order) cudaFree(c->d_order);
+    for (auto& o : c->orders) cudaFree(o.d);
     if (c->d_prof) {
         long long h[32];
         if (cudaMemcpy(h, c->d_prof, sizeof h, cudaMemcpyDeviceToHost) == cudaSuccess) {

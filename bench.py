@@ -195,7 +195,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     if not os.path.exists(binding.lib_path(args.variant)):
-        build.build()
+        build.build(which=(args.variant,))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     dist = None

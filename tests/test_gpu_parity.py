@@ -256,18 +256,96 @@ def test_full_size_config2_systolic_vs_oracle_and_naive(cuda_device, variant):
     compare((E2, H2), want, exact=True)
 
 
-def test_full_size_config5_window_oracle(cuda_device):
-    """BASELINE configs[4] at its full 1536x1536x768 (81 GiB resident, 64-bit offsets, 662k tiles per launch): the host
-    cannot hold the grid, so parity at scale uses windows: after s steps a w^3 window depends only
-    on inputs within s cells, so the oracle runs on a regenerated (w+2s)^3 sub-box (true walls where the box meets
-    them, any wall elsewhere) and the inner window must match bit for bit.  Windows: low corner, high corner, the
-    source, and a point where tile seams of all three axes meet."""
+def _window_oracle_check(w, s, win, origins, need_free):
+    """Parity at sizes the host cannot hold: after s steps a win^3 window depends only on inputs within
+    s cells, so the oracle runs on a regenerated (win+2s)^3 sub-box (true walls where the box meets them, any wall
+    elsewhere) and the inner window must match the device result bit for bit."""
     import torch
     free, _ = torch.cuda.mem_get_info()
-    if free < 100e9:
-        pytest.skip("needs ~90 GB of free device memory")
+    if free < need_free:
+        pytest.skip(f"needs {need_free / 1e9:.0f} GB of free device memory")
+    dev = torch.device("cuda:0")
+    E, H = workloads.make_fields(w, device=dev)
+    ca, cb = workloads.make_coeffs(w, device=dev)
+    src = workloads.make_source(w)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant="nofma")
+    sim.set_fields(E, H)
+    if ca is not None:
+        sim.set_coeffs(ca, cb)
+    if src is not None:
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC, None, s)
+    info = sim.get_kernel()
+    assert info["smem"] in (229632, 147456) and info["tiles"] > 100000
+    sim.step(s)
+    sim.sync()
+    nx, ny, nz = w.n
+    for (i0, j0, k0) in origins:
+        lo = [max(0, i0 - s), max(0, j0 - s), max(0, k0 - s)]
+        hi = [min(nx, i0 + win + s), min(ny, j0 + win + s), min(nz, k0 + win + s)]
+        box = (lo[0], lo[1], lo[2], hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2])
+        Eo, Ho = workloads.make_fields(w, window=box)
+        cao, cbo = workloads.make_coeffs(w, window=box)
+        orc = YeeOracle(box[3:], w.d, w.dt, w.boundary, Eo, Ho, cao, cbo, None)
+        if src is not None:
+            sb = src.box
+            if all(lo[a] <= sb[a] and sb[a] + sb[3 + a] <= hi[a] for a in range(3)):
+                orc.set_source(src.comp, (sb[0] - lo[0], sb[1] - lo[1], sb[2] - lo[2], sb[3], sb[4], sb[5]), src.amp, src.wave)
+        orc.step(s)
+        sl_o = (slice(k0 - lo[2], k0 - lo[2] + win), slice(j0 - lo[1], j0 - lo[1] + win), slice(i0 - lo[0], i0 - lo[0] + win))
+        sl_g = (slice(k0, k0 + win), slice(j0, j0 + win), slice(i0, i0 + win))
+        for g, o in zip(E + H, Eo + Ho):
+            got = g[sl_g].cpu().numpy()
+            assert np.array_equal(got, o[sl_o]), f"window at {(i0, j0, k0)}: max diff {np.abs(got - o[sl_o]).max():.3e}"
+    return E, H, sim
+
+
+def test_full_size_config5_window_oracle(cuda_device):
+    """BASELINE configs[4] at its full 1536x1536x768 (81 GiB resident, 64-bit offsets, 662k tiles per launch).  Windows:
+    low corner, high corner, the source, and a point where tile seams of all three axes meet."""
     w = workloads.config(4)
-    s, win = 32, 24
+    nx, ny, nz = w.n
+    win = 24
+    origins = [(0, 0, 0), (nx - win, ny - win, nz - win), (nx // 2 - win // 2, ny // 2 - win // 2, nz // 2 - win // 2),
+               (31 * 20 - win // 2, 15 * 40 - win // 2, 7 * 50 - win // 2)]
+    E, H, sim = _window_oracle_check(w, 32, win, origins, 100e9)
+    # the pulse has reached the source window (the comparison above is not 0 == 0 there)
+    assert float(E[2][nz // 2 - 2:nz // 2 + 2, ny // 2 - 2:ny // 2 + 2, nx // 2 - 2:nx // 2 + 2].abs().max()) > 0
+    sim.close()
+
+
+def test_full_size_config4_1024_window_oracle(cuda_device):
+    """The largest cube of the BASELINE configs[3] sweep (1024^3 random fields, uniform coefficients, 26 GB): windows at
+    the low corner, at the high walls and across tile seams in the middle, 32 steps in one launch."""
+    w = workloads.config(3, 1024)
+    win = 24
+    origins = [(0, 0, 0), (1024 - win, 1024 - win, 1024 - win), (31 * 16 - 10, 15 * 34 - 10, 7 * 73 - 10)]
+    _, _, sim = _window_oracle_check(w, 32, win, origins, 40e9)
+    sim.close()
+
+
+# degenerate grids through the TMA kernel: smaller than one tile, one cell thick, exactly one box, ragged beyond a box
+TINY = [(4, 4, 4), (8, 1, 1), (4, 1, 9), (32, 16, 8), (36, 3, 2), (64, 17, 5), (128, 2, 31)]
+
+
+@pytest.mark.parametrize("n", TINY)
+@pytest.mark.parametrize("coeffs", ["none", "lossy"])
+def test_tma_kernel_degenerate_grids(cuda_device, n, coeffs):
+    w = workloads.Workload(f"tiny{n}", n, (1.0, 0.7, 1.2), (PEC,) * 3, 23, "uniform", coeffs, "dipole")
+    steps = 23
+    want = oracle_run(w, steps)
+    for T in (1, 4, 23):
+        E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=T, variant="nofma")
+        assert info["smem"] in (229632, 147456)
+        compare((E, H), want, exact=True)
+    E, H, _ = gpu_run(w, steps, binding.KERNEL_NAIVE, variant="nofma")
+    compare((E, H), want, exact=True)
+
+
+def test_zero_steps_and_repeated_short_calls(cuda_device, oracle_results):
+    """fdtd_step(0) is a no-op; many one-step calls (one launch each, T = 1) equal one long call."""
+    import torch
+    w, steps = CASES["C5s"]
     dev = torch.device("cuda:0")
     E, H = workloads.make_fields(w, device=dev)
     ca, cb = workloads.make_coeffs(w, device=dev)
@@ -276,30 +354,10 @@ def test_full_size_config5_window_oracle(cuda_device):
     sim.set_fields(E, H)
     sim.set_coeffs(ca, cb)
     sim.set_source(src.comp, src.box, src.amp, src.wave)
-    sim.set_kernel(binding.KERNEL_SYSTOLIC, None, s)
-    info = sim.get_kernel()
-    assert info["smem"] in (229632, 147456) and info["tiles"] > 100000
-    sim.step(s)
+    sim.step(0)
+    for _ in range(steps):
+        sim.step(1)
     sim.sync()
-    nx, ny, nz = w.n
-    origins = [(0, 0, 0), (nx - win, ny - win, nz - win), (nx // 2 - win // 2, ny // 2 - win // 2, nz // 2 - win // 2),
-               (31 * 20 - win // 2, 15 * 40 - win // 2, 7 * 50 - win // 2)]
-    for (i0, j0, k0) in origins:
-        lo = [max(0, i0 - s), max(0, j0 - s), max(0, k0 - s)]
-        hi = [min(nx, i0 + win + s), min(ny, j0 + win + s), min(nz, k0 + win + s)]
-        box = (lo[0], lo[1], lo[2], hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2])
-        Eo, Ho = workloads.make_fields(w, window=box)
-        cao, cbo = workloads.make_coeffs(w, window=box)
-        orc = YeeOracle(box[3:], w.d, w.dt, w.boundary, Eo, Ho, cao, cbo, None)
-        sb = src.box
-        if all(lo[a] <= sb[a] and sb[a] + sb[3 + a] <= hi[a] for a in range(3)):
-            orc.set_source(src.comp, (sb[0] - lo[0], sb[1] - lo[1], sb[2] - lo[2], sb[3], sb[4], sb[5]), src.amp, src.wave)
-        orc.step(s)
-        sl_o = (slice(k0 - lo[2], k0 - lo[2] + win), slice(j0 - lo[1], j0 - lo[1] + win), slice(i0 - lo[0], i0 - lo[0] + win))
-        sl_g = (slice(k0, k0 + win), slice(j0, j0 + win), slice(i0, i0 + win))
-        for g, o in zip(E + H, Eo + Ho):
-            got = g[sl_g].cpu().numpy()
-            assert np.array_equal(got, o[sl_o]), f"window at {(i0, j0, k0)}: max diff {np.abs(got - o[sl_o]).max():.3e}"
-    # the pulse has reached the source window (the comparison above is not 0 == 0 there)
-    assert float(E[2][nz // 2 - 2:nz // 2 + 2, ny // 2 - 2:ny // 2 + 2, nx // 2 - 2:nx // 2 + 2].abs().max()) > 0
+    assert sim.time == steps
+    compare(([x.cpu().numpy() for x in E], [x.cpu().numpy() for x in H]), oracle_results("C5s"), exact=True)
     sim.close()

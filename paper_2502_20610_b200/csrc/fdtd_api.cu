@@ -82,14 +82,12 @@ bool coef_mixed(const fdtd_ctx* c) { return (c->g.ca[0] != nullptr) != (c->g.cb[
 int default_T(const fdtd_ctx* c)
 {
     // Temporal depth: a launch costs each tile one whole-box load and one whole-tile store (a6) and widens every PEC
-    // axis by T cells of partly filled ramp tiles (a11; wholly empty tile steps are skipped).  Measured on B200:
-    // 256^3 gains up to T = 64 (0.096 TCUPS; 0.089 at 32, 0.098 at 128), 512^3 likewise: n/4 clamped to [4, 64].
-    int m = 1 << 30;
-    for (int a = 0; a < 3; ++a)
-        if (!c->g.per[a] && c->g.n[a] < m) m = c->g.n[a];
-    int T = m == (1 << 30) ? 32 : m / 4;
-    if (T < 4) T = 4;
-    if (T > 64) T = 64;
+    // axis by T cells of ramp tiles (a11).  Since tiles skip the steps at which their region is outside the grid, a deep
+    // launch is cheap even on small grids; measured on B200 (TCUPS at T = 16 / 64 / 128): 64^3 0.021 / - / 0.044,
+    // 128^3 0.077 / - / 0.100, 256^3 (config 2) - / 0.102 / 0.106, 1024^3 - / 0.165 / 0.165.  (fdtd_step(n) with n < T
+    // runs one launch of n steps.)
+    (void)c;
+    int T = 128;
     if (const char* e = getenv("FDTD_T")) {
         const int v = atoi(e);
         if (v > 0) T = v;

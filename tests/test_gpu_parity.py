@@ -245,7 +245,7 @@ def test_api_errors(cuda_device):
 @pytest.mark.parametrize("variant", ["nofma"])
 def test_full_size_config2_systolic_vs_oracle_and_naive(cuda_device, variant):
     """BASELINE configs[1] at its full 256^3 size in the launch configuration bench.py times (library defaults),
-    shortened to 3 launches (96 steps; the oracle needs ~10 s for them): bit-exact against the oracle."""
+    shortened to 96 steps (the oracle needs ~10 s for them): bit-exact against the oracle."""
     w = workloads.config(1)
     steps = 96
     want = oracle_run(w, steps)

@@ -17,9 +17,12 @@
  *                         subdomain on chip, slide it along the x-y-z-t diagonal, exchange only faces through
  *                         global memory and hand off with per-tile flags.  It performs "the exact same update
  *                         equations", so results are identical per cell to the naive schedule.
- *                         Tile 31x15x7 runs the register-resident kernel (fields in registers, coefficients in
- *                         shared memory, loader warps staging the faces with cp.async); other built tile
- *                         shapes run the shared-memory kernel below.
+ *                         Tile 31x15x7 on a grid with all axes FDTD_PEC and nx % 4 == 0 runs the TMA-staged
+ *                         register kernel (fields in registers, coefficients in shared memory, shells fetched by
+ *                         TMA boxes); tile 31x15x7 elsewhere runs FDTD_KERNEL_SYSTOLIC_REG; other built tile
+ *                         shapes run FDTD_KERNEL_SYSTOLIC_SMEM.
+ *   FDTD_KERNEL_SYSTOLIC_REG   the same schedule and register residency with loader warps staging the shells by
+ *                         cp.async (any wall type, any nx; tile 31x15x7 only).
  *   FDTD_KERNEL_SYSTOLIC_SMEM  the same schedule with the whole subdomain in shared memory (the first,
  *                         simpler implementation; kept as a cross-check and for other tile shapes).
  *
@@ -66,6 +69,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
 /* Bind the six field arrays: E[3] = {Ex,Ey,Ez}, H[3] = {Hx,Hy,Hz}; host arrays of DEVICE pointers.
  * The buffers are BORROWED (config 5 is 81 GiB: no copy is affordable) and updated in place by fdtd_step;
  * they must stay valid until rebinding or fdtd_destroy, and must not alias each other.
+ * Performance note: when E[0..2] (and H[0..2]) sit at one positive stride (e.g. views of one [3][nz][ny][nx] block)
+ * the TMA kernel fetches all three components of a shell piece with a single 4-D box; any placement is correct.
  * FDTD_EINVAL: NULL or misaligned pointer.   (the six arrays of eq. (1) and its siblings) */
 int fdtd_set_fields(fdtd_ctx* ctx, float* const E[3], float* const H[3]);
 
@@ -78,7 +83,8 @@ int fdtd_load_fields(fdtd_ctx* ctx, const float* const E[3], const float* const 
  * ca[3], cb[3]: host arrays of DEVICE pointers to per-cell, per-component fp32 arrays (borrowed, read-only),
  *   ca == NULL -> ca_a = 1 everywhere (the multiply is skipped, which is exact);
  *   cb == NULL -> cb_a = dt everywhere (eq. (1)'s vacuum form with 1/d applied inside the curl).
- *   If ca / cb is non-NULL all three entries must be non-NULL.
+ *   If ca / cb is non-NULL all three entries must be non-NULL.  (Same note as for the fields: six arrays at one
+ *   stride, ca first, are fetched with one box per shell piece.)
  * db[3]: HOST array of three scalars (non-magnetic media); NULL -> {dt, dt, dt}.
  * Generator side (not the library's business): ca=(2eps-sigma dt)/(2eps+sigma dt), cb=2dt/(2eps+sigma dt). */
 int fdtd_set_coeffs(fdtd_ctx* ctx, const float* const ca[3], const float* const cb[3], const float db[3]);

@@ -159,7 +159,7 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def cpu_baseline(w):
+def cpu_baseline(w, config_steps):
     """The oracle timed beside the GPU run on a bounded sample (about 10-20 s of CPU work)."""
     from oracle.yee import YeeOracle
     from paper_2502_20610_b200 import workloads
@@ -177,7 +177,7 @@ def cpu_baseline(w):
     orc.step(n)
     dt = time.perf_counter() - t0
     return {"value": w.cells * n / dt / 1e12, "unit": "TCUPS", "cores": orc.nthreads, "kind": "oracle",
-            "sample": f"full {w.n[0]}x{w.n[1]}x{w.n[2]} grid, {n} of the config's {w.steps} time steps (after 2 warm-up steps)"}
+            "sample": f"full {w.n[0]}x{w.n[1]}x{w.n[2]} grid, {n} of the config's {config_steps} time steps (after 2 warm-up steps)"}
 
 
 def main():
@@ -329,7 +329,8 @@ def main():
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
-        line["cpu_baseline"] = cpu_baseline(w)
+        from paper_2502_20610_b200 import workloads as _wl
+        line["cpu_baseline"] = cpu_baseline(w, _wl.config(args.config, args.size or None).steps)
     print(json.dumps(line), flush=True)
     sim.close()
     if dist is not None:

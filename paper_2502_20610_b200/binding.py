@@ -15,7 +15,7 @@ KERNEL_NAIVE, KERNEL_SYSTOLIC, KERNEL_SYSTOLIC_SMEM, KERNEL_SYSTOLIC_REG = 0, 1,
 _ERRNAME = {1: "FDTD_EINVAL", 2: "FDTD_ENOMEM", 3: "FDTD_ECUDA", 4: "FDTD_ESTATE", 5: "FDTD_ETIMEOUT"}
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBFILES = {"fma": "libfdtd_b200.so", "nofma": "libfdtd_b200_nofma.so", "prof": "libfdtd_b200_prof.so"}
+_LIBFILES = {"fma": "libfdtd_b200.so", "nofma": "libfdtd_b200_nofma.so", "dbg": "libfdtd_b200_dbg.so", "prof": "libfdtd_b200_prof.so"}
 _libs = {}
 
 _F3 = C.c_void_p * 3

@@ -1,7 +1,13 @@
-"""Build libfdtd_b200.so (default, FMA contraction allowed) and libfdtd_b200_nofma.so (-fmad=false: bit-exact
-against the fp32 oracle) in-tree with nvcc for sm_100a.  nvcc cross-compiles without a GPU.
+"""Build the shared libraries in-tree with nvcc for sm_100a (nvcc cross-compiles without a GPU).
 
-    python -m paper_2502_20610_b200.build [--force] [--verbose]
+Product libraries:
+    libfdtd_b200.so        default, ptxas may contract mul+add into FMA
+    libfdtd_b200_nofma.so  -fmad=false: bit-exact against the fp32 oracle
+Developer libraries (-DFDTD_DEBUG: timing probes, fault injection, time-level shadow arrays; never the product path):
+    libfdtd_b200_dbg.so    -fmad=false -DFDTD_DEBUG   (perturbed-order, watchdog and level-shadow tests)
+    libfdtd_b200_prof.so   -DFDTD_DEBUG -DFDTD_PROFILE (clock64 section timers, dumped to stderr by fdtd_destroy)
+
+    python -m paper_2502_20610_b200.build [--force] [--verbose] [--all]
 """
 import os
 import subprocess
@@ -14,9 +20,10 @@ HEADERS = ["fdtd_internal.h", "fdtd_types.h", "yee_update.h", "systolic_tile.cuh
 LIBS = {
     "fma": (os.path.join(HERE, "libfdtd_b200.so"), []),
     "nofma": (os.path.join(HERE, "libfdtd_b200_nofma.so"), ["-fmad=false", "-DFDTD_NOFMA"]),
-    # developer build: clock64 section timers inside the systolic kernel, dumped to stderr by fdtd_destroy
-    "prof": (os.path.join(HERE, "libfdtd_b200_prof.so"), ["-DFDTD_PROFILE"]),
+    "dbg": (os.path.join(HERE, "libfdtd_b200_dbg.so"), ["-fmad=false", "-DFDTD_NOFMA", "-DFDTD_DEBUG"]),
+    "prof": (os.path.join(HERE, "libfdtd_b200_prof.so"), ["-DFDTD_DEBUG", "-DFDTD_PROFILE"]),
 }
+DEFAULT = ("fma", "nofma", "dbg")
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared", "--ftz=false", "--prec-div=true", "--prec-sqrt=true",
@@ -38,23 +45,29 @@ def _stale(lib):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False, which=("fma", "nofma")):
-    """Compile what is stale; returns {variant: path}."""
-    out = {}
+def build(force=False, verbose=False, which=DEFAULT):
+    """Compile what is stale (the variants side by side, nvcc --threads inside each); returns {variant: path}."""
+    out, jobs = {}, []
     for key in which:
         lib, extra = LIBS[key]
         if force or _stale(lib):
-            cmd = [_nvcc(), *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []),
+            cmd = [_nvcc(), *NVCC_FLAGS, "--threads", "0", *extra, *(["-Xptxas", "-v"] if verbose else []),
                    "-o", lib + ".tmp", *[os.path.join(CSRC, s) for s in SOURCES]]
-            res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
-            if verbose or res.returncode != 0:
-                sys.stderr.write(res.stdout + res.stderr)
-            if res.returncode != 0:
-                raise RuntimeError("nvcc failed: " + " ".join(cmd))
-            os.replace(lib + ".tmp", lib)
+            jobs.append((key, lib, cmd, subprocess.Popen(cmd, cwd=CSRC, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         out[key] = lib
+    failed = []
+    for key, lib, cmd, proc in jobs:
+        log, _ = proc.communicate()
+        if verbose or proc.returncode != 0:
+            sys.stderr.write(f"---- {key}\n{log}")
+        if proc.returncode != 0:
+            failed.append(" ".join(cmd))
+        else:
+            os.replace(lib + ".tmp", lib)
+    if failed:
+        raise RuntimeError("nvcc failed: " + failed[0])
     return out
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, which=tuple(LIBS) if "--all" in sys.argv else DEFAULT))

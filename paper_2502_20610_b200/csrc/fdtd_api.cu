@@ -50,7 +50,13 @@ struct fdtd_ctx {
     std::vector<OrderEntry> orders;   // one per tile-grid shape seen (fdtd_step(n) ends with a shorter launch: n = qT + r)
     int flag_base;
     long long spin_budget;
+    // tuning variables, read from the environment ONCE in fdtd_create (FDTD_T, FDTD_TILE, FDTD_SPIN_BUDGET_MS)
+    int env_T;
+    int env_tile[3];
+    // FDTD_DEBUG builds only (dbg / prof variants); always zero in the product libraries
     unsigned int delay_seed;
+    int dbg_skip, dbg_withhold;
+    bool dbg_no_tma, dbg_no_group, dbg_lex_order;
     // device
     int device, num_sms, clock_khz;
     cudaEvent_t ev0, ev1;
@@ -60,6 +66,21 @@ struct fdtd_ctx {
 };
 
 namespace {
+
+// Every entry point that touches the device runs on the device the context was created on, whatever device is
+// current in the calling thread, and leaves the caller's current device unchanged.
+struct DeviceGuard {
+    int prev;
+    bool switched;
+    explicit DeviceGuard(const fdtd_ctx* c) : prev(-1), switched(false)
+    {
+        if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 int fail(fdtd_ctx* c, int code, const std::string& msg)
 {
@@ -86,13 +107,7 @@ int default_T(const fdtd_ctx* c)
     // launch is cheap even on small grids; measured on B200 (TCUPS at T = 16 / 64 / 128): 64^3 0.021 / - / 0.044,
     // 128^3 0.077 / - / 0.100, 256^3 (config 2) - / 0.102 / 0.106, 1024^3 - / 0.165 / 0.165.  (fdtd_step(n) with n < T
     // runs one launch of n steps.)
-    (void)c;
-    int T = 128;
-    if (const char* e = getenv("FDTD_T")) {
-        const int v = atoi(e);
-        if (v > 0) T = v;
-    }
-    return T;
+    return c->env_T > 0 ? c->env_T : 128;
 }
 
 int resolve_systolic(fdtd_ctx* c)
@@ -104,26 +119,21 @@ int resolve_systolic(fdtd_ctx* c)
     if (N[0] == 0) {
         if (!smem_only || want_coef) { N[0] = 31; N[1] = 15; N[2] = 7; }
         else                         { N[0] = 31; N[1] = 15; N[2] = 15; }
-        if (const char* e = getenv("FDTD_TILE")) {
-            int x, y, z;
-            if (sscanf(e, "%dx%dx%d", &x, &y, &z) == 3) { N[0] = x; N[1] = y; N[2] = z; }
-        }
+        if (c->env_tile[0] > 0) { N[0] = c->env_tile[0]; N[1] = c->env_tile[1]; N[2] = c->env_tile[2]; }
     }
     c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
     c->use_tma = c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->g.per[0] && !c->g.per[1] && !c->g.per[2] &&
-                 c->g.n[0] % 4 == 0 && !getenv("FDTD_NO_TMA");
+                 c->g.n[0] % 4 == 0 && !c->dbg_no_tma;
     int found = -1;
-    int threads = 0;
+    int per_sm = 0;
     if (c->use_tma) {
-        cudaError_t e = systolic_tma_prepare(want_coef);
-        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+        cudaError_t e = systolic_tma_prepare(want_coef, &per_sm);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
         c->smem = systolic_tma_smem(want_coef);
-        threads = systolic_tma_threads();
     } else if (c->use_reg) {
-        cudaError_t e = systolic_reg_prepare(want_coef);
-        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+        cudaError_t e = systolic_reg_prepare(want_coef, &per_sm);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
         c->smem = systolic_reg_smem(want_coef);
-        threads = systolic_reg_threads();
     } else {
         for (int i = 0; i < systolic_num_configs(); ++i) {
             const SysConfig* s = systolic_config(i);
@@ -135,16 +145,13 @@ int resolve_systolic(fdtd_ctx* c)
                      want_coef ? "with" : "without");
             return fail(c, FDTD_EINVAL, buf);
         }
-        cudaError_t e = systolic_prepare(found);
-        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory)");
+        cudaError_t e = systolic_prepare(found, &per_sm);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
         c->smem = systolic_config(found)->smem;
-        threads = systolic_config(found)->threads;
     }
-    // persistent grid: every CTA resident at once
-    int per_sm = (int)((227u * 1024u) / (c->smem + 1024u));
-    if (per_sm < 1) per_sm = 1;
-    int by_threads = 2048 / threads;
-    if (per_sm > by_threads) per_sm = by_threads;
+    // persistent grid: every CTA resident at once.  Residency comes from the occupancy query of the chosen function
+    // (registers, threads and shared memory), because a ring of tiles deadlocks if a CTA of it is not resident.
+    if (per_sm < 1) return fail(c, FDTD_ECUDA, "the systolic kernel does not fit on an SM of this device");
     if (per_sm > 4) per_sm = 4;
     c->ctas = c->num_sms * per_sm;
     c->T = c->reqT > 0 ? c->reqT : default_T(c);
@@ -217,7 +224,7 @@ int ensure_tmaps(fdtd_ctx* c)
     const cuuint64_t nbytes = (cuuint64_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * 4u;
     // arrays first..first+count-1 at one positive stride (multiple of 16 bytes, no overlap)? -> the stride, else 0
     auto uniform_stride = [&](int first, int count) -> cuuint64_t {
-        if (!arr[first] || getenv("FDTD_TMA_NO_GROUP")) return 0;
+        if (!arr[first] || c->dbg_no_group) return 0;
         const char* b0 = (const char*)arr[first];
         const char* b1 = (const char*)arr[first + 1];
         if (b1 <= b0) return 0;
@@ -315,7 +322,7 @@ int ensure_order(fdtd_ctx* c, const int nb[3])
 // cp.async systolic kernel (a ring of tiles advances in lock step: 0.015 vs 0.070 TCUPS on config 3).
 bool tma_eligible(const fdtd_ctx* c)
 {
-    return !c->g.per[0] && !c->g.per[1] && !c->g.per[2] && c->g.n[0] % 4 == 0 && !coef_mixed(c) && !getenv("FDTD_NO_TMA");
+    return !c->g.per[0] && !c->g.per[1] && !c->g.per[2] && c->g.n[0] % 4 == 0 && !coef_mixed(c) && !c->dbg_no_tma;
 }
 
 int effective_kernel(const fdtd_ctx* c)
@@ -375,7 +382,7 @@ int step_systolic(fdtd_ctx* c, int n)
             c->flag_base = 0;
         }
         P.order = nullptr;
-        if (c->use_tma && !getenv("FDTD_LEX_ORDER")) {
+        if (c->use_tma && !c->dbg_lex_order) {
             const int nb[3] = {P.ax[0].nb, P.ax[1].nb, P.ax[2].nb};
             const int rc2 = ensure_order(c, nb);
             if (rc2 != FDTD_OK) return rc2;
@@ -393,7 +400,8 @@ int step_systolic(fdtd_ctx* c, int n)
         P.delay_seed = c->delay_seed;
         P.prof = c->d_prof;
         for (int g = 0; g < 3; ++g) P.tma_group[g] = c->tma_group[g];
-        P.dbg = getenv("FDTD_DEBUG_SKIP") ? atoi(getenv("FDTD_DEBUG_SKIP")) : 0;
+        P.dbg = c->dbg_skip;
+        P.withhold_tile = c->dbg_withhold;
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
@@ -488,13 +496,30 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->d_order = nullptr;
     c->flag_base = 0;
     c->delay_seed = 0;
+    c->dbg_skip = 0;
+    c->dbg_withhold = -1;
+    c->dbg_no_tma = c->dbg_no_group = c->dbg_lex_order = false;
+    c->env_T = 0;
+    c->env_tile[0] = c->env_tile[1] = c->env_tile[2] = 0;
+    if (const char* env = getenv("FDTD_T")) c->env_T = atoi(env);
+    if (const char* env = getenv("FDTD_TILE")) {
+        int x, y, z;
+        if (sscanf(env, "%dx%dx%d", &x, &y, &z) == 3 && x > 0 && y > 0 && z > 0) { c->env_tile[0] = x; c->env_tile[1] = y; c->env_tile[2] = z; }
+    }
+#ifdef FDTD_DEBUG
+    if (const char* env = getenv("FDTD_DEBUG_DELAY")) c->delay_seed = (unsigned int)strtoul(env, nullptr, 10);
+    if (const char* env = getenv("FDTD_DEBUG_SKIP")) c->dbg_skip = atoi(env);
+    if (const char* env = getenv("FDTD_DEBUG_WITHHOLD")) c->dbg_withhold = atoi(env);
+    c->dbg_no_tma = getenv("FDTD_DEBUG_NO_TMA") != nullptr;
+    c->dbg_no_group = getenv("FDTD_DEBUG_NO_GROUP") != nullptr;
+    c->dbg_lex_order = getenv("FDTD_DEBUG_LEX_ORDER") != nullptr;
+#endif
     c->device = dev;
     c->num_sms = prop.multiProcessorCount;
     c->clock_khz = prop.clockRate;
     double budget_ms = 10000.0;
     if (const char* env = getenv("FDTD_SPIN_BUDGET_MS")) budget_ms = atof(env);
     c->spin_budget = (long long)(budget_ms * (double)(prop.clockRate > 0 ? prop.clockRate : 1965000));
-    if (const char* env = getenv("FDTD_DEBUG_DELAY")) c->delay_seed = (unsigned int)strtoul(env, nullptr, 10);
     c->ev_valid = false;
     memset(c->counters, 0, sizeof c->counters);
     e = cudaMalloc(&c->d_counter, sizeof(unsigned int));
@@ -534,6 +559,7 @@ int fdtd_set_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
 int fdtd_load_fields(fdtd_ctx* c, const float* const E[3], const float* const H[3])
 {
     if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_load_fields before fdtd_set_fields");
     const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * sizeof(float);
     for (int a = 0; a < 3; ++a) {
@@ -572,6 +598,7 @@ int fdtd_set_source(fdtd_ctx* c, int comp, int i0, int j0, int k0, int ni, int n
                     const float* wave, int nwave)
 {
     if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     cudaError_t e = cudaStreamSynchronize(c->stream);   // the old tables may still be in use
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
     if (c->d_amp) cudaFree(c->d_amp);
@@ -608,6 +635,7 @@ int fdtd_set_source(fdtd_ctx* c, int comp, int i0, int j0, int k0, int ni, int n
 int fdtd_step(fdtd_ctx* c, int n)
 {
     if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     if (n < 0) return fail(c, FDTD_EINVAL, "fdtd_step: n < 0");
     if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_step before fdtd_set_fields");
     cudaError_t e = cudaEventRecord(c->ev0, c->stream);
@@ -622,12 +650,14 @@ int fdtd_step(fdtd_ctx* c, int n)
 int fdtd_sync(fdtd_ctx* c)
 {
     if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     return check_async(c);
 }
 
 int fdtd_get_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
 {
     if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     const int rc = check_async(c);
     if (rc != FDTD_OK) return rc;
     if (!E && !H) return FDTD_OK;
@@ -660,11 +690,13 @@ long long fdtd_get_time(const fdtd_ctx* c) { return c ? c->t : -1; }
 int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
 {
     if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     if (which != FDTD_KERNEL_NAIVE && which != FDTD_KERNEL_SYSTOLIC && which != FDTD_KERNEL_SYSTOLIC_SMEM && which != FDTD_KERNEL_SYSTOLIC_REG) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: unknown kernel");
     if (Nx < 0 || Ny < 0 || Nz < 0 || T < 0) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: negative argument");
     if ((Nx == 0) != (Ny == 0) || (Nx == 0) != (Nz == 0)) return fail(c, FDTD_EINVAL, "fdtd_set_kernel: give all of Nx,Ny,Nz or none");
     const int oldN[3] = {c->reqN[0], c->reqN[1], c->reqN[2]};
     const int oldT = c->reqT, oldw = c->which;
+    const bool old_explicit = c->which_explicit;
     c->which = which;
     c->which_explicit = true;
     c->reqN[0] = Nx; c->reqN[1] = Ny; c->reqN[2] = Nz;
@@ -675,6 +707,7 @@ int fdtd_set_kernel(fdtd_ctx* c, int which, int Nx, int Ny, int Nz, int T)
         const int rc = resolve_systolic(c);
         if (rc != FDTD_OK) {
             c->which = oldw; c->reqT = oldT;
+            c->which_explicit = old_explicit;
             c->reqN[0] = oldN[0]; c->reqN[1] = oldN[1]; c->reqN[2] = oldN[2];
             c->cfg_idx = -1;
             c->resolved = false;
@@ -688,6 +721,7 @@ int fdtd_get_kernel(const fdtd_ctx* cc, int out[8])
 {
     fdtd_ctx* c = const_cast<fdtd_ctx*>(cc);
     if (!c || !out) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     memset(out, 0, 8 * sizeof(int));
     out[0] = effective_kernel(c);
     if (out[0] != FDTD_KERNEL_NAIVE) {
@@ -717,6 +751,7 @@ int fdtd_get_counters(const fdtd_ctx* c, long long out[4])
 int fdtd_last_step_ms(fdtd_ctx* c, float* ms)
 {
     if (!c || !ms) return FDTD_EINVAL;
+    DeviceGuard guard(c);
     if (!c->ev_valid) return fail(c, FDTD_ESTATE, "fdtd_last_step_ms before fdtd_step");
     cudaError_t e = cudaEventSynchronize(c->ev1);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventSynchronize");
@@ -768,6 +803,7 @@ const char* fdtd_build_info(void)
 void fdtd_destroy(fdtd_ctx* c)
 {
     if (!c) return;
+    DeviceGuard guard(c);
     cudaStreamSynchronize(c->stream);
     if (c->d_amp) cudaFree(c->d_amp);
     if (c->d_wave) cudaFree(c->d_wave);

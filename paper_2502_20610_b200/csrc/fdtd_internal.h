@@ -15,17 +15,18 @@ int systolic_num_configs();
 const SysConfig* systolic_config(int idx);
 // returns cudaSuccess and launches `ctas` persistent CTAs of configuration cfg_idx
 cudaError_t launch_systolic(int cfg_idx, const SysParams& p, int ctas, cudaStream_t st);
-cudaError_t systolic_prepare(int cfg_idx);   // set max dynamic smem attribute
+// set the max-dynamic-shared-memory attribute; *blocks_per_sm = resident CTAs per SM by the occupancy query
+cudaError_t systolic_prepare(int cfg_idx, int* blocks_per_sm);
 
 // implemented in systolic_reg.cu: the register-resident systolic kernel, tile 31x15x7 in a 32x16x8 box
 size_t systolic_reg_smem(int coef);
 int systolic_reg_threads();
-cudaError_t systolic_reg_prepare(int coef);
+cudaError_t systolic_reg_prepare(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_reg(int coef, const SysParams& p, int ctas, cudaStream_t st);
 
 // implemented in systolic_tma.cu: the TMA-staged systolic kernel (PEC grids, nx % 4 == 0), tile 31x15x7
 size_t systolic_tma_smem(int coef);
 int systolic_tma_threads();
 void systolic_tma_boxes(int box[3][3]);   // TMA box extents (x,y,z) of the z-plane, y-row and x-column shell pieces
-cudaError_t systolic_tma_prepare(int coef);
+cudaError_t systolic_tma_prepare(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);

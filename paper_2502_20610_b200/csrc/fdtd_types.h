@@ -58,6 +58,17 @@ inline AxisPlan make_axis_plan(int n, int per, int N, int T)
     return a;
 }
 
+// Developer builds only (-DFDTD_DEBUG: the "dbg" and "prof" variants of build.py): timing probes that skip work
+// (results invalid), fault injection (pseudo-random sleeps, a withheld flag) and the time-level shadow arrays.
+// The product libraries compile every one of them out: FDTD_DBG() is the constant false there.
+#ifdef FDTD_DEBUG
+#define FDTD_DBG(P, bit) (((P).dbg & (bit)) != 0)
+#define FDTD_DEBUG_ONLY(...) __VA_ARGS__
+#else
+#define FDTD_DBG(P, bit) false
+#define FDTD_DEBUG_ONLY(...)
+#endif
+
 struct SysParams {
     GridParams g;
     AxisPlan ax[3];
@@ -73,9 +84,14 @@ struct SysParams {
     const int* order;      // systolic_tma.cu: claim index -> tile, sorted by wavefront bx+by+bz (NULL: identity)
     int tma_group[3];      // systolic_tma.cu, per group (E, H, coefficients): 0 per-array 3-D maps, 1 one 4-D map per piece, 2 two triples
     long long* prof;       // FDTD_PROFILE build: 32 tick accumulators (NULL otherwise)
+    // FDTD_DEBUG builds only (always 0 / NULL in the product libraries, and never read there):
     int dbg;               // FDTD_DEBUG_SKIP timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes,
                            // 16 no coefficient scatter, 32 no proxy fence, 64 no skipping of empty tile steps
-    unsigned int delay_seed; // debug: != 0 inserts pseudo-random sleeps to perturb the inter-CTA order
+    unsigned int delay_seed; // != 0 inserts pseudo-random sleeps to perturb the inter-CTA order (FDTD_DEBUG_DELAY)
+    int withhold_tile;     // >= 0: this tile never raises its flags, so the hand-off watchdog must fire (FDTD_DEBUG_WITHHOLD)
+    int* levE;             // time-level shadow arrays, one int per cell (FDTD_DEBUG_LEVELS): number of E / H updates the
+    int* levH;             //   value stored in global memory has received; every shell load asserts the level it expects
+    unsigned long long* lev_err;   // [0] = number of violations, [1..4] = first violation (kind, cell index, found, expected)
 };
 
 // 36 CUtensorMap (128 bytes each) passed to systolic_tma.cu as a __grid_constant__ kernel parameter:

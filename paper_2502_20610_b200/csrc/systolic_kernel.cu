@@ -83,6 +83,7 @@ __device__ __forceinline__ void publish_flag(int* flag, int value)
     }
 }
 
+#ifdef FDTD_DEBUG
 __device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k, int phase)
 {
     if (P.delay_seed == 0u) return;
@@ -93,6 +94,7 @@ __device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k,
     }
     __syncthreads();
 }
+#endif
 
 template <int BX, int BY, int BZ, bool COEF, int ZSPLIT>
 __global__ void __launch_bounds__(BX * BY * ZSPLIT, 1) systolic_kernel(const __grid_constant__ SysParams P)
@@ -124,12 +126,12 @@ __global__ void __launch_bounds__(BX * BY * ZSPLIT, 1) systolic_kernel(const __g
                 t.load_h_shell(P, sm, tid);
             }
             __syncthreads();
-            debug_delay(P, tile, k, 0);
+            FDTD_DEBUG_ONLY(debug_delay(P, tile, k, 0);)
             t.e_phase(P, sm, tid);
             __syncthreads();
             t.publish_e(P, sm, tid);
             publish_flag(P.flagE + tile, P.flag_base + k + 1);
-            debug_delay(P, tile, k, 1);
+            FDTD_DEBUG_ONLY(debug_delay(P, tile, k, 1);)
             if (!wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl)) return;
             t.load_e_shell(P, sm, tid);
             __syncthreads();
@@ -192,12 +194,14 @@ const SysConfig* systolic_config(int idx)
     return (idx >= 0 && idx < n) ? &e[idx].cfg : nullptr;
 }
 
-cudaError_t systolic_prepare(int idx)
+cudaError_t systolic_prepare(int idx, int* blocks_per_sm)
 {
     int n;
     const Entry* e = table(&n);
     if (idx < 0 || idx >= n) return cudaErrorInvalidValue;
-    return cudaFuncSetAttribute(e[idx].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e[idx].cfg.smem);
+    cudaError_t err = cudaFuncSetAttribute(e[idx].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)e[idx].cfg.smem);
+    if (err != cudaSuccess) return err;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, e[idx].fn, e[idx].cfg.threads, e[idx].cfg.smem);
 }
 
 cudaError_t launch_systolic(int idx, const SysParams& p, int ctas, cudaStream_t st)

@@ -169,7 +169,7 @@ __device__ __forceinline__ void tile_init(const SysParams& P, int tile, TileGeom
 __device__ __forceinline__ void wait_upwind(const SysParams& P, const TileGeom& t, const int* flags, int target, Ctl* ctl)
 {
     const int lane = threadIdx.x & 31;
-    if (lane < 7 && *(volatile int*)&ctl->abort == 0 && !(P.dbg & 1)) {
+    if (lane < 7 && *(volatile int*)&ctl->abort == 0 && !FDTD_DBG(P, 1)) {
         const int u = t.nbr[lane];
         if (u >= 0) {
             const long long t_start = clock64();
@@ -190,6 +190,7 @@ __device__ __forceinline__ void wait_upwind(const SysParams& P, const TileGeom& 
     __syncwarp();
 }
 
+#ifdef FDTD_DEBUG
 __device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k, int phase)
 {
     if (P.delay_seed == 0u) return;
@@ -197,6 +198,7 @@ __device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k,
     h ^= h >> 15; h *= 2246822519u; h ^= h >> 13; h *= 3266489917u; h ^= h >> 16;
     if ((h & 3u) == 0u) __nanosleep((h >> 8) & 0x3fffu);   // up to ~16 us, one phase in four
 }
+#endif
 
 // ---- loader warps: minus shell of the box of step k, NARR field arrays (+ six coefficient arrays) ---------
 // part / nparts split the work between the loader warps of one kind.
@@ -215,7 +217,7 @@ __device__ __forceinline__ void load_shell(const SysParams& P, const TileGeom& t
         int gx, gy, gz;
         const bool in = resolve(P, 0, o0 + lx, gx) & resolve(P, 1, o1 + ly, gy) & resolve(P, 2, o2 + lz, gz);
         const long long off = in ? gx + nx * (gy + ny * (long long)gz) : 0;
-        if (P.dbg & 2) return;
+        if (FDTD_DBG(P, 2)) return;
 #pragma unroll
         for (int c = 0; c < 3; ++c) cp_async4(d0 + c * dstride, fld[c] + off, in);
         if (COEF && WITH_COEF) {
@@ -399,7 +401,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exEx[(l + 1) * PLANE + slot] = ex[l + 1];
             }
             // publish E of R_k \ R_{k+1} (everything at the last step)                                  (a8, a6)
-            if (colE && !(P.dbg & 4)) {
+            if (colE && !FDTD_DBG(P, 4)) {
                 const bool whole = last || lx == w0 || ly == w1;
                 if (whole) {
 #pragma unroll
@@ -425,7 +427,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         bar_arrive(BAR_EDONE, N_EDONE);
-        if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);
+        FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);)
 
         // ---------------- E minus shell -------------------------------------------------------------------------
         mbar_wait(mbE, phE & 1u);
@@ -480,7 +482,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exHx[m * PLANE + slot] = hx[m];
             }
             // publish H of R_{k+1} \ R_{k+2}: frame-k planes l = w-1 (everything at the last step)       (a8, a6)
-            if (colH && !(P.dbg & 4)) {
+            if (colH && !FDTD_DBG(P, 4)) {
                 const bool whole = last || lx == w0 - 1 || ly == w1 - 1;
                 if (whole) {
 #pragma unroll
@@ -506,7 +508,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         bar_arrive(BAR_HDONE, N_HDONE);
-        if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);
+        FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);)
     }
 }
 
@@ -563,12 +565,12 @@ __global__ void __launch_bounds__(NT, 1) systolic_reg_kernel(const __grid_consta
             for (int k = 0; k < T; ++k) {
                 bar_sync(BAR_EDONE, N_EDONE);
                 if (lane == 0) {
-                    if (!(P.dbg & 8)) __threadfence();
+                    if (!FDTD_DBG(P, 8)) __threadfence();
                     st_release(P.flagE + tile, P.flag_base + k + 1);
                 }
                 bar_sync(BAR_HDONE, N_HDONE);
                 if (lane == 0) {
-                    if (!(P.dbg & 8)) __threadfence();
+                    if (!FDTD_DBG(P, 8)) __threadfence();
                     st_release(P.flagH + tile, P.flag_base + k + 1);
                 }
             }
@@ -581,10 +583,12 @@ __global__ void __launch_bounds__(NT, 1) systolic_reg_kernel(const __grid_consta
 size_t systolic_reg_smem(int coef) { return (size_t)(coef ? Lay<true>::total : Lay<false>::total) * sizeof(float); }
 int systolic_reg_threads() { return NT; }
 
-cudaError_t systolic_reg_prepare(int coef)
+cudaError_t systolic_reg_prepare(int coef, int* blocks_per_sm)
 {
     const void* fn = coef ? (const void*)&systolic_reg_kernel<true> : (const void*)&systolic_reg_kernel<false>;
-    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)systolic_reg_smem(coef));
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)systolic_reg_smem(coef));
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, fn, NT, systolic_reg_smem(coef));
 }
 
 cudaError_t launch_systolic_reg(int coef, const SysParams& p, int ctas, cudaStream_t st)

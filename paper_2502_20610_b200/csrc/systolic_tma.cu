@@ -1,13 +1,17 @@
-// systolic_tma.cu -- the systolic FDTD kernel for sm_100a, TMA-staged version (the product kernel on PEC grids).
+// systolic_tma.cu -- the systolic FDTD kernel for sm_100a, TMA-staged version (the product kernel).
 //
-// Schedule: exactly that of systolic_reg.cu / DESIGN.md section 4 (tile regions R_k = [a-k, a+w-k) sliding along
-// the x-y-z-t diagonal; one E phase and one H phase per step; minus-shell loads and
-// plus-shell publishes through global memory; per-tile acquire/release flags on the seven upwind
-// neighbours).  What differs is how a B200 SM executes it:
+// Schedule: DESIGN.md section 6.2 (tile regions R_k = [a-k, a+w-k) sliding along the x-y-z-t diagonal, PAPER.md:94;
+// one E phase and one H phase per step; minus-shell loads and plus-shell publishes through global
+// memory; per-tile acquire/release flags on the seven upwind neighbours).  How a B200 SM
+// executes it:
 //
-//   * box 32 x 16 x 8 cells (tile 31 x 15 x 7).  Compute thread (lane, warp) owns the (x,y) slot
-//     (gx mod 32, gy mod 16) and keeps the 8-cell z column of all six field components in REGISTERS; the slide
-//     in x/y is modular addressing, the slide in z a register renaming inside the unrolled z march.
+//   * box 32 x 16 x 8 cells (tile 31 x 15 x 7).  Compute thread (lane, warp w) owns the x slot gx mod 32 and the TWO
+//     y slots 2w, 2w+1 (gy mod 16) and keeps both 8-cell z columns of all six field components in REGISTERS
+//     (102 registers); the slide in x/y is modular addressing, the slide in z a register renaming inside the
+//     unrolled z march.  Neighbours: z = registers, x = warp shuffle, y = the thread's other row for half of the
+//     links and a shared-memory exchange row (written by the neighbouring warp) for the other half.
+//   * the (ca, cb) pair of every resident cell and component sits in a thread-private shared-memory slot and is read
+//     with one 64-bit load.
 //   * the compute warps execute NO per-cell predicate: walls and the outside of the domain are data.  Cells
 //     outside the grid are zero-filled by TMA (fields and coefficients), so E stays 0 there (the PEC ghost,
 //     reading #5); frozen wall components get (ca, cb) = (1, 0) when their coefficients enter the chip; shell
@@ -19,26 +23,29 @@
 //     entering row/column coefficients into the owner threads' private shared-memory slots and repack the x column
 //     so that its single owner lane absorbs it with 16-byte loads.
 //   * every hand-off inside the CTA is an mbarrier with one elected arrive per warp; the only CTA-wide barrier is the
-//     512-thread named barrier between absorb and phase.
+//     256-thread named barrier between absorb and phase.
+//   * ONE gpu-scope fence per step: the signal warp copies the leaving x columns of E and of H out of shared memory
+//     (acknowledging each at once, so the compute warps never wait for the fence), stores them, fences, and raises
+//     flagE and flagH together.
 //   * tiles are claimed in wavefront order (bx+by+bz) and skip the steps at which their region lies outside the grid.
 //
-//   compute (warps 0-15)         warp 16: field H shell      warp 17: coefficient shell   warp 18: field E shell     warp 19: flags
+//   compute (warps 0-7)          warp 8: field H shell       warp 9: coefficient shell    warp 10: field E shell     warp 11: flags
 //   --------------------         ------------------------    -------------------------    -----------------------    ---------------
 //   wait HREADY(k), absorb H     poll flagH[u] >= base+k     wait CFREE(k-1)              poll flagE[u] >= base+k+1
 //     -> HFREE                   fence.proxy.async           TMA coefficient shell k      fence.proxy.async
 //   E phase k                    wait HFREE(k-1)             wait EDONE(k-1), landed      wait EFREE(k-1)
 //   wait CREADY(k), absorb       TMA H shell k               scatter row + column         TMA E shell k, landed
 //     coefficient plane -> CFREE wait landed, pack x column  -> CREADY(k)                 pack x column
-//   wait ACKE(k-1), publish E    -> HREADY(k)                (no coefficient arrays: also wait HDONE(k-1)            wait EDONE(k): x column,
-//     -> EDONE                                                raises flagH, see below)    write E exchange column      flagE = base+k+1 -> ACKE
-//   wait EREADY(k), absorb E                                                              -> EREADY(k)               wait HDONE(k): x column,
-//     -> EFREE                                                                                                         flagH = base+k+1 -> ACKH
-//   H phase k
-//   wait ACKH(k-1), publish H -> HDONE
+//   wait ACKE(k-1), publish E    -> HREADY(k)                                             wait HDONE(k-1)            wait EDONE(k): x column
+//     -> EDONE                                                                            write E exchange column      -> registers -> ACKE
+//   wait EREADY(k), absorb E                                                              -> EREADY(k)               wait HDONE(k): x column
+//     -> EFREE                                                                                                         -> registers -> ACKH
+//   H phase k                                                                                                        store both columns, fence,
+//   wait ACKH(k-1), publish H -> HDONE                                                                                 flagE = flagH = base+k+1
 //
 // Per-cell arithmetic is yee_update.h, unchanged: with -fmad=false the result is bit-identical to the oracle.
-// Scope: all three axes PEC and nx % 4 == 0 (TMA strides are multiples of 16 bytes); other grids run
-// systolic_reg.cu.
+// Scope: every axis is a wall axis of the (possibly padded) grid and nx % 4 == 0 (TMA strides are
+// multiples of 16 bytes); P.g.per[] only says which low walls freeze tangential E.
 #include <cuda.h>
 
 #include <type_traits>
@@ -50,13 +57,19 @@ namespace {
 
 constexpr int BX = 32, BY = 16, BZ = 8;
 constexpr int W0 = BX - 1, W1 = BY - 1, W2 = BZ - 1;   // tile widths (PEC axes: always full)
-constexpr int NCOMPUTE = BX * BY;                       // 512 (x,y) slots = compute threads
+#ifndef FDTD_NROW
+#define FDTD_NROW 1
+#endif
+constexpr int NROW = FDTD_NROW;                         // y slots (rows) per compute thread: 1 or 2
+constexpr int NWARPS_C = BY / NROW;                     // compute warps: warp w owns the y slots NROW*w .. NROW*w + NROW-1
+constexpr int NCOMPUTE = 32 * NWARPS_C;                 // compute threads
 constexpr int SX = BX + 1;                              // row stride of the slot-indexed shared arrays: a column of
 constexpr int PLANE = SX * BY;                          // slots (the entering x column) then spans 16 banks, not one
-constexpr int NWARPS_C = NCOMPUTE / 32;
 constexpr int NT = NCOMPUTE + 128;
-constexpr int REGS_COMPUTE = 104, REGS_AUX = 64;     // 512*104 + 128*64 = 61440 = 640*96; (112, 32) spills in the aux warps and is 10 % slower
-constexpr int W_HPROD = 16, W_HAUX = 17, W_EPROD = 18;   // warp 19: signal
+// NROW = 1: the launch gives each of the 640 threads 96 registers: compute warps grow to 104, auxiliary warps shrink to 64
+// (512*104 + 128*64 = 61440 = 640*96).  NROW = 2: 384 threads of 168 registers: 256*208 + 128*64 = 61440 <= 64512.
+constexpr int REGS_COMPUTE = NROW == 1 ? 104 : 208, REGS_AUX = 64;
+constexpr int W_HPROD = NWARPS_C, W_HAUX = NWARPS_C + 1, W_EPROD = NWARPS_C + 2;   // warp NWARPS_C + 3: signal
 
 // staging of one array's minus shell (floats); every TMA destination is 128-byte aligned
 // TMA needs the innermost start coordinate on a 16-byte boundary, the shell slides by one cell per step: every
@@ -78,7 +91,8 @@ constexpr unsigned BYTES_ARR = F_ARR * 4u;   // bytes TMA delivers per array and
 
 template <bool COEF>
 struct Lay {
-    static constexpr int NC = COEF ? 6 : 3;            // resident coefficient arrays (no COEF: cb masks only)
+    static constexpr int NC = COEF ? 6 : 3;            // resident coefficient floats per cell: COEF: three (ca, cb) pairs,
+                                                       // [(c*BZ + z slot)*PLANE + slot] as float2; else three cb masks as float
     static constexpr int stgh = 0;
     static constexpr int stge = stgh + 3 * F_ARR;
     static constexpr int stgc = stge + 3 * F_ARR;
@@ -120,6 +134,17 @@ __device__ __forceinline__ int ld_acquire(const int* p)
 __device__ __forceinline__ void st_release(int* p, int v)
 {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// a9: publish "tile has finished phase v - flag_base"; cumulative over every store the calling thread has observed
+__device__ __forceinline__ void raise_flag(const SysParams& P, int* flags, int tile, int v)
+{
+    FDTD_DEBUG_ONLY(if (tile == P.withhold_tile) return;)   // fault injection: the downwind tiles' watchdog must fire
+    st_release(flags + tile, v);
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+__device__ __forceinline__ void st_relaxed(int* p, int v)
+{
+    asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ int ld_volatile(const int* p)
 {
@@ -194,17 +219,19 @@ __device__ __forceinline__ void tile_init(const SysParams& P, int tile, TileGeom
     }
 }
 
-// frozen tangential E on the low PEC walls (reading #5): component c of the cell at (gx,gy,gz)
-__device__ __forceinline__ bool frozen(int c, int gx, int gy, int gz)
+// frozen tangential E on the low PEC walls (reading #5): component c of the cell at (gx,gy,gz).  An axis with
+// P.g.per[a] != 0 has no wall (a periodic axis running on its padded copy): nothing freezes there.
+__device__ __forceinline__ bool frozen(const SysParams& P, int c, int gx, int gy, int gz)
 {
-    return c == 0 ? (gy == 0) | (gz == 0) : c == 1 ? (gz == 0) | (gx == 0) : (gx == 0) | (gy == 0);
+    const bool fx = (gx == 0) & (P.g.per[0] == 0), fy = (gy == 0) & (P.g.per[1] == 0), fz = (gz == 0) & (P.g.per[2] == 0);
+    return c == 0 ? fy | fz : c == 1 ? fz | fx : fx | fy;
 }
 
 // lanes 0..6 of the calling warp each watch one upwind neighbour (a9); watchdog as in systolic_reg.cu
 __device__ __forceinline__ void wait_upwind(const SysParams& P, const TileGeom& t, const int* flags, int target, Ctl* ctl)
 {
     const int lane = threadIdx.x & 31;
-    if (lane < 7 && *(volatile int*)&ctl->abort == 0 && !(P.dbg & 1)) {
+    if (lane < 7 && *(volatile int*)&ctl->abort == 0 && !FDTD_DBG(P, 1)) {
         const int u = t.nbr[lane];
         if (u >= 0 && ld_acquire(flags + u) < target) {
             const long long t_start = clock64();
@@ -225,12 +252,14 @@ __device__ __forceinline__ void wait_upwind(const SysParams& P, const TileGeom& 
     __syncwarp();
 }
 
+#ifdef FDTD_DEBUG
 __device__ __forceinline__ void debug_delay(const SysParams& P, int tile, int k, int phase)
 {
     unsigned h = P.delay_seed ^ (unsigned)(tile * 2654435761u) ^ (unsigned)(k * 40503u + phase * 97u);
     h ^= h >> 15; h *= 2246822519u; h ^= h >> 13; h *= 3266489917u; h ^= h >> 16;
     if ((h & 3u) == 0u) __nanosleep((h >> 8) & 0x3fffu);   // up to ~16 us, one phase in four
 }
+#endif
 
 __device__ __forceinline__ void tma_load_4d(float* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, unsigned long long* bar)
 {
@@ -269,62 +298,74 @@ __device__ __forceinline__ void issue_shell(const CUtensorMap* maps, int grouped
     }
 }
 
-// coefficient value of component slot c (COEF: ca 0..2, cb 3..5; else cb masks 0..2) for the cell at (gx,gy,gz):
-// staged value v, except frozen wall components -> (ca, cb) = (1, 0); no COEF: dt inside the grid, else 0
-template <bool COEF>
-__device__ __forceinline__ float coef_value(const SysParams& P, int c, float v, int gx, int gy, int gz)
+// cb mask of component c for the cell at (gx,gy,gz) when there are no coefficient arrays: dt inside the grid, 0 on
+// frozen wall components and outside the grid
+__device__ __forceinline__ float cb_mask(const SysParams& P, int c, int gx, int gy, int gz)
 {
-    if (COEF) return frozen(c % 3, gx, gy, gz) ? (c < 3 ? 1.0f : 0.0f) : v;
     const bool in = ((unsigned)gx < (unsigned)P.g.n[0]) & ((unsigned)gy < (unsigned)P.g.n[1]) & ((unsigned)gz < (unsigned)P.g.n[2]);
-    return (in && !frozen(c, gx, gy, gz)) ? P.g.cb_scalar : 0.0f;
+    return (in && !frozen(P, c, gx, gy, gz)) ? P.g.cb_scalar : 0.0f;
+}
+// (ca, cb) pair of component c as it enters the chip: the staged values, except frozen wall components -> (1, 0)
+__device__ __forceinline__ float2 coef_pair(const SysParams& P, int c, float a, float b, int gx, int gy, int gz)
+{
+    return frozen(P, c, gx, gy, gz) ? make_float2(1.0f, 0.0f) : make_float2(a, b);
 }
 
-// ---- H-side auxiliary warps: coefficients of the entering row and column -> the owner threads' private slots ----
-// (the entering plane l_z = 0 is absorbed by the compute threads themselves).  Warp part 0 takes the row l_y = 0,
+// ---- H-side auxiliary warp: coefficients of the entering row and column -> the owner threads' private slots ----
+// (the entering plane l_z = 0 is absorbed by the compute threads themselves).  Part 0 takes the row l_y = 0,
 // part 1 the column l_x = 0; loads of a batch are issued before its stores.
 template <bool COEF>
 __device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int o0, int o1, int o2, int part)
 {
-    constexpr int NC = Lay<COEF>::NC;
     const int lane = threadIdx.x & 31;
     const float* stg = sm + Lay<COEF>::stgc;
-    float* coef = sm + Lay<COEF>::coef;
     const int r0 = o0 & 3;
     if (part == 0) {
         const int gx = o0 + lane, gy = o1;
-        float* dst = coef + (gy & (BY - 1)) * SX + (gx & (BX - 1));
-        // loads of a batch first (staging and slots are the same array to the compiler); three components per batch keep
-        // the auxiliary warps inside their 64-register budget
+        const int slot = (gy & (BY - 1)) * SX + (gx & (BX - 1));
+        if (COEF) {
+            float2* dst = reinterpret_cast<float2*>(sm + Lay<COEF>::coef) + slot;
 #pragma unroll
-        for (int c0 = 0; c0 < NC; c0 += 3) {
-            float v[3][BZ];
+            for (int c = 0; c < 3; ++c) {
+                float a[BZ], b[BZ];
+#pragma unroll
+                for (int l = 1; l < BZ; ++l) {
+                    a[l] = stg[yidx<6>(c, l, r0 + lane)];
+                    b[l] = stg[yidx<6>(3 + c, l, r0 + lane)];
+                }
+#pragma unroll
+                for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_pair(P, c, a[l], b[l], gx, gy, o2 + l);
+            }
+        } else {
+            float* dst = sm + Lay<COEF>::coef + slot;
 #pragma unroll
             for (int c = 0; c < 3; ++c)
 #pragma unroll
-                for (int l = 1; l < BZ; ++l) v[c][l] = COEF ? stg[yidx<6>(c0 + c, l, r0 + lane)] : 0.0f;
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int l = 1; l < BZ; ++l) dst[((c0 + c) * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_value<COEF>(P, c0 + c, v[c][l], gx, gy, o2 + l);
+                for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = cb_mask(P, c, gx, gy, o2 + l);
         }
     } else {
         const int xs = o0 & (BX - 1);
-        float v[NC][4];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {            // 105 cells: idx = (l-1)*15 + (ly-1)
+        for (int r = 0; r < (W1 * W2 + 31) / 32; ++r) {            // 105 cells: idx = (l-1)*15 + (ly-1)
             const int idx = r * 32 + lane;
             const int ly = 1 + idx % W1, l = 1 + idx / W1;
+            const int slot = ((o2 + l) & (BZ - 1)) * PLANE + ((o1 + ly) & (BY - 1)) * SX + xs;
+            if (COEF) {
+                float a[3], b[3];
 #pragma unroll
-            for (int c = 0; c < NC; ++c) v[c][r] = (COEF && idx < W1 * W2) ? stg[xidx<6>(c, ly, l) + r0] : 0.0f;
-        }
+                for (int c = 0; c < 3; ++c) {
+                    a[c] = idx < W1 * W2 ? stg[xidx<6>(c, ly, l) + r0] : 0.0f;
+                    b[c] = idx < W1 * W2 ? stg[xidx<6>(3 + c, ly, l) + r0] : 0.0f;
+                }
+                if (idx < W1 * W2) {
+                    float2* d = reinterpret_cast<float2*>(sm + Lay<COEF>::coef) + slot;
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int idx = r * 32 + lane;
-            const int ly = 1 + idx % W1, l = 1 + idx / W1;
-            if (idx < W1 * W2) {
-                float* d = coef + ((o2 + l) & (BZ - 1)) * PLANE + ((o1 + ly) & (BY - 1)) * SX + xs;
+                    for (int c = 0; c < 3; ++c) d[c * BZ * PLANE] = coef_pair(P, c, a[c], b[c], o0, o1 + ly, o2 + l);
+                }
+            } else if (idx < W1 * W2) {
+                float* d = sm + Lay<COEF>::coef + slot;
 #pragma unroll
-                for (int c = 0; c < NC; ++c) d[c * BZ * PLANE] = coef_value<COEF>(P, c, v[c][r], o0, o1 + ly, o2 + l);
+                for (int c = 0; c < 3; ++c) d[c * BZ * PLANE] = cb_mask(P, c, o0, o1 + ly, o2 + l);
             }
         }
     }
@@ -351,25 +392,41 @@ __device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, 
     }
 }
 
-// signal warp: the leaving x column (global x = gx) of three field arrays, rows ly = ly_lo..ly_hi, six planes starting
-// at local plane l_lo, from xo[(y slot*3 + c)*8 + l] to global memory                                    (a8)
-__device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld, const float* xo, int gx, int o1, int o2, int ly_lo, int ly_hi, int l_lo)
+// signal warp: the leaving x column of three field arrays, rows ly = ly_lo..ly_hi, six planes starting at local plane
+// l_lo, is copied from xo[(y slot*3 + c)*8 + l] into registers (load_xcol; the shared rows are free again as soon as
+// it returns) and later stored to global memory at x = gx (store_xcol)                                        (a8)
+constexpr int XROUNDS = (BY * (W2 - 1) + 31) / 32;
+struct XCol {
+    float v[XROUNDS][3];
+};
+__device__ __forceinline__ void load_xcol(XCol& x, const float* xo, int l_lo)
+{
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int r = 0; r < XROUNDS; ++r) {
+        const int item = r * 32 + lane;            // y slot * 6 + plane
+        const float* v = xo + (item / (W2 - 1)) * 24 + l_lo + item % (W2 - 1);
+        x.v[r][0] = v[0];
+        x.v[r][1] = v[8];
+        x.v[r][2] = v[16];
+    }
+}
+__device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld, const XCol& x, int gx, int o1, int o2, int ly_lo, int ly_hi, int l_lo)
 {
     const int lane = threadIdx.x & 31;
     if ((unsigned)gx >= (unsigned)P.g.n[0]) return;
     const long long nx = P.g.n[0], plane = nx * P.g.n[1];
 #pragma unroll
-    for (int r = 0; r < 3; ++r) {
-        const int item = r * 32 + lane;            // y slot * 6 + plane
-        const int ys = item / 6, l = l_lo + item % 6;
+    for (int r = 0; r < XROUNDS; ++r) {
+        const int item = r * 32 + lane;
+        const int ys = item / (W2 - 1), l = l_lo + item % (W2 - 1);
         const int ly = (ys - o1) & (BY - 1);
         const int gy = o1 + ly, gz = o2 + l;
         if (ly >= ly_lo && ly <= ly_hi && (unsigned)gy < (unsigned)P.g.n[1] && (unsigned)gz < (unsigned)P.g.n[2]) {
             const long long off = gx + nx * gy + plane * gz;
-            const float* v = xo + ys * 24 + l;
-            __stcg(fld[0] + off, v[0]);
-            __stcg(fld[1] + off, v[8]);
-            __stcg(fld[2] + off, v[16]);
+            __stcg(fld[0] + off, x.v[r][0]);
+            __stcg(fld[1] + off, x.v[r][1]);
+            __stcg(fld[2] + off, x.v[r][2]);
         }
     }
 }
@@ -395,9 +452,12 @@ struct Phases {   // completed phases of each mbarrier as seen by this thread's 
 template <bool COEF>
 __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, int k0, int k1, bool fast, float* sm, unsigned long long* mb, Phases& ph)
 {
-    const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
-    const int slot = wy * SX + lane;
-    const int slot_ym = ((wy - 1) & (BY - 1)) * SX + lane, slot_yp = ((wy + 1) & (BY - 1)) * SX + lane;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    constexpr int RL = NROW - 1;                                // the thread's last row
+    const int ys0 = NROW * w;                                   // this thread's y slots (rows): ys0 .. ys0 + RL
+    const int slot0 = ys0 * SX + lane, slot1 = slot0 + RL * SX; // slots of the first and of the last row
+    const int slot_ym = ((ys0 - 1) & (BY - 1)) * SX + lane;     // the row below row 0 = last row of warp w-1
+    const int slot_yp = ((ys0 + NROW) & (BY - 1)) * SX + lane;  // the row above the last row = row 0 of warp w+1
     const int lane_m = (lane - 1) & 31, lane_p = (lane + 1) & 31;
     const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
     const long long plane = (long long)nx * ny;
@@ -406,24 +466,31 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     const float* stgE = sm + Lay<COEF>::stge;
     const float* xpkH = sm + Lay<COEF>::xpkh;
     const float* xpkE = sm + Lay<COEF>::xpke;
-    float* exHz = sm + Lay<COEF>::exch;
+    // y exchange: only the links between a thread's row 1 and the next warp's row 0 go through shared memory
+    float* exHz = sm + Lay<COEF>::exch;       // H_z, H_x of row 1 for the E phase of the next warp's row 0
     float* exHx = exHz + EXP;
-    float* exEz = exHx + EXP;
+    float* exEz = exHx + EXP;                 // E_z, E_x of row 0 for the H phase of the previous warp's row 1
     float* exEx = exEz + EXP;
-    float* coef = sm + Lay<COEF>::coef + slot;   // this thread's private coefficient slots: [(c*BZ + z slot)*PLANE]
+    // this thread's private coefficient slots, row 0 (row 1: + SX): index (c*BZ + z slot)*PLANE; float2 (ca, cb) pairs
+    // with coefficient arrays, float cb masks without
+    float* const cmask = sm + Lay<COEF>::coef + slot0;
+    float2* const cpair = reinterpret_cast<float2*>(sm + Lay<COEF>::coef) + slot0;
 
     const float rdx = P.g.rd[0], rdy = P.g.rd[1], rdz = P.g.rd[2];
     const float dbx = P.g.db[0], dby = P.g.db[1], dbz = P.g.db[2];
     float* const Ex = P.g.E[0]; float* const Ey = P.g.E[1]; float* const Ez = P.g.E[2];
     float* const Hx = P.g.H[0]; float* const Hy = P.g.H[1]; float* const Hz = P.g.H[2];
 
-    // frame k: local l <-> global z = o2 + l.  E(l) lives in e?[l] before the E phase and in e?[l+1] after it;
-    // H(l) lives in h?[l] before the H phase and in h?[l+1] (= frame k+1 index) after it.
-    float ex[BZ + 1], ey[BZ + 1], ez[BZ + 1], hx[BZ], hy[BZ], hz[BZ];
+    // frame k: local l <-> global z = o2 + l.  E(l) lives in e?[r][l] before the E phase and in e?[r][l+1] after it;
+    // H(l) lives in h?[r][l] before the H phase and in h?[r][l+1] (= frame k+1 index) after it.  r = row 0 / 1.
+    float ex[NROW][BZ + 1], ey[NROW][BZ + 1], ez[NROW][BZ + 1], hx[NROW][BZ], hy[NROW][BZ], hz[NROW][BZ];
 #pragma unroll
-    for (int l = 0; l <= BZ; ++l) ex[l] = ey[l] = ez[l] = 0.0f;
+    for (int r = 0; r < NROW; ++r) {
 #pragma unroll
-    for (int l = 0; l < BZ; ++l) hx[l] = hy[l] = hz[l] = 0.0f;
+        for (int l = 0; l <= BZ; ++l) ex[r][l] = ey[r][l] = ez[r][l] = 0.0f;
+#pragma unroll
+        for (int l = 0; l < BZ; ++l) hx[r][l] = hy[r][l] = hz[r][l] = 0.0f;
+    }
 
     const int T = P.T;
     PROF_DECL;
@@ -431,67 +498,91 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         const bool last = (k == T - 1);
         PROF_MARK(7);
         const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
-        const int lx = (lane - o0) & (BX - 1), ly = (wy - o1) & (BY - 1);
-        const int gx = o0 + lx, gy = o1 + ly;
-        const bool col_in = ((unsigned)gx < (unsigned)nx) & ((unsigned)gy < (unsigned)ny);
-        const long long col_off = col_in ? gx + (long long)nx * gy : 0;
+        const int lx = (lane - o0) & (BX - 1);
+        const int gx = o0 + lx;
+        const int xs = (o0 & 3) + lx;          // position inside a staged row
+        int ly[NROW], gy[NROW];
+        bool col_in[NROW];
+        long long col_off[NROW];
+#pragma unroll
+        for (int r = 0; r < NROW; ++r) {
+            ly[r] = (ys0 + r - o1) & (BY - 1);
+            gy[r] = o1 + ly[r];
+            col_in[r] = ((unsigned)gx < (unsigned)nx) & ((unsigned)gy[r] < (unsigned)ny);
+            col_off[r] = col_in[r] ? gx + (long long)nx * gy[r] : 0;
+        }
+        // the entering shell row l_y = 0 is row 0 of one warp or row 1 of one warp (warp-uniform tests)
 
         // ---------------- H (+ coefficient) minus shell ----------------------------------------------------
         if (k == 0) {
             // a6: the whole box straight from global memory; H and coefficients on [0,w]^3, E on R_0 = [1,w]^3
 #pragma unroll
-            for (int l = 0; l < BZ; ++l) {
-                const int gz = o2 + l;
-                const bool ok = col_in && (unsigned)gz < (unsigned)nz;
-                const long long off = ok ? col_off + plane * gz : 0;
-                hx[l] = ok ? __ldcg(Hx + off) : 0.0f;
-                hy[l] = ok ? __ldcg(Hy + off) : 0.0f;
-                hz[l] = ok ? __ldcg(Hz + off) : 0.0f;
-                const bool oke = ok && lx >= 1 && ly >= 1 && l >= 1;
-                ex[l] = oke ? __ldcg(Ex + off) : 0.0f;
-                ey[l] = oke ? __ldcg(Ey + off) : 0.0f;
-                ez[l] = oke ? __ldcg(Ez + off) : 0.0f;
-                float* cs = coef + (gz & (BZ - 1)) * PLANE;
+            for (int r = 0; r < NROW; ++r) {
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const bool fr = frozen(c, gx, gy, gz);
-                    if (COEF) {
-                        const float a = ok ? __ldg(P.g.ca[c] + off) : 0.0f;
-                        const float b = ok ? __ldg(P.g.cb[c] + off) : 0.0f;
-                        cs[c * (BZ * PLANE)] = fr ? 1.0f : a;
-                        cs[(3 + c) * (BZ * PLANE)] = fr ? 0.0f : b;
-                    } else {
-                        cs[c * (BZ * PLANE)] = (ok && !fr) ? P.g.cb_scalar : 0.0f;
+                for (int l = 0; l < BZ; ++l) {
+                    const int gz = o2 + l;
+                    const bool ok = col_in[r] && (unsigned)gz < (unsigned)nz;
+                    const long long off = ok ? col_off[r] + plane * gz : 0;
+                    hx[r][l] = ok ? __ldcg(Hx + off) : 0.0f;
+                    hy[r][l] = ok ? __ldcg(Hy + off) : 0.0f;
+                    hz[r][l] = ok ? __ldcg(Hz + off) : 0.0f;
+                    const bool oke = ok && lx >= 1 && ly[r] >= 1 && l >= 1;
+                    ex[r][l] = oke ? __ldcg(Ex + off) : 0.0f;
+                    ey[r][l] = oke ? __ldcg(Ey + off) : 0.0f;
+                    ez[r][l] = oke ? __ldcg(Ez + off) : 0.0f;
+                    const int cidx = r * SX + (gz & (BZ - 1)) * PLANE;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        if (COEF) {
+                            const float a = ok ? __ldg(P.g.ca[c] + off) : 0.0f;
+                            const float b = ok ? __ldg(P.g.cb[c] + off) : 0.0f;
+                            cpair[cidx + c * (BZ * PLANE)] = coef_pair(P, c, a, b, gx, gy[r], gz);
+                        } else {
+                            cmask[cidx + c * (BZ * PLANE)] = cb_mask(P, c, gx, gy[r], gz);
+                        }
                     }
                 }
             }
 #pragma unroll
             for (int l = 1; l < BZ; ++l) {
-                exHz[(l - 1) * PLANE + slot] = hz[l];
-                exHx[(l - 1) * PLANE + slot] = hx[l];
+                exHz[(l - 1) * PLANE + slot1] = hz[RL][l];
+                exHx[(l - 1) * PLANE + slot1] = hx[RL][l];
             }
         } else {
             mbar_wait(mb + MB_HREADY, ph.hready & 1u);
             ++ph.hready;
-            const int xs = (o0 & 3) + lx;     // position inside a staged row
-            hx[0] = stgH[zidx<3>(0, ly, xs)];
-            hy[0] = stgH[zidx<3>(1, ly, xs)];
-            hz[0] = stgH[zidx<3>(2, ly, xs)];
-            if (ly == 0) {            // warp-uniform: the entering row; its y+1 neighbours read it from the exchange
 #pragma unroll
-                for (int l = 1; l < BZ; ++l) {
-                    hx[l] = stgH[yidx<3>(0, l, xs)];
-                    hy[l] = stgH[yidx<3>(1, l, xs)];
-                    hz[l] = stgH[yidx<3>(2, l, xs)];
-                    exHz[(l - 1) * PLANE + slot] = hz[l];
-                    exHx[(l - 1) * PLANE + slot] = hx[l];
+            for (int r = 0; r < NROW; ++r) {
+                hx[r][0] = stgH[zidx<3>(0, ly[r], xs)];
+                hy[r][0] = stgH[zidx<3>(1, ly[r], xs)];
+                hz[r][0] = stgH[zidx<3>(2, ly[r], xs)];
+            }
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
+                if (ly[r] == 0) {         // warp-uniform: the entering row
+#pragma unroll
+                    for (int l = 1; l < BZ; ++l) {
+                        hx[r][l] = stgH[yidx<3>(0, l, xs)];
+                        hy[r][l] = stgH[yidx<3>(1, l, xs)];
+                        hz[r][l] = stgH[yidx<3>(2, l, xs)];
+                        if (r == RL) {    // its y+1 neighbour is the next warp's row 0, which reads it from the exchange
+                            exHz[(l - 1) * PLANE + slot1] = hz[r][l];
+                            exHx[(l - 1) * PLANE + slot1] = hx[r][l];
+                        }
+                    }
                 }
-            } else if (lx == 0) {     // one lane per warp: the entering column, packed by the H-side warps
-                const float4* s4 = reinterpret_cast<const float4*>(xpkH + wy * 24);
-                const float4 a0 = s4[0], a1 = s4[1], b0 = s4[2], b1 = s4[3], c0 = s4[4], c1 = s4[5];
-                hx[1] = a0.y; hx[2] = a0.z; hx[3] = a0.w; hx[4] = a1.x; hx[5] = a1.y; hx[6] = a1.z; hx[7] = a1.w;
-                hy[1] = b0.y; hy[2] = b0.z; hy[3] = b0.w; hy[4] = b1.x; hy[5] = b1.y; hy[6] = b1.z; hy[7] = b1.w;
-                hz[1] = c0.y; hz[2] = c0.z; hz[3] = c0.w; hz[4] = c1.x; hz[5] = c1.y; hz[6] = c1.z; hz[7] = c1.w;
+            }
+            if (lx == 0) {                // one lane per warp: the entering column, packed by the H-side warp
+#pragma unroll
+                for (int r = 0; r < NROW; ++r) {
+                    if (ly[r] != 0) {
+                        const float4* s4 = reinterpret_cast<const float4*>(xpkH + (ys0 + r) * 24);
+                        const float4 a0 = s4[0], a1 = s4[1], b0 = s4[2], b1 = s4[3], c0 = s4[4], c1 = s4[5];
+                        hx[r][1] = a0.y; hx[r][2] = a0.z; hx[r][3] = a0.w; hx[r][4] = a1.x; hx[r][5] = a1.y; hx[r][6] = a1.z; hx[r][7] = a1.w;
+                        hy[r][1] = b0.y; hy[r][2] = b0.z; hy[r][3] = b0.w; hy[r][4] = b1.x; hy[r][5] = b1.y; hy[r][6] = b1.z; hy[r][7] = b1.w;
+                        hz[r][1] = c0.y; hz[r][2] = c0.z; hz[r][3] = c0.w; hz[r][4] = c1.x; hz[r][5] = c1.y; hz[r][6] = c1.z; hz[r][7] = c1.w;
+                    }
+                }
             }
             warp_arrive(mb + MB_HFREE);
         }
@@ -505,31 +596,36 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         constexpr bool FAST = decltype(fastc)::value;
 #pragma unroll
         for (int l = BZ - 1; l >= 1; --l) {
-            const float hz_xm = __shfl_sync(0xffffffffu, hz[l], lane_m);
-            const float hy_xm = __shfl_sync(0xffffffffu, hy[l], lane_m);
+            const int cidx = ((o2 + l) & (BZ - 1)) * PLANE;
             const float hz_ym = exHz[(l - 1) * PLANE + slot_ym];
             const float hx_ym = exHx[(l - 1) * PLANE + slot_ym];
-            const float* cs = coef + ((o2 + l) & (BZ - 1)) * PLANE;
-            float cax = 1.0f, cay = 1.0f, caz = 1.0f, cbx, cby, cbz;
-            if (COEF) {
-                cax = cs[0 * (BZ * PLANE)]; cay = cs[1 * (BZ * PLANE)]; caz = cs[2 * (BZ * PLANE)];
-                cbx = cs[3 * (BZ * PLANE)]; cby = cs[4 * (BZ * PLANE)]; cbz = cs[5 * (BZ * PLANE)];
-            } else if (FAST) {
-                cbx = cby = cbz = P.g.cb_scalar;
-            } else {
-                cbx = cs[0 * (BZ * PLANE)]; cby = cs[1 * (BZ * PLANE)]; cbz = cs[2 * (BZ * PLANE)];
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
+                const float hz_xm = __shfl_sync(0xffffffffu, hz[r][l], lane_m);
+                const float hy_xm = __shfl_sync(0xffffffffu, hy[r][l], lane_m);
+                // y-1 neighbour: row 0 reads the previous warp's last row from the exchange, row 1 reads row 0's registers
+                const float hz_y = r == 0 ? hz_ym : hz[r > 0 ? r - 1 : 0][l];
+                const float hx_y = r == 0 ? hx_ym : hx[r > 0 ? r - 1 : 0][l];
+                float cax = 1.0f, cay = 1.0f, caz = 1.0f, cbx, cby, cbz;
+                if (COEF) {
+                    const float2 px = cpair[cidx + r * SX], py = cpair[cidx + r * SX + BZ * PLANE], pz = cpair[cidx + r * SX + 2 * BZ * PLANE];
+                    cax = px.x; cbx = px.y; cay = py.x; cby = py.y; caz = pz.x; cbz = pz.y;
+                } else if (FAST) {
+                    cbx = cby = cbz = P.g.cb_scalar;
+                } else {
+                    cbx = cmask[cidx + r * SX]; cby = cmask[cidx + r * SX + BZ * PLANE]; cbz = cmask[cidx + r * SX + 2 * BZ * PLANE];
+                }
+                // E_x: (Hz - Hz[j-1])/dy - (Hy - Hy[k-1])/dz      eq. (1)
+                ex[r][l + 1] = yee_e_update<COEF>(ex[r][l], hz[r][l], hz_y, hy[r][l], hy[r][l - 1], rdy, rdz, cax, cbx);
+                // E_y: (Hx - Hx[k-1])/dz - (Hz - Hz[i-1])/dx
+                ey[r][l + 1] = yee_e_update<COEF>(ey[r][l], hx[r][l], hx[r][l - 1], hz[r][l], hz_xm, rdz, rdx, cay, cby);
+                // E_z: (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy
+                ez[r][l + 1] = yee_e_update<COEF>(ez[r][l], hy[r][l], hy_xm, hx[r][l], hx_y, rdx, rdy, caz, cbz);
             }
-            // E_x: (Hz - Hz[j-1])/dy - (Hy - Hy[k-1])/dz      eq. (1)
-            ex[l + 1] = yee_e_update<COEF>(ex[l], hz[l], hz_ym, hy[l], hy[l - 1], rdy, rdz, cax, cbx);
-            // E_y: (Hx - Hx[k-1])/dz - (Hz - Hz[i-1])/dx
-            ey[l + 1] = yee_e_update<COEF>(ey[l], hx[l], hx[l - 1], hz[l], hz_xm, rdz, rdx, cay, cby);
-            // E_z: (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy
-            ez[l + 1] = yee_e_update<COEF>(ez[l], hy[l], hy_xm, hx[l], hx_ym, rdx, rdy, caz, cbz);
         }
         };
         if (!COEF && fast) e_phase(std::true_type{});
         else e_phase(std::false_type{});
-        const bool actE = (lx >= 1) & (ly >= 1);            // column belongs to R_k
         // soft source after the E update of step t0 + k (a4): rare, CTA-uniform test first
         {
             const long long ts = P.t0 + k;
@@ -537,29 +633,34 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 P.g.src_box[0] <= o0 + W0 && P.g.src_box[0] + P.g.src_box[3] > o0 + 1 &&
                 P.g.src_box[1] <= o1 + W1 && P.g.src_box[1] + P.g.src_box[4] > o1 + 1 &&
                 P.g.src_box[2] <= o2 + W2 && P.g.src_box[2] + P.g.src_box[5] > o2 + 1) {
-                const int sx = gx - P.g.src_box[0], sy = gy - P.g.src_box[1];
-                if (actE && sx >= 0 && sx < P.g.src_box[3] && sy >= 0 && sy < P.g.src_box[4]) {
-                    const float wsrc = __ldg(P.g.src_wave + ts);
+                const float wsrc = __ldg(P.g.src_wave + ts);
+                const int sx = gx - P.g.src_box[0];
 #pragma unroll
-                    for (int l = 1; l < BZ; ++l) {
-                        const int sz = o2 + l - P.g.src_box[2];
-                        if (sz >= 0 && sz < P.g.src_box[5]) {
-                            const float amp = __ldg(P.g.src_amp + (sx + P.g.src_box[3] * (sy + (long long)P.g.src_box[4] * sz)));
-                            const float inj = amp * wsrc;
-                            if (P.g.src_comp == 0) ex[l + 1] = ex[l + 1] + inj;
-                            else if (P.g.src_comp == 1) ey[l + 1] = ey[l + 1] + inj;
-                            else ez[l + 1] = ez[l + 1] + inj;
+                for (int r = 0; r < NROW; ++r) {
+                    const int sy = gy[r] - P.g.src_box[1];
+                    if ((lx >= 1) & (ly[r] >= 1) && sx >= 0 && sx < P.g.src_box[3] && sy >= 0 && sy < P.g.src_box[4]) {
+#pragma unroll
+                        for (int l = 1; l < BZ; ++l) {
+                            const int sz = o2 + l - P.g.src_box[2];
+                            if (sz >= 0 && sz < P.g.src_box[5]) {
+                                const float amp = __ldg(P.g.src_amp + (sx + P.g.src_box[3] * (sy + (long long)P.g.src_box[4] * sz)));
+                                const float inj = amp * wsrc;
+                                if (P.g.src_comp == 0) ex[r][l + 1] = ex[r][l + 1] + inj;
+                                else if (P.g.src_comp == 1) ey[r][l + 1] = ey[r][l + 1] + inj;
+                                else ez[r][l + 1] = ez[r][l + 1] + inj;
+                            }
                         }
                     }
                 }
             }
         }
-        // E of planes 1..6 for the y+1 readers of the H phase; the shell column lx = 0 is written by the E-side warp
+        // E of row 0, planes 1..6, for the previous warp's row 1 in the H phase; the shell column lx = 0 is written by the
+        // E-side warp
         if (lx != 0) {
 #pragma unroll
             for (int l = 1; l < BZ - 1; ++l) {
-                exEz[l * PLANE + slot] = ez[l + 1];
-                exEx[l * PLANE + slot] = ex[l + 1];
+                exEz[l * PLANE + slot0] = ez[0][l + 1];
+                exEx[l * PLANE + slot0] = ex[0][l + 1];
             }
         }
         // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
@@ -568,89 +669,105 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         if (k >= 1 && !fast) {
             mbar_wait(mb + MB_CREADY, ph.cready & 1u);
             ++ph.cready;
-            const int xs = (o0 & 3) + lx;
-            {   // the entering plane l_z = 0 -> this thread's private slots (row and column: auxiliary warp 17)
-                float* cs = coef + (o2 & (BZ - 1)) * PLANE;
+            // the entering plane l_z = 0 -> this thread's private slots (row and column: auxiliary warp)
+            const int cidx = (o2 & (BZ - 1)) * PLANE;
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
                 if (COEF) {
                     const float* sc = sm + Lay<COEF>::stgc;
                     float v[6];
 #pragma unroll
-                    for (int c = 0; c < 6; ++c) v[c] = sc[zidx<6>(c, ly, xs)];
+                    for (int c = 0; c < 6; ++c) v[c] = sc[zidx<6>(c, ly[r], xs)];
+                    float2 pr[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) pr[c] = make_float2(v[c], v[3 + c]);
                     if ((o0 <= 0) | (o1 <= 0) | (o2 <= 0)) {   // CTA-uniform: the box touches a low wall
 #pragma unroll
-                        for (int c = 0; c < 6; ++c) v[c] = coef_value<COEF>(P, c, v[c], gx, gy, o2);
+                        for (int c = 0; c < 3; ++c) pr[c] = coef_pair(P, c, v[c], v[3 + c], gx, gy[r], o2);
                     }
 #pragma unroll
-                    for (int c = 0; c < 6; ++c) cs[c * (BZ * PLANE)] = v[c];
+                    for (int c = 0; c < 3; ++c) cpair[cidx + r * SX + c * (BZ * PLANE)] = pr[c];
                 } else {
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) cs[c * (BZ * PLANE)] = coef_value<COEF>(P, c, 0.0f, gx, gy, o2);
+                    for (int c = 0; c < 3; ++c) cmask[cidx + r * SX + c * (BZ * PLANE)] = cb_mask(P, c, gx, gy[r], o2);
                 }
             }
             warp_arrive(mb + MB_CFREE);
         }
         PROF_MARK(2);
-        if (k > k0) {   // the signal warp has finished step k-1: the DONE barriers cannot lap it, the x-out rows are free
+        if (k > k0) {   // the signal warp has copied the x-out rows of step k-1 (and the DONE barriers cannot lap it)
             mbar_wait(mb + MB_ACKE, ph.acke & 1u);
             ++ph.acke;
         }
         // publish E of R_k \ R_{k+1} (everything at the last step)                                      (a8, a6)
-        if (actE && col_in && !(P.dbg & 4)) {
-            if ((unsigned)(o2 + W2) < (unsigned)nz) {            // the leaving plane l = 7: every column
-                const long long off = col_off + plane * (o2 + W2);
-                __stcg(Ex + off, ex[W2 + 1]);
-                __stcg(Ey + off, ey[W2 + 1]);
-                __stcg(Ez + off, ez[W2 + 1]);
-            }
-            if (last | (ly == W1)) {                             // warp-uniform: the leaving row (or the whole tile), planes 1..6
-                long long off = col_off + plane * (o2 + 1);
 #pragma unroll
-                for (int l = 1; l < W2; ++l) {
-                    if ((unsigned)(o2 + l) < (unsigned)nz) {
-                        __stcg(Ex + off, ex[l + 1]);
-                        __stcg(Ey + off, ey[l + 1]);
-                        __stcg(Ez + off, ez[l + 1]);
-                    }
-                    off += plane;
+        for (int r = 0; r < NROW; ++r) {
+            if ((lx >= 1) & (ly[r] >= 1) && col_in[r] && !FDTD_DBG(P, 4)) {
+                if ((unsigned)(o2 + W2) < (unsigned)nz) {            // the leaving plane l = 7: every column
+                    const long long off = col_off[r] + plane * (o2 + W2);
+                    __stcg(Ex + off, ex[r][W2 + 1]);
+                    __stcg(Ey + off, ey[r][W2 + 1]);
+                    __stcg(Ez + off, ez[r][W2 + 1]);
                 }
-            } else if (lx == W0) {                               // one lane per warp: the leaving column goes out through
-                float* xo = sm + Lay<COEF>::xoute + wy * 24;     // shared memory; the signal warp stores it
+                if (last | (ly[r] == W1)) {                          // warp-uniform: the leaving row (or the whole tile), planes 1..6
+                    long long off = col_off[r] + plane * (o2 + 1);
 #pragma unroll
-                for (int l = 1; l < W2; ++l) {
-                    xo[l] = ex[l + 1];
-                    xo[8 + l] = ey[l + 1];
-                    xo[16 + l] = ez[l + 1];
+                    for (int l = 1; l < W2; ++l) {
+                        if ((unsigned)(o2 + l) < (unsigned)nz) {
+                            __stcg(Ex + off, ex[r][l + 1]);
+                            __stcg(Ey + off, ey[r][l + 1]);
+                            __stcg(Ez + off, ez[r][l + 1]);
+                        }
+                        off += plane;
+                    }
+                } else if (lx == W0) {                               // one lane per warp: the leaving column goes out through
+                    float* xo = sm + Lay<COEF>::xoute + (ys0 + r) * 24;   // shared memory; the signal warp stores it
+#pragma unroll
+                    for (int l = 1; l < W2; ++l) {
+                        xo[l] = ex[r][l + 1];
+                        xo[8 + l] = ey[r][l + 1];
+                        xo[16 + l] = ez[r][l + 1];
+                    }
                 }
             }
         }
         warp_arrive(mb + MB_EDONE);
-        if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);
+        FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);)
 
         // ---------------- E minus shell -------------------------------------------------------------------------
         PROF_MARK(3);
         mbar_wait(mb + MB_EREADY, ph.eready & 1u);
         ++ph.eready;
         PROF_MARK(4);
-        {
-            const int xs = (o0 & 3) + lx;
-            ex[1] = stgE[zidx<3>(0, ly, xs)];
-            ey[1] = stgE[zidx<3>(1, ly, xs)];
-            ez[1] = stgE[zidx<3>(2, ly, xs)];
-            exEz[slot] = ez[1];
-            exEx[slot] = ex[1];
-            if (ly == 0) {
+#pragma unroll
+        for (int r = 0; r < NROW; ++r) {
+            ex[r][1] = stgE[zidx<3>(0, ly[r], xs)];
+            ey[r][1] = stgE[zidx<3>(1, ly[r], xs)];
+            ez[r][1] = stgE[zidx<3>(2, ly[r], xs)];
+        }
+        exEz[slot0] = ez[0][1];
+        exEx[slot0] = ex[0][1];
+#pragma unroll
+        for (int r = 0; r < NROW; ++r) {
+            if (ly[r] == 0) {             // warp-uniform: the entering row
 #pragma unroll
                 for (int l = 1; l < BZ; ++l) {
-                    ex[l + 1] = stgE[yidx<3>(0, l, xs)];
-                    ey[l + 1] = stgE[yidx<3>(1, l, xs)];
-                    ez[l + 1] = stgE[yidx<3>(2, l, xs)];
+                    ex[r][l + 1] = stgE[yidx<3>(0, l, xs)];
+                    ey[r][l + 1] = stgE[yidx<3>(1, l, xs)];
+                    ez[r][l + 1] = stgE[yidx<3>(2, l, xs)];
                 }
-            } else if (lx == 0) {
-                const float4* s4 = reinterpret_cast<const float4*>(xpkE + wy * 24);
-                const float4 a0 = s4[0], a1 = s4[1], b0 = s4[2], b1 = s4[3], c0 = s4[4], c1 = s4[5];
-                ex[2] = a0.y; ex[3] = a0.z; ex[4] = a0.w; ex[5] = a1.x; ex[6] = a1.y; ex[7] = a1.z; ex[8] = a1.w;
-                ey[2] = b0.y; ey[3] = b0.z; ey[4] = b0.w; ey[5] = b1.x; ey[6] = b1.y; ey[7] = b1.z; ey[8] = b1.w;
-                ez[2] = c0.y; ez[3] = c0.z; ez[4] = c0.w; ez[5] = c1.x; ez[6] = c1.y; ez[7] = c1.z; ez[8] = c1.w;
+            }
+        }
+        if (lx == 0) {
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
+                if (ly[r] != 0) {
+                    const float4* s4 = reinterpret_cast<const float4*>(xpkE + (ys0 + r) * 24);
+                    const float4 a0 = s4[0], a1 = s4[1], b0 = s4[2], b1 = s4[3], c0 = s4[4], c1 = s4[5];
+                    ex[r][2] = a0.y; ex[r][3] = a0.z; ex[r][4] = a0.w; ex[r][5] = a1.x; ex[r][6] = a1.y; ex[r][7] = a1.z; ex[r][8] = a1.w;
+                    ey[r][2] = b0.y; ey[r][3] = b0.z; ey[r][4] = b0.w; ey[r][5] = b1.x; ey[r][6] = b1.y; ey[r][7] = b1.z; ey[r][8] = b1.w;
+                    ez[r][2] = c0.y; ez[r][3] = c0.z; ez[r][4] = c0.w; ez[r][5] = c1.x; ez[r][6] = c1.y; ez[r][7] = c1.z; ez[r][8] = c1.w;
+                }
             }
         }
         warp_arrive(mb + MB_EFREE);
@@ -660,51 +777,60 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         // ---------------- H phase on R_{k+1} = [0,w-1]^3 (a2): every slot computes ----------------------------
 #pragma unroll
         for (int l = BZ - 2; l >= 0; --l) {
-            const float ey_xp = __shfl_sync(0xffffffffu, ey[l + 1], lane_p);
-            const float ez_xp = __shfl_sync(0xffffffffu, ez[l + 1], lane_p);
             const float ez_yp = exEz[l * PLANE + slot_yp];
             const float ex_yp = exEx[l * PLANE + slot_yp];
-            hx[l + 1] = yee_h_update(hx[l], ez_yp, ez[l + 1], ey[l + 2], ey[l + 1], rdy, rdz, dbx);   // (Ez[j+1]-Ez)/dy - (Ey[k+1]-Ey)/dz
-            hy[l + 1] = yee_h_update(hy[l], ex[l + 2], ex[l + 1], ez_xp, ez[l + 1], rdz, rdx, dby);   // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
-            hz[l + 1] = yee_h_update(hz[l], ey_xp, ey[l + 1], ex_yp, ex[l + 1], rdx, rdy, dbz);       // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
-            exHz[l * PLANE + slot] = hz[l + 1];
-            exHx[l * PLANE + slot] = hx[l + 1];
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
+                const float ey_xp = __shfl_sync(0xffffffffu, ey[r][l + 1], lane_p);
+                const float ez_xp = __shfl_sync(0xffffffffu, ez[r][l + 1], lane_p);
+                // y+1 neighbour: the last row reads the next warp's row 0 from the exchange, row 0 of two reads row 1's registers
+                const float ez_y = r == RL ? ez_yp : ez[r < RL ? r + 1 : RL][l + 1];
+                const float ex_y = r == RL ? ex_yp : ex[r < RL ? r + 1 : RL][l + 1];
+                hx[r][l + 1] = yee_h_update(hx[r][l], ez_y, ez[r][l + 1], ey[r][l + 2], ey[r][l + 1], rdy, rdz, dbx);   // (Ez[j+1]-Ez)/dy - (Ey[k+1]-Ey)/dz
+                hy[r][l + 1] = yee_h_update(hy[r][l], ex[r][l + 2], ex[r][l + 1], ez_xp, ez[r][l + 1], rdz, rdx, dby);   // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
+                hz[r][l + 1] = yee_h_update(hz[r][l], ey_xp, ey[r][l + 1], ex_y, ex[r][l + 1], rdx, rdy, dbz);           // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
+            }
+            exHz[l * PLANE + slot1] = hz[RL][l + 1];
+            exHx[l * PLANE + slot1] = hx[RL][l + 1];
         }
-        if (k > k0) {   // the H signal duty of step k-1 is done (its x-out rows are free, HDONE cannot lap its waiter)
+        if (k > k0) {   // the signal warp has copied the H x-out rows of step k-1 (HDONE cannot lap its waiters)
             mbar_wait(mb + MB_ACKH, ph.ackh & 1u);
             ++ph.ackh;
         }
         // publish H of R_{k+1} \ R_{k+2} (everything at the last step)                                  (a8, a6)
-        if ((lx <= W0 - 1) & (ly <= W1 - 1) && col_in && !(P.dbg & 4)) {
-            if ((unsigned)(o2 + W2 - 1) < (unsigned)nz) {        // the leaving plane l = 6: every column
-                const long long off = col_off + plane * (o2 + W2 - 1);
-                __stcg(Hx + off, hx[W2]);
-                __stcg(Hy + off, hy[W2]);
-                __stcg(Hz + off, hz[W2]);
-            }
-            if (last | (ly == W1 - 1)) {                         // warp-uniform: leaving row (or whole tile), planes 0..5
-                long long off = col_off + plane * o2;
 #pragma unroll
-                for (int l = 0; l < W2 - 1; ++l) {
-                    if ((unsigned)(o2 + l) < (unsigned)nz) {
-                        __stcg(Hx + off, hx[l + 1]);
-                        __stcg(Hy + off, hy[l + 1]);
-                        __stcg(Hz + off, hz[l + 1]);
-                    }
-                    off += plane;
+        for (int r = 0; r < NROW; ++r) {
+            if ((lx <= W0 - 1) & (ly[r] <= W1 - 1) && col_in[r] && !FDTD_DBG(P, 4)) {
+                if ((unsigned)(o2 + W2 - 1) < (unsigned)nz) {        // the leaving plane l = 6: every column
+                    const long long off = col_off[r] + plane * (o2 + W2 - 1);
+                    __stcg(Hx + off, hx[r][W2]);
+                    __stcg(Hy + off, hy[r][W2]);
+                    __stcg(Hz + off, hz[r][W2]);
                 }
-            } else if (lx == W0 - 1) {                           // the leaving column: out through shared memory
-                float* xo = sm + Lay<COEF>::xouth + wy * 24;
+                if (last | (ly[r] == W1 - 1)) {                      // warp-uniform: leaving row (or whole tile), planes 0..5
+                    long long off = col_off[r] + plane * o2;
 #pragma unroll
-                for (int l = 0; l < W2 - 1; ++l) {
-                    xo[l] = hx[l + 1];
-                    xo[8 + l] = hy[l + 1];
-                    xo[16 + l] = hz[l + 1];
+                    for (int l = 0; l < W2 - 1; ++l) {
+                        if ((unsigned)(o2 + l) < (unsigned)nz) {
+                            __stcg(Hx + off, hx[r][l + 1]);
+                            __stcg(Hy + off, hy[r][l + 1]);
+                            __stcg(Hz + off, hz[r][l + 1]);
+                        }
+                        off += plane;
+                    }
+                } else if (lx == W0 - 1) {                           // the leaving column: out through shared memory
+                    float* xo = sm + Lay<COEF>::xouth + (ys0 + r) * 24;
+#pragma unroll
+                    for (int l = 0; l < W2 - 1; ++l) {
+                        xo[l] = hx[r][l + 1];
+                        xo[8 + l] = hy[r][l + 1];
+                        xo[16 + l] = hz[r][l + 1];
+                    }
                 }
             }
         }
         warp_arrive(mb + MB_HDONE);
-        if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);
+        FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);)
         PROF_MARK(6);
     }
     if (threadIdx.x < 32) PROF_FLUSH(0);
@@ -774,28 +900,27 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             k1 = min(k1, t.a[q] + wq);
         }
         if (k1 < k0) k1 = k0;
-        if (P.dbg & 64) { k0 = 0; k1 = T; }
+        if (FDTD_DBG(P, 64)) { k0 = 0; k1 = T; }
         // no coefficient arrays and the box stays strictly inside the grid (never index 0, never outside) for the whole
         // launch: every cb mask would be dt -- the tile runs without masks, without their scatter and without CREADY/CFREE
-        bool fast = !COEF && !(P.dbg & 256);
+        bool fast = !COEF && !FDTD_DBG(P, 256);
         for (int q = 0; q < 3; ++q) {
             const int wq = q == 0 ? W0 : q == 1 ? W1 : W2;
             fast = fast && (t.a[q] - k1 >= 1) && (t.a[q] - k0 + wq <= P.g.n[q]);
         }
         if (k0 > 0 && warp < NWARPS_C) {
             // started late: nothing is loaded from the grid; the box holds zero fields (registers) and zero coefficients
-            float* cs = sm + Lay<COEF>::coef + (tid >> 5) * SX + lane;
-#pragma unroll
-            for (int c = 0; c < Lay<COEF>::NC * BZ; ++c) cs[c * PLANE] = 0.0f;
+            float* cs = sm + Lay<COEF>::coef;
+            for (int i = tid; i < Lay<COEF>::NC * BZ * PLANE; i += NCOMPUTE) cs[i] = 0.0f;
         }
         bar_sync(0, NT);
         J.tile = tile; J.k0 = k0; J.k1 = k1; J.fast = fast;
         return true;
     };
 
-    // Register split (setmaxnreg): the launch gives each of the 640 threads 96 registers; uncapped the compute code wants
-    // ~140 (deeper load hoisting in the phases), the auxiliary warps need few.  Each role has its own tile loop so that
-    // the register budget of a region is the one set at its head.
+    // Register split (setmaxnreg): the launch gives each of the 384 threads 168 registers; the compute code keeps 102 field
+    // values per thread and wants room to hoist loads, the auxiliary warps need few.  Each role has its own tile loop so
+    // that the register budget of a region is the one set at its head.
     if (warp < NWARPS_C) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_COMPUTE));
         TileJob J;
@@ -819,11 +944,6 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             // step k-1 published (flagH), and -- before the coefficient slots are overwritten -- E phase k-1 done
             PROF_DECL;
             const int hk0 = max(k0, 1);       // step 0 loads its whole box itself
-            // Who raises flagH.  A release store waits ~1-2 us for the SM's outstanding stores; two per step in one warp
-            // (19) lengthen the ACK round trip.  Without coefficient arrays warp 17 is nearly idle and takes the H flag
-            // (measured +7 % at 768^3); with them it carries the coefficient pipeline and warp 19 keeps both flags.
-            const bool hsig = !COEF && warp == W_HAUX;
-            if (hsig && k0 > 0 && lane == 0) st_release(P.flagH + tile, P.flag_base + k0);
             for (int j = k0; j <= k1; ++j) {
                 if (j >= hk0 && j < k1) {
                     const int k = j;
@@ -834,19 +954,19 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                         // still in use, copy, repack the entering column -> HREADY(k)
                         if (k == hk0 || !EARLY) {      // later steps: acquired while the previous copy was in flight
                             wait_upwind(P, t, P.flagH, P.flag_base + k, &ctl);
-                            if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                            if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                         }
                         PROF_MARK(0);
                         if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                         PROF_MARK(1);
-                        if (lane == 0 && !(P.dbg & 2)) issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
+                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         __syncwarp();
                         if (k + 1 < k1 && EARLY) {
                             wait_upwind(P, t, P.flagH, P.flag_base + k + 1, &ctl);
-                            if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                            if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                         }
                         PROF_MARK(2);
-                        if (!(P.dbg & 2)) { mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull; }
+                        if (!FDTD_DBG(P, 2)) { mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull; }
                         PROF_MARK(3);
                         pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
                         warp_arrive(mb + MB_HREADY);
@@ -858,14 +978,14 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                         if (!fast) {                 // (a uniform interior tile has no coefficient pipeline)
                         if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
                         PROF_MARK(0);
-                        if (COEF && lane == 0 && !(P.dbg & 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        if (COEF && lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                         __syncwarp();
                         PROF_MARK(1);
                         if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
                         PROF_MARK(2);
-                        if (COEF && !(P.dbg & 2)) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
+                        if (COEF && !FDTD_DBG(P, 2)) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
                         PROF_MARK(3);
-                        if (!(P.dbg & 16)) {
+                        if (!FDTD_DBG(P, 16)) {
                             scatter_coef<COEF>(P, sm, o0, o1, o2, 0);
                             scatter_coef<COEF>(P, sm, o0, o1, o2, 1);
                         }
@@ -874,22 +994,9 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                         }
                     }
                 }
-                if (hsig && j > k0) {
-                    const int k = j - 1;       // H flag of step k                                                (a9)
-                    const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
-                    mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
-                    if (k != T - 1 && !(P.dbg & 4)) store_xcol(P, P.g.H, sm + Lay<COEF>::xouth, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
-                    __syncwarp();
-                    if (lane == 0) {
-                        st_release(P.flagH + tile, P.flag_base + k + 1);
-                        mbar_arrive(mb + MB_ACKH);
-                    }
-                    __syncwarp();
-                }
             }
             if (warp == W_HPROD) PROF_FLUSH(8);
             if (warp == W_HAUX) PROF_FLUSH(16);
-            if (hsig && k1 < T && lane == 0) st_release(P.flagH + tile, P.flag_base + T);
             // phases of the last step that this warp does not wait for: covered by the CTA barrier at the tile boundary
             if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else if (!fast) ++n_cfree; }
             if (k1 > k0 && warp == W_HAUX) n_edone += fast ? (unsigned)(k1 - k0) : 1u;
@@ -898,24 +1005,24 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             // flight: the ~0.7 us proxy fence is off the EFREE -> EREADY chain
             if (k0 < k1) {
                 wait_upwind(P, t, P.flagE, P.flag_base + k0 + 1, &ctl);
-                if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
             }
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                 if (k > k0 && !EARLY) {
                     wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
-                    if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                    if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                 }
                 if (k > k0) {
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
                 }
-                if (lane == 0 && !(P.dbg & 2)) issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
+                if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
                 __syncwarp();
                 if (k + 1 < k1 && EARLY) {
                     wait_upwind(P, t, P.flagE, P.flag_base + k + 2, &ctl);
-                    if (lane == 0 && !(P.dbg & 32)) fence_proxy_async();
+                    if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                 }
-                if (!(P.dbg & 2)) { mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull; }
+                if (!FDTD_DBG(P, 2)) { mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull; }
                 const float* stg = sm + Lay<COEF>::stge;
                 pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
                 if (k > k0) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
@@ -935,37 +1042,44 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             }
             if (k1 > k0) { ++n_efree; ++n_hdone; }   // phases of the last step: covered by the CTA barrier at the tile boundary
         } else {
-            // signal warp: every publish of a phase has been issued before its warp arrived on the DONE barrier (or is this
-            // warp's own store of the leaving x column); the release store of the tile flag is cumulative over them   (a9)
-            // steps outside [k0, k1) publish nothing: their flags are raised at once
+            // signal warp.  Every publish of a phase has been issued before its warp arrived on the DONE barrier.  The
+            // leaving x columns are copied out of shared memory as soon as their phase is done and acknowledged at once, so
+            // the compute warps never wait for the fence; both columns are stored, ONE gpu-scope fence orders every publish
+            // of the step (cumulative over what this warp observed through the mbarriers), then both flags go up.     (a9)
+            // Steps outside [k0, k1) publish nothing: their flags are raised at once.
             if (k0 > 0 && lane == 0) {
-                st_release(P.flagE + tile, P.flag_base + k0);
-                if (COEF) st_release(P.flagH + tile, P.flag_base + k0);
+                raise_flag(P, P.flagE, tile, P.flag_base + k0);
+                raise_flag(P, P.flagH, tile, P.flag_base + k0);
             }
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
+                XCol ce, ch;
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
-                if (k != T - 1 && !(P.dbg & 4)) store_xcol(P, P.g.E, sm + Lay<COEF>::xoute, o0 + W0, o1, o2, 1, W1 - 1, 1);
+                load_xcol(ce, sm + Lay<COEF>::xoute, 1);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(mb + MB_ACKE);
+                mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
+                load_xcol(ch, sm + Lay<COEF>::xouth, 0);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(mb + MB_ACKH);
+                if (k != T - 1 && !FDTD_DBG(P, 4)) {
+                    store_xcol(P, P.g.E, ce, o0 + W0, o1, o2, 1, W1 - 1, 1);
+                    store_xcol(P, P.g.H, ch, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
+                }
                 __syncwarp();
                 if (lane == 0) {
-                    st_release(P.flagE + tile, P.flag_base + k + 1);
-                    mbar_arrive(mb + MB_ACKE);
+                    fence_acq_rel_gpu();
+                    FDTD_DEBUG_ONLY(if (tile != P.withhold_tile))
+                    {
+                        st_relaxed(P.flagE + tile, P.flag_base + k + 1);
+                        st_relaxed(P.flagH + tile, P.flag_base + k + 1);
+                    }
                 }
                 __syncwarp();
-                if (COEF) {
-                    mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
-                    if (k != T - 1 && !(P.dbg & 4)) store_xcol(P, P.g.H, sm + Lay<COEF>::xouth, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
-                    __syncwarp();
-                    if (lane == 0) {
-                        st_release(P.flagH + tile, P.flag_base + k + 1);
-                        mbar_arrive(mb + MB_ACKH);
-                    }
-                    __syncwarp();
-                }
             }
             if (k1 < T && lane == 0) {
-                st_release(P.flagE + tile, P.flag_base + T);
-                if (COEF) st_release(P.flagH + tile, P.flag_base + T);
+                raise_flag(P, P.flagE, tile, P.flag_base + T);
+                raise_flag(P, P.flagH, tile, P.flag_base + T);
             }
         }
     }
@@ -987,10 +1101,12 @@ void systolic_tma_boxes(int box[3][3])
         for (int q = 0; q < 3; ++q) box[f][q] = b[f][q];
 }
 
-cudaError_t systolic_tma_prepare(int coef)
+cudaError_t systolic_tma_prepare(int coef, int* blocks_per_sm)
 {
     const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
-    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)systolic_tma_smem(coef));
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)systolic_tma_smem(coef));
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, fn, NT, systolic_tma_smem(coef));
 }
 
 cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st)

@@ -15,7 +15,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["fdtd_api.cu", "naive_kernels.cu", "systolic_kernel.cu", "systolic_reg.cu", "systolic_tma.cu"]
+SOURCES = ["fdtd_api.cu", "naive_kernels.cu", "pad_kernels.cu", "systolic_kernel.cu", "systolic_reg.cu", "systolic_tma.cu"]
 HEADERS = ["fdtd_internal.h", "fdtd_types.h", "yee_update.h", "systolic_tile.cuh", os.path.join("..", "..", "include", "fdtd.h")]
 LIBS = {
     "fma": (os.path.join(HERE, "libfdtd_b200.so"), []),

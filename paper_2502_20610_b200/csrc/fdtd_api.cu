@@ -30,7 +30,14 @@ struct fdtd_ctx {
     int reqT;         // requested temporal depth (0 = default)
     int cfg_idx;      // resolved shared-memory systolic configuration, -1 = unresolved / not used
     bool use_reg;     // resolved: the register-resident kernel (tile 31x15x7) runs
-    bool use_tma;     // resolved: its TMA-staged version runs (PEC grids, nx % 4 == 0)
+    bool use_tma;     // resolved: its TMA-staged version runs
+    // resolved: the TMA kernel runs on a padded working copy of the grid (periodic axis or nx % 4 != 0)
+    bool use_pad;
+    PadGeom pg;
+    float* pad_fld;   // 6 padded arrays E0..2 H0..2 at stride pad_stride (library-owned)
+    float* pad_coef;  // 6 padded arrays ca0..2 cb0..2, or NULL
+    long long pad_stride;
+    bool pad_coef_valid;
     TmaMaps tmaps;    // 36 CUtensorMap: [E0..2 H0..2 ca0..2 cb0..2][z plane, y row, x column]
     int tma_group[3]; // per group (E, H, coefficients): 0 per-array maps, 1 one 4-D map per piece, 2 two triples
     bool tmaps_valid;
@@ -110,6 +117,28 @@ int default_T(const fdtd_ctx* c)
     return c->env_T > 0 ? c->env_T : 128;
 }
 
+// Temporal depth on a padded periodic axis: the ghost zones are 2T cells of redundant work per n cells of the axis, so T
+// follows the shortest periodic extent (n/8: 25 % redundant cells), within [8, 128].
+int default_T_padded(const fdtd_ctx* c)
+{
+    if (c->env_T > 0) return c->env_T;
+    int nmin = 1 << 30;
+    for (int a = 0; a < 3; ++a)
+        if (c->g.per[a] && c->g.n[a] < nmin) nmin = c->g.n[a];
+    if (nmin == (1 << 30)) return default_T(c);      // no periodic axis: only the row pitch is padded
+    int T = nmin / 8;
+    T = T < 8 ? 8 : T > 128 ? 128 : T;
+    return T;
+}
+
+void free_pad(fdtd_ctx* c)
+{
+    if (c->pad_fld) cudaFree(c->pad_fld);
+    if (c->pad_coef) cudaFree(c->pad_coef);
+    c->pad_fld = c->pad_coef = nullptr;
+    c->pad_coef_valid = false;
+}
+
 int resolve_systolic(fdtd_ctx* c)
 {
     if (coef_mixed(c)) return fail(c, FDTD_EINVAL, "systolic kernel needs ca and cb both bound or both NULL");
@@ -122,8 +151,8 @@ int resolve_systolic(fdtd_ctx* c)
         if (c->env_tile[0] > 0) { N[0] = c->env_tile[0]; N[1] = c->env_tile[1]; N[2] = c->env_tile[2]; }
     }
     c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
-    c->use_tma = c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->g.per[0] && !c->g.per[1] && !c->g.per[2] &&
-                 c->g.n[0] % 4 == 0 && !c->dbg_no_tma;
+    c->use_tma = c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->dbg_no_tma;
+    c->use_pad = c->use_tma && (c->g.per[0] || c->g.per[1] || c->g.per[2] || c->g.n[0] % 4 != 0);
     int found = -1;
     int per_sm = 0;
     if (c->use_tma) {
@@ -154,24 +183,67 @@ int resolve_systolic(fdtd_ctx* c)
     if (per_sm < 1) return fail(c, FDTD_ECUDA, "the systolic kernel does not fit on an SM of this device");
     if (per_sm > 4) per_sm = 4;
     c->ctas = c->num_sms * per_sm;
-    c->T = c->reqT > 0 ? c->reqT : default_T(c);
-    // a ring of tiles along a periodic axis advances in lock step: all of it (and everything the claim order
-    // interleaves with it) must be resident at once (SURVEY.md section 7 hard part 2)
-    int span = 1, ring = 1;
-    for (int a = 0; a < 3; ++a) {
-        const AxisPlan ap = make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T);
-        span *= ap.nb;
-        if (c->g.per[a]) ring = span;
+    c->T = c->reqT > 0 ? c->reqT : c->use_pad ? default_T_padded(c) : default_T(c);
+    if (!c->use_tma) {
+        // a ring of tiles along a periodic axis advances in lock step: all of it (and everything the claim order
+        // interleaves with it) must be resident at once (SURVEY.md section 7 hard part 2)
+        int span = 1, ring = 1;
+        for (int a = 0; a < 3; ++a) {
+            const AxisPlan ap = make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T);
+            span *= ap.nb;
+            if (c->g.per[a]) ring = span;
+        }
+        if (ring > c->ctas) {
+            char buf[160];
+            snprintf(buf, sizeof buf, "periodic ring of %d tiles exceeds the %d resident CTAs; use a larger tile or the naive kernel", ring, c->ctas);
+            return fail(c, FDTD_EINVAL, buf);
+        }
     }
-    if (ring > c->ctas) {
-        char buf[160];
-        snprintf(buf, sizeof buf, "periodic ring of %d tiles exceeds the %d resident CTAs; use a larger tile or the naive kernel", ring, c->ctas);
-        return fail(c, FDTD_EINVAL, buf);
+    free_pad(c);
+    if (c->use_pad) {
+        // the padded working copy: G = T ghost cells on either side of every periodic axis, rows of a multiple of 4 cells
+        long long cells = 1;
+        for (int a = 0; a < 3; ++a) {
+            c->pg.n[a] = c->g.n[a];
+            c->pg.G[a] = c->g.per[a] ? c->T : 0;
+            c->pg.m[a] = c->g.n[a] + 2 * c->pg.G[a];
+        }
+        c->pg.ldx = (c->pg.m[0] + 3) / 4 * 4;
+        cells = c->pg.ldx * c->pg.m[1] * c->pg.m[2];
+        if (c->pg.m[0] > (1 << 16) || c->pg.m[1] > (1 << 16) || c->pg.m[2] > (1 << 16) || cells >= (1ll << 40))
+            return fail(c, FDTD_EINVAL, "padded working grid too large; use a smaller temporal depth");
+        c->pad_stride = (cells + 63) / 64 * 64;
+        cudaError_t e = cudaMalloc(&c->pad_fld, (size_t)c->pad_stride * 6 * sizeof(float));
+        if (e == cudaSuccess && want_coef) e = cudaMalloc(&c->pad_coef, (size_t)c->pad_stride * 6 * sizeof(float));
+        if (e != cudaSuccess) {
+            free_pad(c);
+            return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(padded working copy): ") + cudaGetErrorString(e));
+        }
     }
+    c->tmaps_valid = false;
     c->cfg_idx = found;
     for (int a = 0; a < 3; ++a) c->N[a] = N[a];
     c->resolved = true;
     return FDTD_OK;
+}
+
+// The grid the systolic kernel works on: the caller's arrays, or the padded working copy (then every axis is an open /
+// wall axis of extent m, and the source box moves with the interior).  *ldx = row pitch in elements.
+GridParams work_grid(const fdtd_ctx* c, long long* ldx)
+{
+    GridParams g = c->g;
+    *ldx = c->g.n[0];
+    if (!c->use_pad) return g;
+    for (int a = 0; a < 3; ++a) {
+        g.E[a] = c->pad_fld + c->pad_stride * a;
+        g.H[a] = c->pad_fld + c->pad_stride * (3 + a);
+        g.ca[a] = c->pad_coef ? c->pad_coef + c->pad_stride * a : nullptr;
+        g.cb[a] = c->pad_coef ? c->pad_coef + c->pad_stride * (3 + a) : nullptr;
+        g.n[a] = c->pg.m[a];
+        g.src_box[a] = c->g.src_box[a] + c->pg.G[a];
+    }
+    *ldx = c->pg.ldx;
+    return g;
 }
 
 int ensure_flags(fdtd_ctx* c, size_t ntiles)
@@ -211,17 +283,19 @@ int ensure_tmaps(fdtd_ctx* c)
     }
     int box[3][3];
     systolic_tma_boxes(box);
+    long long ldx = 0;
+    const GridParams wg = work_grid(c, &ldx);
     const void* arr[12];
     for (int a = 0; a < 3; ++a) {
-        arr[a] = c->g.E[a];
-        arr[3 + a] = c->g.H[a];
-        arr[6 + a] = c->g.ca[a];
-        arr[9 + a] = c->g.cb[a];
+        arr[a] = wg.E[a];
+        arr[3 + a] = wg.H[a];
+        arr[6 + a] = wg.ca[a];
+        arr[9 + a] = wg.cb[a];
     }
     static_assert(sizeof(CUtensorMap) * 36 == sizeof(TmaMaps), "TmaMaps layout");
     CUtensorMap* host = reinterpret_cast<CUtensorMap*>(c->tmaps.bytes);
     memset(c->tmaps.bytes, 0, sizeof c->tmaps.bytes);
-    const cuuint64_t nbytes = (cuuint64_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * 4u;
+    const cuuint64_t nbytes = (cuuint64_t)ldx * wg.n[1] * wg.n[2] * 4u;
     // arrays first..first+count-1 at one positive stride (multiple of 16 bytes, no overlap)? -> the stride, else 0
     auto uniform_stride = [&](int first, int count) -> cuuint64_t {
         if (!arr[first] || c->dbg_no_group) return 0;
@@ -235,8 +309,9 @@ int ensure_tmaps(fdtd_ctx* c)
         return d;
     };
     auto encode_maps = [&](CUtensorMap* dst, const void* base, int narr, cuuint64_t astride) -> int {
-        const cuuint64_t dims[4] = {(cuuint64_t)c->g.n[0], (cuuint64_t)c->g.n[1], (cuuint64_t)c->g.n[2], (cuuint64_t)narr};
-        const cuuint64_t strides[3] = {(cuuint64_t)c->g.n[0] * 4u, (cuuint64_t)c->g.n[0] * c->g.n[1] * 4u, astride};
+        // extents are the logical grid (elements beyond it are delivered as zeros), strides follow the row pitch
+        const cuuint64_t dims[4] = {(cuuint64_t)wg.n[0], (cuuint64_t)wg.n[1], (cuuint64_t)wg.n[2], (cuuint64_t)narr};
+        const cuuint64_t strides[3] = {(cuuint64_t)ldx * 4u, (cuuint64_t)ldx * wg.n[1] * 4u, astride};
         const cuuint32_t estr[4] = {1, 1, 1, 1};
         for (int f = 0; f < 3; ++f) {
             const cuuint32_t b[4] = {(cuuint32_t)box[f][0], (cuuint32_t)box[f][1], (cuuint32_t)box[f][2], (cuuint32_t)narr};
@@ -317,17 +392,12 @@ int ensure_order(fdtd_ctx* c, const int nb[3])
     return FDTD_OK;
 }
 
-// Library default (no fdtd_set_kernel call): the systolic schedule where its TMA-staged kernel applies (all axes PEC,
-// nx % 4 == 0); grids with a periodic axis or another nx run the naive kernel, which is ~4x faster there than the
-// cp.async systolic kernel (a ring of tiles advances in lock step: 0.015 vs 0.070 TCUPS on config 3).
-bool tma_eligible(const fdtd_ctx* c)
-{
-    return !c->g.per[0] && !c->g.per[1] && !c->g.per[2] && c->g.n[0] % 4 == 0 && !coef_mixed(c) && !c->dbg_no_tma;
-}
-
+// Library default (no fdtd_set_kernel call): the systolic schedule on every grid (its TMA-staged kernel; grids with a
+// periodic axis or nx % 4 != 0 run it on the padded working copy).  Only a half-bound coefficient set (ca without cb or
+// the reverse), which the systolic kernel does not take, falls back to the naive kernel.
 int effective_kernel(const fdtd_ctx* c)
 {
-    if (!c->which_explicit && c->which == FDTD_KERNEL_SYSTOLIC && !tma_eligible(c)) return FDTD_KERNEL_NAIVE;
+    if (!c->which_explicit && c->which == FDTD_KERNEL_SYSTOLIC && coef_mixed(c)) return FDTD_KERNEL_NAIVE;
     return c->which;
 }
 
@@ -362,15 +432,71 @@ int step_systolic(fdtd_ctx* c, int n)
         if (rc != FDTD_OK) return rc;
     }
     const int N[3] = {c->N[0], c->N[1], c->N[2]};
+    long long ldx = 0;
+    const GridParams wg = work_grid(c, &ldx);
+    // source images on the working grid: the box itself and, on the padded copy, its periodic copies that meet a ghost zone
+    int nsrc = 0, src_org[MAX_SRC_IMAGES][3];
+    if (c->use_tma && c->g.src_comp >= 0) {
+        int lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+        for (int a = 0; a < 3; ++a) {
+            if (!c->use_pad || c->pg.G[a] == 0) continue;
+            // images j * n[a] of the box [b, b + w) that intersect [0, m[a])
+            const int b0 = wg.src_box[a], w = wg.src_box[3 + a], na = c->g.n[a], ma = wg.n[a];
+            while (b0 + (lo[a] - 1) * na + w > 0) --lo[a];
+            while (b0 + (hi[a] + 1) * na < ma) ++hi[a];
+        }
+        for (int jz = lo[2]; jz <= hi[2]; ++jz)
+            for (int jy = lo[1]; jy <= hi[1]; ++jy)
+                for (int jx = lo[0]; jx <= hi[0]; ++jx) {
+                    if (nsrc == MAX_SRC_IMAGES) return fail(c, FDTD_EINVAL, "temporal depth too large for this periodic grid: more than 125 source images");
+                    src_org[nsrc][0] = wg.src_box[0] + jx * c->g.n[0];
+                    src_org[nsrc][1] = wg.src_box[1] + jy * c->g.n[1];
+                    src_org[nsrc][2] = wg.src_box[2] + jz * c->g.n[2];
+                    ++nsrc;
+                }
+    }
+    PadArrays pf, pc;
+    if (c->use_pad && n > 0) {
+        memset(&pf, 0, sizeof pf);
+        memset(&pc, 0, sizeof pc);
+        for (int a = 0; a < 3; ++a) {
+            pf.usr[a] = c->g.E[a];
+            pf.usr[3 + a] = c->g.H[a];
+            pc.usr[a] = const_cast<float*>(c->g.ca[a]);
+            pc.usr[3 + a] = const_cast<float*>(c->g.cb[a]);
+        }
+        pf.ext = c->pad_fld; pf.stride = c->pad_stride; pf.narr = 6;
+        pc.ext = c->pad_coef; pc.stride = c->pad_stride; pc.narr = 6;
+        if (c->pad_coef && !c->pad_coef_valid) {           // constants of the run: copied (with their images) once
+            cudaError_t e = launch_pad_copy_in(c->pg, pc, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "padded copy of the coefficient arrays");
+            c->pad_coef_valid = true;
+            c->counters[0]++;
+        }
+        // the caller's arrays are the state between calls (they may have been rewritten): copy in, interior and ghosts
+        cudaError_t e = launch_pad_copy_in(c->pg, pf, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "padded copy of the field arrays");
+        c->counters[0]++;
+    }
+    bool first = true;
     int left = n;
     while (left > 0) {
         const int T = left < c->T ? left : c->T;
+        if (c->use_pad && !first) {      // ghost zones <- periodic images of the interior the last launch left behind
+            cudaError_t e = launch_pad_ghost_fill(c->pg, pf, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "ghost fill");
+            c->counters[0]++;
+        }
+        first = false;
         SysParams P;
         memset(&P, 0, sizeof P);
-        P.g = c->g;
+        P.g = c->use_tma ? wg : c->g;
+        P.ldx = (int)ldx;
+        P.nsrc = nsrc;
+        memcpy(P.src_org, src_org, sizeof src_org);
         long long ntiles = 1;
         for (int a = 0; a < 3; ++a) {
-            P.ax[a] = make_axis_plan(c->g.n[a], c->g.per[a], N[a], T);
+            P.ax[a] = make_axis_plan(P.g.n[a], c->use_tma ? 0 : c->g.per[a], N[a], T);
             ntiles *= P.ax[a].nb;
         }
         if (ntiles >= (1ll << 30)) return fail(c, FDTD_EINVAL, "too many tiles for one launch");
@@ -416,6 +542,11 @@ int step_systolic(fdtd_ctx* c, int n)
         c->counters[1] += T;
         c->counters[2]++;
         c->counters[3] += ntiles;
+    }
+    if (c->use_pad && n > 0) {
+        cudaError_t e = launch_pad_copy_out(c->pg, pf, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "copy out of the padded working copy");
+        c->counters[0]++;
     }
     return FDTD_OK;
 }
@@ -483,6 +614,11 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->cfg_idx = -1;
     c->use_reg = false;
     c->use_tma = false;
+    c->use_pad = false;
+    c->pad_fld = c->pad_coef = nullptr;
+    c->pad_stride = 0;
+    c->pad_coef_valid = false;
+    memset(&c->pg, 0, sizeof c->pg);
     c->tmaps_valid = false;
     c->resolved = false;
     c->smem = 0;
@@ -733,7 +869,9 @@ int fdtd_get_kernel(const fdtd_ctx* cc, int out[8])
         out[4] = c->T;
         long long nt = 1;
         const int N[3] = {out[1], out[2], out[3]};
-        for (int a = 0; a < 3; ++a) nt *= make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T).nb;
+        for (int a = 0; a < 3; ++a)
+            nt *= c->use_tma ? make_axis_plan(c->use_pad ? c->pg.m[a] : c->g.n[a], 0, N[a], c->T).nb
+                             : make_axis_plan(c->g.n[a], c->g.per[a], N[a], c->T).nb;
         out[5] = (int)nt;
         out[6] = nt < c->ctas ? (int)nt : c->ctas;
         out[7] = (int)c->smem;
@@ -810,6 +948,7 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->d_flags) cudaFree(c->d_flags);
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);
+    free_pad(c);
     for (auto& o : c->orders) cudaFree(o.d);
     if (c->d_prof) {
         long long h[32];

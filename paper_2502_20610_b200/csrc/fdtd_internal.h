@@ -30,3 +30,8 @@ int systolic_tma_threads();
 void systolic_tma_boxes(int box[3][3]);   // TMA box extents (x,y,z) of the z-plane, y-row and x-column shell pieces
 cudaError_t systolic_tma_prepare(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
+
+// implemented in pad_kernels.cu: copies between the caller's arrays and the padded working copy (periodic images)
+cudaError_t launch_pad_copy_in(const PadGeom& g, const PadArrays& a, cudaStream_t st);     // all padded cells <- images
+cudaError_t launch_pad_ghost_fill(const PadGeom& g, const PadArrays& a, cudaStream_t st);  // ghost cells <- interior
+cudaError_t launch_pad_copy_out(const PadGeom& g, const PadArrays& a, cudaStream_t st);    // interior -> caller

@@ -69,6 +69,23 @@ inline AxisPlan make_axis_plan(int n, int per, int N, int T)
 #define FDTD_DEBUG_ONLY(...)
 #endif
 
+constexpr int MAX_SRC_IMAGES = 125;
+
+// The padded working copy of the grid (pad_kernels.cu): a periodic axis a carries G[a] ghost cells on
+// either side (m[a] = n[a] + 2 G[a]); wall axes have G[a] = 0; rows are ldx >= m[0] elements long (a multiple of 4).
+struct PadGeom {
+    int n[3];
+    int m[3];
+    int G[3];
+    long long ldx;
+};
+struct PadArrays {
+    float* usr[6];        // the caller's arrays (n[0]*n[1]*n[2] each)
+    float* ext;           // narr padded arrays of ldx*m[1]*m[2] elements at a uniform stride
+    long long stride;
+    int narr;
+};
+
 struct SysParams {
     GridParams g;
     AxisPlan ax[3];
@@ -83,6 +100,11 @@ struct SysParams {
     long long spin_budget; // clock64 ticks a single wait may take
     const int* order;      // systolic_tma.cu: claim index -> tile, sorted by wavefront bx+by+bz (NULL: identity)
     int tma_group[3];      // systolic_tma.cu, per group (E, H, coefficients): 0 per-array 3-D maps, 1 one 4-D map per piece, 2 two triples
+    // systolic_tma.cu on a padded copy of the grid: row pitch of the arrays in elements (>= g.n[0], a
+    // multiple of 4), and the images of the source box (a box on a periodic axis also drives its ghost copies)
+    int ldx;
+    int nsrc;              // 0: no source; else number of images of g.src_box
+    int src_org[MAX_SRC_IMAGES][3];
     long long* prof;       // FDTD_PROFILE build: 32 tick accumulators (NULL otherwise)
     // FDTD_DEBUG builds only (always 0 / NULL in the product libraries, and never read there):
     int dbg;               // FDTD_DEBUG_SKIP timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes,

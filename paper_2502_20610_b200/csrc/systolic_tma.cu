@@ -100,12 +100,12 @@ struct Lay {
     static constexpr int xpke = xpkh + XPK;
     static constexpr int xoute = xpke + XPK;           // leaving x column of E, [y slot][component][8], stored by the signal warp
     static constexpr int xouth = xoute + XPK;
-    static constexpr int exch = xouth + XPK;           // exHz, exHx, exEz, exEx
+    static constexpr int exch = xouth + XPK;           // y exchange: float2 (H_z, H_x)[W2][PLANE] then float2 (E_z, E_x)[W2][PLANE]
     static constexpr int coef = exch + 4 * EXP;
     static constexpr int total = coef + NC * BZ * PLANE;
 };
 
-enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_ACKE, MB_ACKH, MB_CREADY, MB_CFREE, MB_COUNT };
+enum { MB_HFULL = 0, MB_CFULL, MB_EFULL, MB_HREADY, MB_EREADY, MB_HFREE, MB_EFREE, MB_EDONE, MB_HDONE, MB_ACKE, MB_ACKH, MB_CFREE, MB_COUNT };
 
 struct TileGeom {
     int a[3];
@@ -310,63 +310,57 @@ __device__ __forceinline__ float2 coef_pair(const SysParams& P, int c, float a, 
 {
     return frozen(P, c, gx, gy, gz) ? make_float2(1.0f, 0.0f) : make_float2(a, b);
 }
-
-// ---- H-side auxiliary warp: coefficients of the entering row and column -> the owner threads' private slots ----
-// (the entering plane l_z = 0 is absorbed by the compute threads themselves).  Part 0 takes the row l_y = 0,
-// part 1 the column l_x = 0; loads of a batch are issued before its stores.
-template <bool COEF>
-__device__ __forceinline__ void scatter_coef(const SysParams& P, float* sm, int o0, int o1, int o2, int part)
+// the same when the caller knows (CTA-uniform) whether the box touches a low wall at all
+__device__ __forceinline__ float2 coef_pair(const SysParams& P, bool wall, int c, float a, float b, int gx, int gy, int gz)
 {
-    const int lane = threadIdx.x & 31;
+    return wall ? coef_pair(P, c, a, b, gx, gy, gz) : make_float2(a, b);
+}
+
+// ---- coefficients of the cells that enter with the shell of a step -> their owner threads' private slots -------------
+// All compute threads take part, one shell cell each (after the barrier that follows E phase k, so nobody still reads the
+// slots of the cells that left): every thread its own cell of the entering plane l_z = 0, warps 0..6 the entering row
+// l_y = 0 (one plane each, lane = x), warps 7..10 the 105 cells of the entering column l_x = 0.  The slots are first read
+// by E phase k+1, behind the next CTA barrier.
+template <bool COEF>
+__device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm, int o0, int o1, int o2, int lx, const int (&ly)[NROW], int ys0)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const float* stg = sm + Lay<COEF>::stgc;
+    float* const cmask = sm + Lay<COEF>::coef;
+    float2* const cpair = reinterpret_cast<float2*>(sm + Lay<COEF>::coef);
     const int r0 = o0 & 3;
-    if (part == 0) {
-        const int gx = o0 + lane, gy = o1;
-        const int slot = (gy & (BY - 1)) * SX + (gx & (BX - 1));
-        if (COEF) {
-            float2* dst = reinterpret_cast<float2*>(sm + Lay<COEF>::coef) + slot;
+    const bool wall = (o0 <= 0) | (o1 <= 0) | (o2 <= 0);   // CTA-uniform: only then can a shell cell be frozen
+    auto put = [&](int slot, int gx, int gy, int gz, const float (&v)[6]) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                float a[BZ], b[BZ];
-#pragma unroll
-                for (int l = 1; l < BZ; ++l) {
-                    a[l] = stg[yidx<6>(c, l, r0 + lane)];
-                    b[l] = stg[yidx<6>(3 + c, l, r0 + lane)];
-                }
-#pragma unroll
-                for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = coef_pair(P, c, a[l], b[l], gx, gy, o2 + l);
-            }
-        } else {
-            float* dst = sm + Lay<COEF>::coef + slot;
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int l = 1; l < BZ; ++l) dst[(c * BZ + ((o2 + l) & (BZ - 1))) * PLANE] = cb_mask(P, c, gx, gy, o2 + l);
+        for (int c = 0; c < 3; ++c) {
+            if (COEF) cpair[slot + c * (BZ * PLANE)] = coef_pair(P, wall, c, v[c], v[3 + c], gx, gy, gz);
+            else cmask[slot + c * (BZ * PLANE)] = cb_mask(P, c, gx, gy, gz);
         }
-    } else {
-        const int xs = o0 & (BX - 1);
+    };
+    // the entering plane: this thread's own cells
 #pragma unroll
-        for (int r = 0; r < (W1 * W2 + 31) / 32; ++r) {            // 105 cells: idx = (l-1)*15 + (ly-1)
-            const int idx = r * 32 + lane;
-            const int ly = 1 + idx % W1, l = 1 + idx / W1;
-            const int slot = ((o2 + l) & (BZ - 1)) * PLANE + ((o1 + ly) & (BY - 1)) * SX + xs;
-            if (COEF) {
-                float a[3], b[3];
+    for (int r = 0; r < NROW; ++r) {
+        float v[6];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    a[c] = idx < W1 * W2 ? stg[xidx<6>(c, ly, l) + r0] : 0.0f;
-                    b[c] = idx < W1 * W2 ? stg[xidx<6>(3 + c, ly, l) + r0] : 0.0f;
-                }
-                if (idx < W1 * W2) {
-                    float2* d = reinterpret_cast<float2*>(sm + Lay<COEF>::coef) + slot;
+        for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[zidx<6>(c, ly[r], r0 + lx)] : 0.0f;
+        put((o2 & (BZ - 1)) * PLANE + (ys0 + r) * SX + lane, o0 + lx, o1 + ly[r], o2, v);
+    }
+    constexpr int ROW_WARPS = W2, COL_WARPS = (W1 * W2 + 31) / 32;
+    static_assert(ROW_WARPS + COL_WARPS <= NWARPS_C, "not enough compute warps for the coefficient shell");
+    if (w < ROW_WARPS) {                       // the entering row, plane l = w + 1: lane = x offset inside the box
+        const int l = w + 1, gx = o0 + lane;
+        float v[6];
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) d[c * BZ * PLANE] = coef_pair(P, c, a[c], b[c], o0, o1 + ly, o2 + l);
-                }
-            } else if (idx < W1 * W2) {
-                float* d = sm + Lay<COEF>::coef + slot;
+        for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
+        put(((o2 + l) & (BZ - 1)) * PLANE + (o1 & (BY - 1)) * SX + (gx & (BX - 1)), gx, o1, o2 + l, v);
+    } else if (w < ROW_WARPS + COL_WARPS) {    // the entering column: idx = (l-1)*15 + (ly-1)
+        const int idx = (w - ROW_WARPS) * 32 + lane;
+        if (idx < W1 * W2) {
+            const int cy = 1 + idx % W1, l = 1 + idx / W1;
+            float v[6];
 #pragma unroll
-                for (int c = 0; c < 3; ++c) d[c * BZ * PLANE] = cb_mask(P, c, o0, o1 + ly, o2 + l);
-            }
+            for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[xidx<6>(c, cy, l) + r0] : 0.0f;
+            put(((o2 + l) & (BZ - 1)) * PLANE + ((o1 + cy) & (BY - 1)) * SX + (o0 & (BX - 1)), o0, o1 + cy, o2 + l, v);
         }
     }
 }
@@ -415,7 +409,7 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
 {
     const int lane = threadIdx.x & 31;
     if ((unsigned)gx >= (unsigned)P.g.n[0]) return;
-    const long long nx = P.g.n[0], plane = nx * P.g.n[1];
+    const long long nx = P.ldx, plane = nx * P.g.n[1];
 #pragma unroll
     for (int r = 0; r < XROUNDS; ++r) {
         const int item = r * 32 + lane;
@@ -433,8 +427,9 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
 
 // ---- compute warps ---------------------------------------------------------------------------------------------
 // FDTD_PROFILE build only: lane 0 of compute warp 0 accumulates clock64 ticks per section of the step into
-// P.prof[0..7] (wait HREADY+absorb, barrier, E phase+publish, wait SIGACK, wait EREADY, absorb+barrier, H phase+publish,
-// steps); aux warps add theirs to P.prof[8..].
+// P.prof[0..7] (0 wait HREADY + absorb H, 1 barrier, 2 E phase + source + exchange stores, 3 wait ACKE + publish E,
+// 4 wait EREADY, 5 absorb E + barrier, 6 H phase + wait ACKH + publish H, 7 wait CREADY + absorb coefficient plane);
+// aux warps add theirs to P.prof[8..].
 #ifdef FDTD_PROFILE
 #define PROF_DECL long long pt_ = clock64(), pacc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
 #define PROF_MARK(i) do { const long long n_ = clock64(); pacc_[i] += n_ - pt_; pt_ = n_; } while (0)
@@ -446,7 +441,7 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
 #endif
 
 struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
-    unsigned hready, eready, acke, ackh, cready;
+    unsigned hready, eready, acke, ackh, cfull;
 };
 
 template <bool COEF>
@@ -460,17 +455,16 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     const int slot_yp = ((ys0 + NROW) & (BY - 1)) * SX + lane;  // the row above the last row = row 0 of warp w+1
     const int lane_m = (lane - 1) & 31, lane_p = (lane + 1) & 31;
     const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
-    const long long plane = (long long)nx * ny;
+    const long long ldx = P.ldx, plane = ldx * ny;
 
     const float* stgH = sm + Lay<COEF>::stgh;
     const float* stgE = sm + Lay<COEF>::stge;
     const float* xpkH = sm + Lay<COEF>::xpkh;
     const float* xpkE = sm + Lay<COEF>::xpke;
     // y exchange: only the links between a thread's row 1 and the next warp's row 0 go through shared memory
-    float* exHz = sm + Lay<COEF>::exch;       // H_z, H_x of row 1 for the E phase of the next warp's row 0
-    float* exHx = exHz + EXP;
-    float* exEz = exHx + EXP;                 // E_z, E_x of row 0 for the H phase of the previous warp's row 1
-    float* exEx = exEz + EXP;
+    // (z, x) component pairs: one 64-bit access per link
+    float2* exH = reinterpret_cast<float2*>(sm + Lay<COEF>::exch);   // (H_z, H_x) of the last row for the E phase of the next warp's row 0
+    float2* exE = exH + EXP;                                         // (E_z, E_x) of row 0 for the H phase of the previous warp's last row
     // this thread's private coefficient slots, row 0 (row 1: + SX): index (c*BZ + z slot)*PLANE; float2 (ca, cb) pairs
     // with coefficient arrays, float cb masks without
     float* const cmask = sm + Lay<COEF>::coef + slot0;
@@ -496,7 +490,6 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     PROF_DECL;
     for (int k = k0; k < k1; ++k) {
         const bool last = (k == T - 1);
-        PROF_MARK(7);
         const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
         const int lx = (lane - o0) & (BX - 1);
         const int gx = o0 + lx;
@@ -509,7 +502,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             ly[r] = (ys0 + r - o1) & (BY - 1);
             gy[r] = o1 + ly[r];
             col_in[r] = ((unsigned)gx < (unsigned)nx) & ((unsigned)gy[r] < (unsigned)ny);
-            col_off[r] = col_in[r] ? gx + (long long)nx * gy[r] : 0;
+            col_off[r] = col_in[r] ? gx + ldx * gy[r] : 0;
         }
         // the entering shell row l_y = 0 is row 0 of one warp or row 1 of one warp (warp-uniform tests)
 
@@ -545,8 +538,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
 #pragma unroll
             for (int l = 1; l < BZ; ++l) {
-                exHz[(l - 1) * PLANE + slot1] = hz[RL][l];
-                exHx[(l - 1) * PLANE + slot1] = hx[RL][l];
+                exH[(l - 1) * PLANE + slot1] = make_float2(hz[RL][l], hx[RL][l]);
             }
         } else {
             mbar_wait(mb + MB_HREADY, ph.hready & 1u);
@@ -566,8 +558,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                         hy[r][l] = stgH[yidx<3>(1, l, xs)];
                         hz[r][l] = stgH[yidx<3>(2, l, xs)];
                         if (r == RL) {    // its y+1 neighbour is the next warp's row 0, which reads it from the exchange
-                            exHz[(l - 1) * PLANE + slot1] = hz[r][l];
-                            exHx[(l - 1) * PLANE + slot1] = hx[r][l];
+                            exH[(l - 1) * PLANE + slot1] = make_float2(hz[r][l], hx[r][l]);
                         }
                     }
                 }
@@ -597,8 +588,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #pragma unroll
         for (int l = BZ - 1; l >= 1; --l) {
             const int cidx = ((o2 + l) & (BZ - 1)) * PLANE;
-            const float hz_ym = exHz[(l - 1) * PLANE + slot_ym];
-            const float hx_ym = exHx[(l - 1) * PLANE + slot_ym];
+            const float2 h_ym = exH[(l - 1) * PLANE + slot_ym];
+            const float hz_ym = h_ym.x, hx_ym = h_ym.y;
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 const float hz_xm = __shfl_sync(0xffffffffu, hz[r][l], lane_m);
@@ -626,28 +617,32 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         };
         if (!COEF && fast) e_phase(std::true_type{});
         else e_phase(std::false_type{});
-        // soft source after the E update of step t0 + k (a4): rare, CTA-uniform test first
+        // soft source after the E update of step t0 + k (a4): rare, CTA-uniform tests first.  P.src_org lists the images
+        // of the source box (one on a wall grid; a box on a periodic axis also drives its copies in the ghost zones).
         {
             const long long ts = P.t0 + k;
-            if (P.g.src_comp >= 0 && ts >= 0 && ts < P.g.src_nwave &&
-                P.g.src_box[0] <= o0 + W0 && P.g.src_box[0] + P.g.src_box[3] > o0 + 1 &&
-                P.g.src_box[1] <= o1 + W1 && P.g.src_box[1] + P.g.src_box[4] > o1 + 1 &&
-                P.g.src_box[2] <= o2 + W2 && P.g.src_box[2] + P.g.src_box[5] > o2 + 1) {
-                const float wsrc = __ldg(P.g.src_wave + ts);
-                const int sx = gx - P.g.src_box[0];
+            if (P.nsrc > 0 && ts >= 0 && ts < P.g.src_nwave) {
+                for (int si = 0; si < P.nsrc; ++si) {
+                    const int b0 = P.src_org[si][0], b1 = P.src_org[si][1], b2 = P.src_org[si][2];
+                    if (b0 <= o0 + W0 && b0 + P.g.src_box[3] > o0 + 1 && b1 <= o1 + W1 && b1 + P.g.src_box[4] > o1 + 1 &&
+                        b2 <= o2 + W2 && b2 + P.g.src_box[5] > o2 + 1) {
+                        const float wsrc = __ldg(P.g.src_wave + ts);
+                        const int sx = gx - b0;
 #pragma unroll
-                for (int r = 0; r < NROW; ++r) {
-                    const int sy = gy[r] - P.g.src_box[1];
-                    if ((lx >= 1) & (ly[r] >= 1) && sx >= 0 && sx < P.g.src_box[3] && sy >= 0 && sy < P.g.src_box[4]) {
+                        for (int r = 0; r < NROW; ++r) {
+                            const int sy = gy[r] - b1;
+                            if ((lx >= 1) & (ly[r] >= 1) && sx >= 0 && sx < P.g.src_box[3] && sy >= 0 && sy < P.g.src_box[4]) {
 #pragma unroll
-                        for (int l = 1; l < BZ; ++l) {
-                            const int sz = o2 + l - P.g.src_box[2];
-                            if (sz >= 0 && sz < P.g.src_box[5]) {
-                                const float amp = __ldg(P.g.src_amp + (sx + P.g.src_box[3] * (sy + (long long)P.g.src_box[4] * sz)));
-                                const float inj = amp * wsrc;
-                                if (P.g.src_comp == 0) ex[r][l + 1] = ex[r][l + 1] + inj;
-                                else if (P.g.src_comp == 1) ey[r][l + 1] = ey[r][l + 1] + inj;
-                                else ez[r][l + 1] = ez[r][l + 1] + inj;
+                                for (int l = 1; l < BZ; ++l) {
+                                    const int sz = o2 + l - b2;
+                                    if (sz >= 0 && sz < P.g.src_box[5]) {
+                                        const float amp = __ldg(P.g.src_amp + (sx + P.g.src_box[3] * (sy + (long long)P.g.src_box[4] * sz)));
+                                        const float inj = amp * wsrc;
+                                        if (P.g.src_comp == 0) ex[r][l + 1] = ex[r][l + 1] + inj;
+                                        else if (P.g.src_comp == 1) ey[r][l + 1] = ey[r][l + 1] + inj;
+                                        else ez[r][l + 1] = ez[r][l + 1] + inj;
+                                    }
+                                }
                             }
                         }
                     }
@@ -659,40 +654,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         if (lx != 0) {
 #pragma unroll
             for (int l = 1; l < BZ - 1; ++l) {
-                exEz[l * PLANE + slot0] = ez[0][l + 1];
-                exEx[l * PLANE + slot0] = ex[0][l + 1];
+                exE[l * PLANE + slot0] = make_float2(ez[0][l + 1], ex[0][l + 1]);
             }
-        }
-        // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
-        // They are first used by E phase k+1 (shell cells are not in R_k), so their copy and scatter run a phase behind
-        // the field shell: the compute warps wait for them here, after E phase k, not at the top of the step.
-        if (k >= 1 && !fast) {
-            mbar_wait(mb + MB_CREADY, ph.cready & 1u);
-            ++ph.cready;
-            // the entering plane l_z = 0 -> this thread's private slots (row and column: auxiliary warp)
-            const int cidx = (o2 & (BZ - 1)) * PLANE;
-#pragma unroll
-            for (int r = 0; r < NROW; ++r) {
-                if (COEF) {
-                    const float* sc = sm + Lay<COEF>::stgc;
-                    float v[6];
-#pragma unroll
-                    for (int c = 0; c < 6; ++c) v[c] = sc[zidx<6>(c, ly[r], xs)];
-                    float2 pr[3];
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) pr[c] = make_float2(v[c], v[3 + c]);
-                    if ((o0 <= 0) | (o1 <= 0) | (o2 <= 0)) {   // CTA-uniform: the box touches a low wall
-#pragma unroll
-                        for (int c = 0; c < 3; ++c) pr[c] = coef_pair(P, c, v[c], v[3 + c], gx, gy[r], o2);
-                    }
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) cpair[cidx + r * SX + c * (BZ * PLANE)] = pr[c];
-                } else {
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) cmask[cidx + r * SX + c * (BZ * PLANE)] = cb_mask(P, c, gx, gy[r], o2);
-                }
-            }
-            warp_arrive(mb + MB_CFREE);
         }
         PROF_MARK(2);
         if (k > k0) {   // the signal warp has copied the x-out rows of step k-1 (and the DONE barriers cannot lap it)
@@ -745,8 +708,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             ey[r][1] = stgE[zidx<3>(1, ly[r], xs)];
             ez[r][1] = stgE[zidx<3>(2, ly[r], xs)];
         }
-        exEz[slot0] = ez[0][1];
-        exEx[slot0] = ex[0][1];
+        exE[slot0] = make_float2(ez[0][1], ex[0][1]);
 #pragma unroll
         for (int r = 0; r < NROW; ++r) {
             if (ly[r] == 0) {             // warp-uniform: the entering row
@@ -771,14 +733,25 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         warp_arrive(mb + MB_EFREE);
-        bar_sync(1, NCOMPUTE);   // exchange rows of E are visible
+        bar_sync(1, NCOMPUTE);   // exchange rows of E are visible; every warp has finished E phase k
         PROF_MARK(5);
+        // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
+        // first used by E phase k+1 (shell cells are not in R_k); copied a whole step ahead (issued after CFREE(k-1))
+        if (k >= 1 && !fast) {
+            if (COEF) {
+                mbar_wait(mb + MB_CFULL, ph.cfull & 1u);
+                ++ph.cfull;
+            }
+            absorb_coef_shell<COEF>(P, sm, o0, o1, o2, lx, ly, ys0);
+            warp_arrive(mb + MB_CFREE);
+        }
+        PROF_MARK(7);
 
         // ---------------- H phase on R_{k+1} = [0,w-1]^3 (a2): every slot computes ----------------------------
 #pragma unroll
         for (int l = BZ - 2; l >= 0; --l) {
-            const float ez_yp = exEz[l * PLANE + slot_yp];
-            const float ex_yp = exEx[l * PLANE + slot_yp];
+            const float2 e_yp = exE[l * PLANE + slot_yp];
+            const float ez_yp = e_yp.x, ex_yp = e_yp.y;
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 const float ey_xp = __shfl_sync(0xffffffffu, ey[r][l + 1], lane_p);
@@ -790,8 +763,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 hy[r][l + 1] = yee_h_update(hy[r][l], ex[r][l + 2], ex[r][l + 1], ez_xp, ez[r][l + 1], rdz, rdx, dby);   // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
                 hz[r][l + 1] = yee_h_update(hz[r][l], ey_xp, ey[r][l + 1], ex_y, ex[r][l + 1], rdx, rdy, dbz);           // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
             }
-            exHz[l * PLANE + slot1] = hz[RL][l + 1];
-            exHx[l * PLANE + slot1] = hx[RL][l + 1];
+            exH[l * PLANE + slot1] = make_float2(hz[RL][l + 1], hx[RL][l + 1]);
         }
         if (k > k0) {   // the signal warp has copied the H x-out rows of step k-1 (HDONE cannot lap its waiters)
             mbar_wait(mb + MB_ACKH, ph.ackh & 1u);
@@ -851,7 +823,6 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         mbar_init(mb + MB_CFULL, 1);
         mbar_init(mb + MB_EFULL, 1);
         mbar_init(mb + MB_HREADY, 1);
-        mbar_init(mb + MB_CREADY, 1);
         mbar_init(mb + MB_CFREE, NWARPS_C);
         mbar_init(mb + MB_EREADY, 1);
         mbar_init(mb + MB_HFREE, NWARPS_C);
@@ -972,25 +943,14 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                         warp_arrive(mb + MB_HREADY);
                         PROF_MARK(4);
                     } else {
-                        // coefficient shell (constants of the run: no flag, no proxy fence): copy once the compute warps have
-                        // absorbed the previous plane, scatter row and column once E phase k-1 has read the leaving
-                        // cells' slots -> CREADY(k), awaited after E phase k
-                        if (!fast) {                 // (a uniform interior tile has no coefficient pipeline)
+                        // coefficient shell (constants of the run: no flag, no proxy fence): copied as soon as the compute
+                        // warps have taken the previous one out of the staging (CFREE), a whole step before it is needed
+                        if (COEF && !fast) {         // (a uniform tile has no coefficient copy)
                         if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
                         PROF_MARK(0);
-                        if (COEF && lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                         __syncwarp();
                         PROF_MARK(1);
-                        if (k > k0) { mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone; }
-                        PROF_MARK(2);
-                        if (COEF && !FDTD_DBG(P, 2)) { mbar_wait(mb + MB_CFULL, n_cfull & 1u); ++n_cfull; }
-                        PROF_MARK(3);
-                        if (!FDTD_DBG(P, 16)) {
-                            scatter_coef<COEF>(P, sm, o0, o1, o2, 0);
-                            scatter_coef<COEF>(P, sm, o0, o1, o2, 1);
-                        }
-                        warp_arrive(mb + MB_CREADY);
-                        PROF_MARK(4);
                         }
                     }
                 }
@@ -998,8 +958,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             if (warp == W_HPROD) PROF_FLUSH(8);
             if (warp == W_HAUX) PROF_FLUSH(16);
             // phases of the last step that this warp does not wait for: covered by the CTA barrier at the tile boundary
-            if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else if (!fast) ++n_cfree; }
-            if (k1 > k0 && warp == W_HAUX) n_edone += fast ? (unsigned)(k1 - k0) : 1u;
+            if (k1 > hk0) { if (warp == W_HPROD) ++n_hfree; else if (COEF && !fast) ++n_cfree; }
         } else if (warp == W_EPROD) {
             // the flags of step k are acquired (and the async proxy ordered after them) while the copy of step k-1 is in
             // flight: the ~0.7 us proxy fence is off the EFREE -> EREADY chain
@@ -1027,15 +986,13 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
                 if (k > k0) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
                 // the shell column's Ez, Ex of planes 1..6 for its y-1 readers in the H phase
-                float* exEz = sm + Lay<COEF>::exch + 2 * EXP;
-                float* exEx = exEz + EXP;
+                float2* exE = reinterpret_cast<float2*>(sm + Lay<COEF>::exch) + EXP;
                 for (int r = 0; r < 3; ++r) {
                     const int idx = r * 32 + lane;            // (l-1)*15 + (ly-1), l = 1..6
                     if (idx < W1 * (W2 - 1)) {
                         const int ly = 1 + idx % W1, l = 1 + idx / W1;
                         const int s = ((o1 + ly) & (BY - 1)) * SX + (o0 & (BX - 1));
-                        exEz[l * PLANE + s] = stg[xidx<3>(2, ly, l) + (o0 & 3)];
-                        exEx[l * PLANE + s] = stg[xidx<3>(0, ly, l) + (o0 & 3)];
+                        exE[l * PLANE + s] = make_float2(stg[xidx<3>(2, ly, l) + (o0 & 3)], stg[xidx<3>(0, ly, l) + (o0 & 3)]);
                     }
                 }
                 warp_arrive(mb + MB_EREADY);

@@ -160,6 +160,46 @@ def test_tma_kernel_per_array_maps_separate_allocations(cuda_device):
         _compare(E, H, Eo, Ho, exact=True)
 
 
+# ---- periodic axes and odd nx through the product kernel (padded working copy) --------------------------
+PADDED = {
+    "per-x": ((64, 56, 40), (1, 1, 1), (PERIODIC, PEC, PEC), "waveguide", "sheet"),
+    "per-y-odd-nx": ((37, 29, 23), (1, 0.8, 1.3), (PEC, PERIODIC, PEC), "lossy", "dipole"),
+    "per-xyz": ((24, 20, 12), (1, 1, 1), (PERIODIC,) * 3, "blocks", "sheet"),
+    "per-z-vac": ((40, 33, 50), (1, 1, 0.5), (PEC, PEC, PERIODIC), "none", "dipole"),
+    "odd-nx-pec": ((45, 31, 19), (1, 1, 1), (PEC,) * 3, "lossy", "dipole"),
+}
+
+
+@pytest.mark.parametrize("variant", ["nofma", "fma"])
+@pytest.mark.parametrize("T", [0, 3, 8, 20])
+@pytest.mark.parametrize("name", list(PADDED))
+def test_padded_working_copy_matches_oracle(cuda_device, name, T, variant):
+    """Grids with a periodic axis (ghost zones refilled between launches, source images in the ghosts) or nx % 4 != 0
+    (row pitch padded) run the TMA kernel on the library's padded copy; 70 steps in pieces, several launches each."""
+    n, d, bnd, coeffs, source = PADDED[name]
+    w = workloads.Workload(name, n, d, bnd, 70, "uniform", coeffs, source, seed=21)
+    E0, H0 = workloads.make_fields(w)
+    ca, cb = workloads.make_coeffs(w)
+    s = workloads.make_source(w)
+    src = (s.comp, s.box, s.amp, s.wave)
+    Eo, Ho = _run_oracle(w.n, w.d, w.dt, w.boundary, E0, H0, ca, cb, None, src, 70)
+    E, H = _to_dev(E0), _to_dev(H0)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant=variant)
+    sim.set_fields(E, H)
+    if ca is not None:
+        g = _to_dev(list(ca) + list(cb))
+        sim.set_coeffs(g[:3], g[3:], None)
+    sim.set_source(*src)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC, (31, 15, 7) if T else None, T)
+    info = sim.get_kernel()
+    assert info["which"] == binding.KERNEL_SYSTOLIC and info["smem"] in (229632, 147456)
+    for part in (1, 29, 40):
+        sim.step(part)
+    sim.sync()
+    sim.close()
+    _compare(E, H, Eo, Ho, exact=(variant == "nofma"))
+
+
 # ---- (c) "after the full run", library defaults, both builds -----------------------------------------------------
 FULL = [("C1", 0, None), ("C4-64", 3, 64), ("C4-128", 3, 128), ("C4-256", 3, 256), ("C2", 1, None), ("C4-512", 3, 512)]
 

@@ -1,14 +1,18 @@
 #!/usr/bin/env python
-"""bench.py -- TCUPS of the FDTD hot path on BASELINE.json configs[1] (256^3 heterogeneous dielectric, six per-cell
-coefficient arrays, z-dipole Gaussian-pulse source, PEC walls, 1000 steps, fp32), one JSON line on stdout.
+"""bench.py -- TCUPS of the FDTD hot path, one JSON line on stdout.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--tsteps S] [--kernel systolic|naive] [--impl reference]
+                    [--config I] [--size n] [--no-sweep] [--no-e2e] [--no-cpu-baseline]
 
-A bench "step" is one fdtd_step(S) call: S = 100 FDTD time steps of the whole grid (all rows of SURVEY.md 8(a):
-E half-step, source, H half-step, walls, and for the systolic kernel tile residency, shell load/store, flags,
-slide, launch ramp), so the default K = 10 is exactly the configuration's 1000 steps.  `value` is timed with the
-fields resident in HBM (CUDA events on the stream the kernels run on); `e2e` goes through the same C-ABI calls
-with HOST buffers: pinned host -> device copy of the six field arrays, S steps, device -> host copy, every step.
+Headline workload: BASELINE.json configs[4] (1536x1536x768 lossy heterogeneous grid, six per-cell coefficient arrays,
+anisotropic cells, point source, 81 GiB resident) -- the largest single-GPU configuration, far above L2, and the one
+closest to the paper's own "bare-bones" benchmark (permittivity and conductivity fields).  A bench "step"
+is one fdtd_step(S) call: S = 100 FDTD time steps of the whole grid (all rows of SURVEY.md 8(a): E half-step, source,
+H half-step, walls, tile residency, shell load/store, flags, slide, launch ramp).  `value` is timed with the fields
+resident in HBM (CUDA events on the stream the kernels run on); `e2e` goes through the same C-ABI calls with HOST
+buffers: pinned host -> device copy of the six field arrays, S steps, device -> host copy, every step.
+`sweep` (same JSON line, N = 1 only) is the metric "TCUPS vs grid size": naive and systolic kernels on configs 1, 2, 3,
+the configs[3] cubes 64^3 .. 1024^3 and config 5, each timed in this run, with the fraction of its own roofline.
 N > 1: the path does not shard ("replicas only"): every rank runs the same workload on its own GPU and
 `value` sums them over the max-over-ranks time.
 """
@@ -20,28 +24,35 @@ import threading
 import time
 from dataclasses import replace
 
+# the CPU oracle's OpenMP team: one thread per core, pinned, set before libgomp is loaded (stable cpu_baseline numbers)
+os.environ.setdefault("OMP_PROC_BIND", "close")
+os.environ.setdefault("OMP_PLACES", "cores")
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "TCUPS (6-component Yee cell updates/s, fp32) vs grid size; HBM GB/s"
-TMA_SMEM = (229632, 147456)     # dynamic shared memory of systolic_tma.cu with / without coefficient arrays
+HEADLINE_CONFIG = 4
+SM_COUNT, SM_HZ_NOMINAL = 148, 1.965e9
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--tsteps", type=int, default=100, help="FDTD time steps per bench step")
     ap.add_argument("--kernel", default="systolic", choices=["systolic", "naive"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (0-based)")
+    ap.add_argument("--config", type=int, default=HEADLINE_CONFIG, help="BASELINE.json configs index (0-based)")
     ap.add_argument("--size", type=int, default=0, help="cube size for the configs[3] sweep")
     ap.add_argument("--tile", default="", help="NXxNYxNZ systolic tile (default: library choice)")
     ap.add_argument("--T", type=int, default=0, help="temporal depth (default: library choice)")
-    ap.add_argument("--variant", default="fma", choices=["fma", "nofma", "prof"])
+    ap.add_argument("--variant", default="nofma", choices=["nofma", "fma", "prof"],
+                    help="nofma = the product library (bit-exact); fma = optional contracted build")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true")
     return ap.parse_args()
 
 
@@ -70,8 +81,8 @@ class ClockSampler(threading.Thread):
         if self.nv is None:
             return
         nv = self.nv
-        names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown if hasattr(nv, "nvmlClocksEventReasonHwSlowdown") else 0x8,
-                 "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4, "hw_power_brake": 0x80}
+        names = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4,
+                 "hw_power_brake": 0x80}
         while not self.stop_flag:
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
@@ -92,12 +103,12 @@ class ClockSampler(threading.Thread):
                 "samples": len(s)}
 
 
-def algorithmic_bytes_per_cell_update(kernel, info, has_coef):
-    """SURVEY.md 8(d) / DESIGN.md: global-memory bytes the schedule must move per 6-component cell update."""
+def algorithmic_bytes_per_cell_update(kernel, tile, T, has_coef):
+    """SURVEY.md 8(d) / DESIGN.md 6.5: global-memory bytes the schedule must move per 6-component cell update.
+    T is the depth of the launch that was actually timed (min(library depth, steps per call))."""
     if kernel == "naive":
         return 96.0 if has_coef else 72.0
-    Nx, Ny, Nz = info["tile"]
-    T = info["T"]
+    Nx, Ny, Nz = tile
     V = Nx * Ny * Nz
     B = (Nx + 1) * (Ny + 1) * (Nz + 1)
     X = B - V                                   # minus shell of the box
@@ -125,59 +136,176 @@ def job_tcups(world, cell_updates_per_rank, seconds):
     return world * cell_updates_per_rank / seconds / 1e12
 
 
-def run_reference(args):
-    """--impl reference: the CPU oracle as it stands, on the host cores, same config / metric / unit."""
-    import numpy as np
+# ---- the CPU oracle beside the GPU run ----------------------------------------------------------------------------
+def oracle_sample(w):
+    """A bounded sample of workload w for the CPU oracle: the whole grid up to 64 M cells, else the same recipe on a grid
+    a quarter as long per axis (config 5: 384x384x192, 28 M cells; the full grid would need 87 GB of host arrays)."""
+    if w.cells <= (1 << 26):
+        return w, f"full {w.n[0]}x{w.n[1]}x{w.n[2]} grid"
+    n = tuple(max(32, x // 4) for x in w.n)
+    return w.scaled(n, steps=w.steps, name=w.name), f"{n[0]}x{n[1]}x{n[2]} grid of the same recipe (1/64 of the cells of {w.name})"
+
+
+def make_oracle(w):
     from oracle.yee import YeeOracle
     from paper_2502_20610_b200 import workloads
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return
-    ref_tsteps = 2                               # bounded sample: each bench step advances the full grid 2 time steps
-    w = workload_of(args, (args.steps + args.warmup) * ref_tsteps)
     E, H = workloads.make_fields(w)
     ca, cb = workloads.make_coeffs(w)
     orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None)
     src = workloads.make_source(w)
     if src is not None:
         orc.set_source(src.comp, src.box, src.amp, src.wave)
-    for _ in range(args.warmup):
+    return orc
+
+
+def cpu_baseline(w_full, config_steps, budget_s=12.0):
+    """The oracle as it stands, timed on the host cores on a bounded sample (about 10-20 s of CPU work).  Runs before any
+    CUDA or pinned-memory allocation of this process, with the OpenMP team pinned (see the top of this file)."""
+    w, what = oracle_sample(w_full)
+    orc = make_oracle(w)
+    orc.step(2)                                   # warm-up: page faults, thread team
+    t0 = time.perf_counter()
+    orc.step(2)
+    per_step = (time.perf_counter() - t0) / 2
+    n = int(min(400, max(4, budget_s / max(per_step, 1e-6))))
+    t0 = time.perf_counter()
+    orc.step(n)
+    dt = time.perf_counter() - t0
+    return {"value": w.cells * n / dt / 1e12, "unit": "TCUPS", "cores": orc.nthreads, "kind": "oracle",
+            "sample": f"{what}, {n} of the config's {config_steps} time steps (after 4 warm-up steps)"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores, same config / metric / unit; each bench step is a
+    bounded sample (2 time steps of oracle_sample(config))."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    ref_tsteps = 2
+    from paper_2502_20610_b200 import workloads
+    w_full = workload_of(args, (args.steps + args.warmup) * ref_tsteps)
+    w, what = oracle_sample(w_full)
+    orc = make_oracle(w)
+    for _ in range(max(args.warmup, 1)):
         orc.step(ref_tsteps)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         orc.step(ref_tsteps)
     dt = time.perf_counter() - t0
     tcups = w.cells * ref_tsteps * args.steps / dt / 1e12
-    sample = f"full {w.n[0]}x{w.n[1]}x{w.n[2]} grid, {ref_tsteps} time steps per bench step (of the config's 1000)"
+    sample = f"{what}, {ref_tsteps} time steps per bench step (of the config's {workloads.config(args.config, args.size or None).steps})"
     line = {"impl": "reference", "metric": METRIC, "value": tcups, "unit": "TCUPS", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "grid": list(w.n), "time_steps_per_bench_step": ref_tsteps},
+            "config": {"workload": w_full.name, "grid": list(w_full.n), "sample_grid": list(w.n), "time_steps_per_bench_step": ref_tsteps},
             "cpu_baseline": {"value": tcups, "unit": "TCUPS", "cores": orc.nthreads, "kind": "oracle", "sample": sample},
             "e2e": {"value": tcups, "unit": "TCUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def cpu_baseline(w, config_steps):
-    """The oracle timed beside the GPU run on a bounded sample (about 10-20 s of CPU work)."""
-    from oracle.yee import YeeOracle
-    from paper_2502_20610_b200 import workloads
-    E, H = workloads.make_fields(w)
-    ca, cb = workloads.make_coeffs(w)
-    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None)
+# ---- one timed case on the device --------------------------------------------------------------------------------
+def setup_case(w, kernel, variant, dev, tile=None, T=0):
+    """Seeded inputs of workload w on the device, a context bound to them."""
+    from paper_2502_20610_b200 import binding, workloads
+    E, H = workloads.make_fields(w, device=dev)
+    ca, cb = workloads.make_coeffs(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant=variant)
+    sim.set_fields(E, H)
+    if ca is not None:
+        sim.set_coeffs(ca, cb, None)
     src = workloads.make_source(w)
     if src is not None:
-        orc.set_source(src.comp, src.box, src.amp, src.wave)
-    t0 = time.perf_counter()
-    orc.step(2)
-    per_step = (time.perf_counter() - t0) / 2
-    n = int(min(200, max(2, 12.0 / max(per_step, 1e-6))))
-    t0 = time.perf_counter()
-    orc.step(n)
-    dt = time.perf_counter() - t0
-    return {"value": w.cells * n / dt / 1e12, "unit": "TCUPS", "cores": orc.nthreads, "kind": "oracle",
-            "sample": f"full {w.n[0]}x{w.n[1]}x{w.n[2]} grid, {n} of the config's {config_steps} time steps (after 2 warm-up steps)"}
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC if kernel == "systolic" else binding.KERNEL_NAIVE, tile, T)
+    return sim, (E, H, ca, cb)
+
+
+def load_counters():
+    """Measured per-cell-update counters of the systolic kernel (ncu captures, profiles/traffic.json)."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    except Exception:
+        return {}
+
+
+def roofline_of(kernel, w, info, has_coef, S, tcups, peak_gbs, counters):
+    """HBM roofline of one case: algorithmic bytes per cell update of the launch that was timed x achieved rate / peak."""
+    T = min(info["T"], S) if kernel == "systolic" else 0
+    bpc = algorithmic_bytes_per_cell_update(kernel, info["tile"], max(T, 1), has_coef)
+    achieved = bpc * tcups * 1e12 / 1e9
+    out = {"bytes_per_cell_update": bpc, "T_launched": T, "achieved_gbs": achieved, "frac": achieved / peak_gbs,
+           "roof_tcups": peak_gbs * 1e9 / bpc / 1e12}
+    key = "systolic:coef" if has_coef else "systolic:uniform"
+    if kernel == "systolic" and key in counters:
+        c = counters[key]
+        # explanatory on-chip ceilings from MEASURED counters: every warp instruction takes one of 4 issue slots per SM and
+        # clock; every shared-memory wavefront one cycle of the SM's 128-byte data path
+        hz = SM_HZ_NOMINAL
+        out["issue_roof_tcups"] = SM_COUNT * 4 * hz / c["warp_inst_per_cell_update"] / 1e12
+        out["smem_roof_tcups"] = SM_COUNT * hz / c["smem_wavefronts_per_cell_update"] / 1e12
+    return out
+
+
+def time_case(sim, S, K, W, barrier=None):
+    """W untimed + K timed fdtd_step(S) calls; CUDA events on the stream the kernels run on.  Returns (ms, launches)."""
+    import torch
+    for _ in range(W):
+        sim.step(S)
+    sim.sync()
+    if barrier is not None:
+        barrier()
+    c0 = sim.counters()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(K):
+        sim.step(S)
+    ev1.record()
+    if barrier is not None:
+        barrier()
+    sim.sync()
+    return ev0.elapsed_time(ev1), sim.counters()["launches"] - c0["launches"]
+
+
+SWEEP = [("C1", 0, None), ("C4-64", 3, 64), ("C4-128", 3, 128), ("C4-256", 3, 256), ("C2", 1, None), ("C4-512", 3, 512),
+         ("C3", 2, None), ("C4-768", 3, 768), ("C4-1024", 3, 1024), ("C5", 4, None)]
+
+
+def run_sweep(variant, dev, peak_gbs, counters, headline, skip_name):
+    """TCUPS vs grid size (the metric; Fig. 1): both kernels on every config, a few launches each."""
+    import torch
+    from paper_2502_20610_b200 import workloads
+    rows = []
+    for name, idx, size in SWEEP:
+        w0 = workloads.config(idx, size)
+        if w0.name == skip_name:            # the headline workload was just timed: reuse its numbers
+            rows.append(headline)
+            continue
+        # S time steps per call, K calls: the config's own step count where that is a few launches, never less than 2 calls
+        S = min(w0.steps, 100 if w0.cells > (1 << 24) else 200)
+        row = {"workload": w0.name, "grid": list(w0.n), "working_set_mb": (12 if w0.has_coeff_arrays else 6) * w0.cells * 4 / 1e6,
+               "time_steps_per_call": S}
+        for kernel in ("naive", "systolic"):
+            K, W = (2, 1) if w0.cells > (1 << 27) else (3, 2)
+            Sk = S if kernel == "systolic" else max(10, min(S, int(2e10 / w0.cells)))       # the naive rate does not depend on S
+            w = replace(w0, steps=max(w0.steps, (K + W) * Sk + 1))
+            sim, keep = setup_case(w, kernel, variant, dev)
+            info = sim.get_kernel()
+            ms, launches = time_case(sim, Sk, K, W)
+            tc = w.cells * Sk * K / (ms * 1e-3) / 1e12
+            r = roofline_of(kernel, w, info, w.has_coeff_arrays, Sk, tc, peak_gbs, counters)
+            row[kernel + "_tcups"] = tc
+            row[kernel + "_frac"] = r["frac"]
+            row[kernel + "_bytes_per_cell_update"] = r["bytes_per_cell_update"]
+            if kernel == "systolic":
+                row["T"] = r["T_launched"]
+                row["tiles_per_launch"] = info["tiles"]
+            sim.close()
+            del sim, keep
+            torch.cuda.empty_cache()
+        row["systolic_over_naive"] = row["systolic_tcups"] / row["naive_tcups"]
+        rows.append(row)
+    return rows
 
 
 def main():
@@ -185,13 +313,20 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
-    import numpy as np
-    import torch
-    from paper_2502_20610_b200 import binding, build, workloads
-
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    S, K, W = args.tsteps, args.steps, max(args.warmup, 0)
+    w = workload_of(args, (K + W) * S * 2)
+
+    # ---- the CPU oracle first: before CUDA initialisation and before any pinned allocation of this process --------
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        from paper_2502_20610_b200 import workloads as _wl
+        cpu = cpu_baseline(w, _wl.config(args.config, args.size or None).steps)
+
+    import torch
+    from paper_2502_20610_b200 import binding, build, workloads
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     if not os.path.exists(binding.lib_path(args.variant)):
@@ -203,22 +338,10 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
-    S, K, W = args.tsteps, args.steps, max(args.warmup, 0)
-    w = workload_of(args, (K + W) * S * 2)
-    kernel = binding.KERNEL_SYSTOLIC if args.kernel == "systolic" else binding.KERNEL_NAIVE
     tile = tuple(int(x) for x in args.tile.split("x")) if args.tile else None
-
-    E, H = workloads.make_fields(w, device=dev)
-    ca, cb = workloads.make_coeffs(w, device=dev)
-    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant=args.variant)
-    sim.set_fields(E, H)
-    if ca is not None:
-        sim.set_coeffs(ca, cb, None)
-    src = workloads.make_source(w)
-    if src is not None:
-        sim.set_source(src.comp, src.box, src.amp, src.wave)
-    sim.set_kernel(kernel, tile, args.T)
+    sim, keep = setup_case(w, args.kernel, args.variant, dev, tile, args.T)
     info = sim.get_kernel()
+    has_coef = keep[2] is not None
 
     def barrier():
         if dist is not None:
@@ -231,22 +354,9 @@ def main():
     sim.sync()
     sampler = ClockSampler(local)
     sampler.start()
-    barrier()
-    c0 = sim.counters()
-    kernel_ms = 0.0
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    for _ in range(K):
-        sim.step(S)
-    ev1.record()
-    barrier()
-    sim.sync()
-    total_ms = ev0.elapsed_time(ev1)
-    kernel_ms = total_ms          # the region holds nothing but the enqueued kernels (and a 4-byte memset per launch)
-    c1 = sim.counters()
+    total_ms, launches = time_case(sim, S, K, 0, barrier)
     sampler.stop_flag = True
     sampler.join()
-    launches = c1["launches"] - c0["launches"]
     total_ms = max_over_ranks(dist, total_ms, dev)
     cell_updates = w.cells * S * K
     value = job_tcups(world, cell_updates, total_ms * 1e-3)
@@ -254,15 +364,21 @@ def main():
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     e2e = None
     if not args.no_e2e:
-        Eh, Hh = workloads.make_fields(w)
-        pin = lambda a: torch.from_numpy(a).pin_memory()
-        Ein, Hin = [pin(a) for a in Eh], [pin(a) for a in Hh]
-        Eout = [torch.empty_like(t).pin_memory() for t in Ein]
-        Hout = [torch.empty_like(t).pin_memory() for t in Hin]
-        ke = max(2, min(K, 5))
-        sim.set_time(0)
+        shape = (w.n[2], w.n[1], w.n[0])
+        nbytes = 6 * w.cells * 4
+        ke = 2 if nbytes > (8 << 30) else max(2, min(K, 5))
+        if w.fields == "zero":
+            Ein = [torch.zeros(shape, dtype=torch.float32).pin_memory() for _ in range(3)]
+            Hin = [torch.zeros(shape, dtype=torch.float32).pin_memory() for _ in range(3)]
+        else:
+            Eh, Hh = workloads.make_fields(w)
+            Ein, Hin = [torch.from_numpy(a).pin_memory() for a in Eh], [torch.from_numpy(a).pin_memory() for a in Hh]
+            del Eh, Hh
+        Eout = [torch.empty(shape, dtype=torch.float32).pin_memory() for _ in range(3)]
+        Hout = [torch.empty(shape, dtype=torch.float32).pin_memory() for _ in range(3)]
 
         def one():
+            sim.set_time(0)
             sim.load_fields(Ein, Hin)
             sim.step(S)
             sim.get_fields(Eout, Hout)
@@ -270,18 +386,17 @@ def main():
         barrier()
         t0 = time.perf_counter()
         for _ in range(ke):
-            sim.set_time(0)
             one()
         barrier()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dist, dt, dev)
-        nbytes = 6 * w.cells * 4
+        dt = max_over_ranks(dist, time.perf_counter() - t0, dev)
         e2e = {"value": job_tcups(world, w.cells * S * ke, dt), "unit": "TCUPS", "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": ke,
                "note": "six field arrays pinned host->device, S time steps, six arrays device->host, per bench step; "
                        "the six coefficient arrays are problem constants bound once"}
+        del Ein, Hin, Eout, Hout
 
     if rank != 0:
+        sim.close()
         if dist is not None:
             dist.destroy_process_group()
         return
@@ -293,46 +408,62 @@ def main():
     except Exception:
         pass
     peak = float(peaks.get("hbm_gbs", 6650.0))
-    bpc = algorithmic_bytes_per_cell_update(args.kernel, info, ca is not None)
-    achieved = bpc * cell_updates / (kernel_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+    counters = load_counters()
+    r = roofline_of(args.kernel, w, info, has_coef, S, value / world, peak, counters)
+    tma = info["smem"] in (229632, 147456)
+    roofline = {"bound": "hbm", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"], "traffic": None,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy)" if "hbm_gbs" in peaks else "fallback 6.65 TB/s",
-                "algorithmic_bytes_per_cell_update": bpc,
-                "kernel": ("systolic_tma_kernel" if info["smem"] in TMA_SMEM else "systolic_reg_kernel") if args.kernel == "systolic" else "e_half_naive+h_half_naive",
-                "launches_in_region": launches, "avg_launch_ms": kernel_ms / max(launches, 1),
-                "roof_tcups": peak * 1e9 / bpc / 1e12,
-                # explanatory ceilings of the systolic kernel: arithmetic-only issue floor (33 FMA-contracted
-                # instructions per cell), the kernel's own instruction mix at 100 % issue, the shared-memory pipe
-                "fp32_roof_tcups": 148 * 128 * 1.965e9 / 33 / 1e12,
-                "issue_roof_tcups": 148 * 128 * 1.965e9 / 118 / 1e12,
-                "smem_roof_tcups": 148 * 1.965e9 * 3255 / 2300 / 1e12}
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(prof):
-        try:
-            tr = json.load(open(prof))
-            key = f"{args.kernel}:{w.name}"
-            if key in tr:
-                roofline["traffic"] = tr[key]["dram_bytes_per_launch"]
-                roofline["traffic_source"] = tr[key].get("source")
-        except Exception:
-            pass
+                "algorithmic_bytes_per_cell_update": r["bytes_per_cell_update"], "T_launched": r["T_launched"],
+                "kernel": ("systolic_tma_kernel" if tma else "systolic_reg_kernel") if args.kernel == "systolic" else "e_half_naive+h_half_naive",
+                "launches_in_region": launches, "avg_launch_ms": total_ms / max(launches, 1), "roof_tcups": r["roof_tcups"],
+                # arithmetic-only ceiling: 45 separately rounded fp32 operations per cell update, 128 lanes per SM and clock
+                "fp32_roof_tcups": SM_COUNT * 128 * SM_HZ_NOMINAL / 45 / 1e12}
+    for k in ("issue_roof_tcups", "smem_roof_tcups"):
+        if k in r:
+            roofline[k] = r[k]
+            roofline["on_chip_counters_source"] = counters.get("source")
+    key = f"{args.kernel}:{w.name}"
+    if key in counters:
+        roofline["traffic"] = counters[key]["dram_bytes_per_launch"]
+        roofline["traffic_source"] = counters[key].get("source")
 
+    ws = (6 + (6 if has_coef else 0)) * w.cells * 4
     line = {"metric": METRIC, "value": value, "unit": "TCUPS", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "grid": list(w.n), "time_steps_per_bench_step": S, "kernel": args.kernel,
                        "tile": list(info["tile"]), "T": info["T"], "tiles_per_launch": info["tiles"], "ctas": info["ctas"],
                        "smem_per_cta": info["smem"], "variant": args.variant, "parallelism": "replicas" if world > 1 else "single",
-                       "l2": "inputs exceed L2 (%.0f MB of fields+coefficients vs 126 MB)" % ((6 + (6 if ca is not None else 0)) * w.cells * 4 / 1e6)
-                             if (6 + (6 if ca is not None else 0)) * w.cells * 4 > 200e6 else "inputs fit L2 (no flush): below-L2 point of the size sweep"},
+                       "l2": "inputs exceed L2 (%.0f MB of fields+coefficients vs 126 MB)" % (ws / 1e6) if ws > 200e6
+                             else "inputs fit L2 (no flush): below-L2 point of the size sweep"},
             "clocks": sampler.result(), "gpu_launches": int(launches), "roofline": roofline}
     if e2e is not None:
         line["e2e"] = e2e
-    if not args.no_cpu_baseline and world == 1:
-        from paper_2502_20610_b200 import workloads as _wl
-        line["cpu_baseline"] = cpu_baseline(w, _wl.config(args.config, args.size or None).steps)
-    print(json.dumps(line), flush=True)
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
     sim.close()
+    headline_row = {"workload": w.name, "grid": list(w.n), "working_set_mb": ws / 1e6, "time_steps_per_call": S,
+                    args.kernel + "_tcups": value / world, args.kernel + "_frac": r["frac"],
+                    args.kernel + "_bytes_per_cell_update": r["bytes_per_cell_update"], "T": r["T_launched"],
+                    "tiles_per_launch": info["tiles"]}
+    if world == 1 and not args.no_sweep and args.kernel == "systolic" and not args.tile and not args.T:
+        # the headline row still needs its naive leg
+        other = replace(w, steps=max(w.steps, 64))
+        Sn = max(10, min(S, int(2e10 / w.cells)))
+        del keep
+        torch.cuda.empty_cache()
+        nsim, nkeep = setup_case(other, "naive", args.variant, dev)
+        ninfo = nsim.get_kernel()
+        ms, _ = time_case(nsim, Sn, 2, 1)
+        ntc = w.cells * Sn * 2 / (ms * 1e-3) / 1e12
+        nr = roofline_of("naive", w, ninfo, has_coef, Sn, ntc, peak, counters)
+        headline_row.update({"naive_tcups": ntc, "naive_frac": nr["frac"], "naive_bytes_per_cell_update": nr["bytes_per_cell_update"],
+                             "systolic_over_naive": headline_row["systolic_tcups"] / ntc})
+        nsim.close()
+        del nsim, nkeep
+        torch.cuda.empty_cache()
+        line["sweep"] = run_sweep(args.variant, dev, peak, counters, headline_row, w.name)
+    print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
 

@@ -17,10 +17,12 @@
  *                         subdomain on chip, slide it along the x-y-z-t diagonal, exchange only faces through
  *                         global memory and hand off with per-tile flags.  It performs "the exact same update
  *                         equations", so results are identical per cell to the naive schedule.
- *                         Tile 31x15x7 on a grid with all axes FDTD_PEC and nx % 4 == 0 runs the TMA-staged
- *                         register kernel (fields in registers, coefficients in shared memory, shells fetched by
- *                         TMA boxes); tile 31x15x7 elsewhere runs FDTD_KERNEL_SYSTOLIC_REG; other built tile
- *                         shapes run FDTD_KERNEL_SYSTOLIC_SMEM.
+ *                         Tile 31x15x7 (the default) runs the TMA-staged register kernel (fields in registers,
+ *                         coefficients in shared memory, shells fetched by TMA boxes) on every grid: a grid with
+ *                         a periodic axis, or with nx % 4 != 0, runs it on a library-owned padded working copy
+ *                         (ghost zones of T cells on either side of a periodic axis, refilled before each launch
+ *                         of T steps; copy-in / copy-out of the bound arrays around every fdtd_step call).
+ *                         Other built tile shapes run FDTD_KERNEL_SYSTOLIC_SMEM.
  *   FDTD_KERNEL_SYSTOLIC_REG   the same schedule and register residency with loader warps staging the shells by
  *                         cp.async (any wall type, any nx; tile 31x15x7 only).
  *   FDTD_KERNEL_SYSTOLIC_SMEM  the same schedule with the whole subdomain in shared memory (the first,
@@ -60,7 +62,8 @@ enum { FDTD_KERNEL_NAIVE = 0, FDTD_KERNEL_SYSTOLIC = 1, FDTD_KERNEL_SYSTOLIC_SME
  * and per-axis wall type boundary[3] (host array of FDTD_PEC | FDTD_PERIODIC).
  * cuda_stream: a cudaStream_t (as void*) on which all work is enqueued; NULL = the legacy default stream.
  * Default schedule (no fdtd_set_kernel call): FDTD_KERNEL_SYSTOLIC with library-chosen tile shape and temporal depth
- * where its TMA-staged kernel applies (all axes PEC, nx % 4 == 0), FDTD_KERNEL_NAIVE otherwise; fdtd_get_kernel tells.
+ * on every grid (FDTD_KERNEL_NAIVE only while ca is bound without cb or the reverse); fdtd_get_kernel tells.
+ * All later calls run on the device that was current here, whatever device is current in the calling thread.
  * *out is written only on FDTD_OK.  FDTD_EINVAL: bad dims (each 1..2^15, product < 2^40), spacings, dt, boundary.
  * FDTD_ECUDA: no usable sm_100 device / CUDA failure.   (problem statement: PAPER.md:35-37) */
 int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, float dz, float dt,
@@ -112,10 +115,12 @@ int fdtd_sync(fdtd_ctx* ctx);
 int fdtd_set_time(fdtd_ctx* ctx, long long t);
 long long fdtd_get_time(const fdtd_ctx* ctx);
 
-/* Choose the schedule.  which = FDTD_KERNEL_NAIVE | FDTD_KERNEL_SYSTOLIC | FDTD_KERNEL_SYSTOLIC_SMEM.
+/* Choose the schedule.  which = FDTD_KERNEL_NAIVE | FDTD_KERNEL_SYSTOLIC | FDTD_KERNEL_SYSTOLIC_SMEM |
+ * FDTD_KERNEL_SYSTOLIC_REG (all four are accepted; the last two are slow cross-check implementations).
  * For the systolic kernel (Nx,Ny,Nz) is the updated tile ("subdomain": 31x15x15 updated inside a
  * 32x16x16 cached block) and T the temporal depth (steps a tile stays resident per launch); 0 = library default.
- * FDTD_EINVAL if the shape is not one the kernel was built for or the grid cannot run it (see fdtd_last_error). */
+ * FDTD_EINVAL if the shape is not one the kernel was built for or the grid cannot run it (see fdtd_last_error);
+ * the context then keeps the schedule it had before the call. */
 int fdtd_set_kernel(fdtd_ctx* ctx, int which, int Nx, int Ny, int Nz, int T);
 
 /* What fdtd_step will run: out[0]=which, out[1..3]=tile Nx,Ny,Nz, out[4]=T, out[5]=tiles per launch,
@@ -141,6 +146,14 @@ int fdtd_plan_tiles(const int n[3], const int boundary[3], const int N[3], int T
  * library uses for that axis (uniform b*N on a PEC axis; as even as possible on a ring).
  * Writes *tile, *offset.  (reading #11: cell g at step s belongs to the tile whose region [a_b - s, a_{b+1} - s) holds it) */
 int fdtd_plan_owner(int n, int boundary, int N, int T, int g, int s, int* tile, int* offset);
+
+/* Developer builds only (libfdtd_b200_dbg.so with FDTD_DEBUG_LEVELS=1 in the environment at fdtd_create): the systolic
+ * kernel keeps per-cell time-level shadow arrays and checks every value a tile takes from global memory against the
+ * level the schedule promises (the race detector of the hand-off protocol, "delayed synchronization").
+ * Synchronises; out[0] = number of violations so far, out[1..4] = the first one (kind: 1/2 H/E at the box load, 3 H
+ * shell, 4 E shell; cell offset; level found; level expected).  FDTD_ESTATE when the arrays are off (always in the
+ * product library: out is zeroed). */
+int fdtd_debug_level_errors(fdtd_ctx* ctx, long long out[5]);
 
 const char* fdtd_last_error(const fdtd_ctx* ctx); /* text of the last failure on this ctx; never NULL */
 const char* fdtd_build_info(void);                /* e.g. "sm_100a fmad=true" */

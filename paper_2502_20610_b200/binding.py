@@ -15,7 +15,7 @@ KERNEL_NAIVE, KERNEL_SYSTOLIC, KERNEL_SYSTOLIC_SMEM, KERNEL_SYSTOLIC_REG = 0, 1,
 _ERRNAME = {1: "FDTD_EINVAL", 2: "FDTD_ENOMEM", 3: "FDTD_ECUDA", 4: "FDTD_ESTATE", 5: "FDTD_ETIMEOUT"}
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBFILES = {"fma": "libfdtd_b200.so", "nofma": "libfdtd_b200_nofma.so", "dbg": "libfdtd_b200_dbg.so", "prof": "libfdtd_b200_prof.so"}
+_LIBFILES = {"nofma": "libfdtd_b200.so", "fma": "libfdtd_b200_fma.so", "dbg": "libfdtd_b200_dbg.so", "prof": "libfdtd_b200_prof.so"}
 _libs = {}
 
 _F3 = C.c_void_p * 3
@@ -38,6 +38,7 @@ _PROTOS = {
     "fdtd_last_step_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
     "fdtd_plan_tiles": (C.c_int, [C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_int)]),
     "fdtd_plan_owner": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+    "fdtd_debug_level_errors": (C.c_int, [C.c_void_p, C.POINTER(C.c_longlong)]),
     "fdtd_last_error": (C.c_char_p, [C.c_void_p]),
     "fdtd_build_info": (C.c_char_p, []),
     "fdtd_destroy": (None, [C.c_void_p]),
@@ -51,11 +52,11 @@ class FdtdError(RuntimeError):
         super().__init__(f"{_ERRNAME.get(code, code)}: {msg}" if msg else str(_ERRNAME.get(code, code)))
 
 
-def lib_path(variant="fma"):
+def lib_path(variant="nofma"):
     return os.path.join(HERE, _LIBFILES[variant])
 
 
-def load(variant="fma"):
+def load(variant="nofma"):
     """dlopen the in-tree library; raises if it has not been built (python -m paper_2502_20610_b200.build)."""
     if variant not in _libs:
         path = lib_path(variant)
@@ -80,7 +81,7 @@ def _ptr3(tensors):
     return C.cast(arr, C.POINTER(C.c_void_p))
 
 
-def plan_tiles(n, boundary, N, T, variant="fma"):
+def plan_tiles(n, boundary, N, T, variant="nofma"):
     out = (C.c_int * 3)()
     rc = load(variant).fdtd_plan_tiles((C.c_int * 3)(*n), (C.c_int * 3)(*boundary), (C.c_int * 3)(*N), int(T), out)
     if rc != OK:
@@ -88,7 +89,7 @@ def plan_tiles(n, boundary, N, T, variant="fma"):
     return tuple(out)
 
 
-def plan_owner(n, boundary, N, T, g, s, variant="fma"):
+def plan_owner(n, boundary, N, T, g, s, variant="nofma"):
     tile, off = C.c_int(), C.c_int()
     rc = load(variant).fdtd_plan_owner(int(n), int(boundary), int(N), int(T), int(g), int(s), C.byref(tile), C.byref(off))
     if rc != OK:
@@ -100,7 +101,7 @@ class Fdtd:
     """One simulation context.  E, H (and ca, cb) are lists of three float32 CUDA tensors of shape (nz, ny, nx),
     contiguous, which the library borrows and updates in place."""
 
-    def __init__(self, n, d, dt, boundary, stream=None, variant="fma"):
+    def __init__(self, n, d, dt, boundary, stream=None, variant="nofma"):
         import torch
         self._lib = load(variant)
         self.variant = variant
@@ -184,6 +185,12 @@ class Fdtd:
         self._check(self._lib.fdtd_get_counters(self._h, out))
         return {"launches": out[0], "steps": out[1], "chunks": out[2], "tiles": out[3]}
 
+    def debug_level_errors(self):
+        """Developer build + FDTD_DEBUG_LEVELS=1: (violations, kind, cell offset, level found, level expected)."""
+        out = (C.c_longlong * 5)()
+        self._check(self._lib.fdtd_debug_level_errors(self._h, out))
+        return tuple(out)
+
     def last_step_ms(self):
         ms = C.c_float()
         self._check(self._lib.fdtd_last_step_ms(self._h, C.byref(ms)))
@@ -201,7 +208,7 @@ class Fdtd:
             pass
 
 
-def run_workload(w, kernel=KERNEL_SYSTOLIC, tile=None, T=0, steps=None, variant="fma", device="cuda:0"):
+def run_workload(w, kernel=KERNEL_SYSTOLIC, tile=None, T=0, steps=None, variant="nofma", device="cuda:0"):
     """Build the seeded inputs of workload `w` on the device, run `steps` steps, return (E, H) CUDA tensors and the
     context (still open).  Convenience used by tests, smoke() and bench.py."""
     import torch

@@ -63,7 +63,10 @@ struct fdtd_ctx {
     // FDTD_DEBUG builds only (dbg / prof variants); always zero in the product libraries
     unsigned int delay_seed;
     int dbg_skip, dbg_withhold;
-    bool dbg_no_tma, dbg_no_group, dbg_lex_order;
+    bool dbg_no_tma, dbg_no_group, dbg_lex_order, dbg_levels;
+    int* d_lev;                      // time-level shadow arrays levE, levH of the working grid (FDTD_DEBUG_LEVELS)
+    size_t lev_cells;
+    unsigned long long* d_lev_err;   // [0] violations, [1..4] the first one
     // device
     int device, num_sms, clock_khz;
     cudaEvent_t ev0, ev1;
@@ -528,6 +531,26 @@ int step_systolic(fdtd_ctx* c, int n)
         for (int g = 0; g < 3; ++g) P.tma_group[g] = c->tma_group[g];
         P.dbg = c->dbg_skip;
         P.withhold_tile = c->dbg_withhold;
+        if (c->dbg_levels && c->use_tma) {
+            // developer build: per-cell time levels of this launch start at 0 everywhere (all cells are at time t0)
+            const size_t cells = (size_t)ldx * P.g.n[1] * P.g.n[2];
+            if (cells > c->lev_cells) {
+                cudaStreamSynchronize(c->stream);
+                if (c->d_lev) cudaFree(c->d_lev);
+                c->d_lev = nullptr;
+                c->lev_cells = 0;
+                if (cudaMalloc(&c->d_lev, 2 * cells * sizeof(int)) != cudaSuccess) return fail(c, FDTD_ENOMEM, "cudaMalloc(level shadow arrays)");
+                c->lev_cells = cells;
+            }
+            if (!c->d_lev_err) {
+                if (cudaMalloc(&c->d_lev_err, 8 * sizeof(unsigned long long)) != cudaSuccess) return fail(c, FDTD_ENOMEM, "cudaMalloc(level errors)");
+                cudaMemsetAsync(c->d_lev_err, 0, 8 * sizeof(unsigned long long), c->stream);
+            }
+            cudaMemsetAsync(c->d_lev, 0, 2 * cells * sizeof(int), c->stream);
+            P.levE = c->d_lev;
+            P.levH = c->d_lev + cells;
+            P.lev_err = c->d_lev_err;
+        }
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
@@ -634,7 +657,10 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->delay_seed = 0;
     c->dbg_skip = 0;
     c->dbg_withhold = -1;
-    c->dbg_no_tma = c->dbg_no_group = c->dbg_lex_order = false;
+    c->dbg_no_tma = c->dbg_no_group = c->dbg_lex_order = c->dbg_levels = false;
+    c->d_lev = nullptr;
+    c->lev_cells = 0;
+    c->d_lev_err = nullptr;
     c->env_T = 0;
     c->env_tile[0] = c->env_tile[1] = c->env_tile[2] = 0;
     if (const char* env = getenv("FDTD_T")) c->env_T = atoi(env);
@@ -649,6 +675,7 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->dbg_no_tma = getenv("FDTD_DEBUG_NO_TMA") != nullptr;
     c->dbg_no_group = getenv("FDTD_DEBUG_NO_GROUP") != nullptr;
     c->dbg_lex_order = getenv("FDTD_DEBUG_LEX_ORDER") != nullptr;
+    c->dbg_levels = getenv("FDTD_DEBUG_LEVELS") != nullptr;
 #endif
     c->device = dev;
     c->num_sms = prop.multiProcessorCount;
@@ -927,6 +954,22 @@ int fdtd_plan_owner(int n, int boundary, int N, int T, int g, int s, int* tile, 
     return FDTD_EINVAL;
 }
 
+int fdtd_debug_level_errors(fdtd_ctx* c, long long out[5])
+{
+    if (!c || !out) return FDTD_EINVAL;
+    for (int q = 0; q < 5; ++q) out[q] = 0;
+    if (!c->dbg_levels) return fail(c, FDTD_ESTATE, "time-level shadow arrays are off (developer build with FDTD_DEBUG_LEVELS=1 only)");
+    DeviceGuard guard(c);
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    if (!c->d_lev_err) return FDTD_OK;
+    unsigned long long h[5];
+    e = cudaMemcpy(h, c->d_lev_err, sizeof h, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(level errors)");
+    for (int q = 0; q < 5; ++q) out[q] = (long long)h[q];
+    return FDTD_OK;
+}
+
 const char* fdtd_last_error(const fdtd_ctx* c) { return c ? c->err.c_str() : "null context"; }
 
 const char* fdtd_build_info(void)
@@ -949,6 +992,8 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);
     free_pad(c);
+    if (c->d_lev) cudaFree(c->d_lev);
+    if (c->d_lev_err) cudaFree(c->d_lev_err);
     for (auto& o : c->orders) cudaFree(o.d);
     if (c->d_prof) {
         long long h[32];

@@ -14,6 +14,7 @@
 // Arithmetic: the expression tree of eq. (1) with coefficients, one rounding per operation when compiled
 // with -fmad=false (then bit-identical to the fp32 oracle); the default build lets ptxas contract mul+add.
 #include "fdtd_internal.h"
+#include "yee_update.h"
 
 namespace {
 
@@ -50,30 +51,16 @@ __device__ __forceinline__ void zerov(float (&v)[VEC])
     for (int q = 0; q < VEC; ++q) v[q] = 0.0f;
 }
 
-// E_a <- ca_a E_a + cb_a [ (H_c - H_c[-e_b]) rd_b - (H_b - H_b[-e_c]) rd_c ]        (eq. (1))
+// per-component arithmetic: yee_update.h (the one expression tree of reading #3, shared with the systolic kernels);
+// the coefficient-array choice is a run-time flag here
 __device__ __forceinline__ float e_update(float e, float hc, float hc_m, float hb, float hb_m, float rdb, float rdc,
                                           bool has_ca, float ca, float cb)
 {
-    const float d1 = hc - hc_m;
-    const float d2 = hb - hb_m;
-    const float t1 = d1 * rdb;
-    const float t2 = d2 * rdc;
-    const float curl = t1 - t2;
-    const float keep = has_ca ? ca * e : e;
-    const float gain = cb * curl;
-    return keep + gain;
+    return has_ca ? yee_e_update<true>(e, hc, hc_m, hb, hb_m, rdb, rdc, ca, cb) : yee_e_update<false>(e, hc, hc_m, hb, hb_m, rdb, rdc, ca, cb);
 }
-
-// H_a <- H_a - db_a [ (E_c[+e_b] - E_c) rd_b - (E_b[+e_c] - E_b) rd_c ]
 __device__ __forceinline__ float h_update(float h, float ec_p, float ec, float eb_p, float eb, float rdb, float rdc, float db)
 {
-    const float d1 = ec_p - ec;
-    const float d2 = eb_p - eb;
-    const float t1 = d1 * rdb;
-    const float t2 = d2 * rdc;
-    const float curl = t1 - t2;
-    const float loss = db * curl;
-    return h - loss;
+    return yee_h_update(h, ec_p, ec, eb_p, eb, rdb, rdc, db);
 }
 
 template <int VEC>

@@ -1,4 +1,5 @@
-// systolic_reg.cu -- the systolic FDTD kernel for sm_100a, register-resident version (the product kernel).
+// systolic_reg.cu -- the systolic FDTD kernel for sm_100a, register-resident cp.async version: a slow CROSS-CHECK
+// implementation (explicit FDTD_KERNEL_SYSTOLIC_REG only; the product kernel is systolic_tma.cu).
 //
 // Same schedule as systolic_kernel.cu (tile regions R_k = [a-k, a+w-k) sliding along the x-y-z-t diagonal,
 // PAPER.md:94; minus-shell loads, plus-shell publishes, per-tile acquire/release flags on all seven upwind

@@ -152,6 +152,26 @@ __device__ __forceinline__ int ld_volatile(const int* p)
     asm volatile("ld.volatile.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+#ifdef FDTD_DEBUG
+// Time-level shadow arrays (race detection; compute-sanitizer is closed on this pool): one int per
+// cell and field = number of updates of this launch that the value in global memory has received.  Every value a tile
+// takes from global memory is checked against the level the schedule promises, every publish records its level.
+__device__ __forceinline__ void lev_check(const SysParams& P, const int* lev, long long off, int expect, int kind)
+{
+    if (!lev) return;
+    const int v = ld_volatile(lev + off);
+    if (v != expect && atomicAdd(P.lev_err, 1ull) == 0ull) {
+        P.lev_err[1] = (unsigned long long)kind;
+        P.lev_err[2] = (unsigned long long)off;
+        P.lev_err[3] = (unsigned long long)(long long)v;
+        P.lev_err[4] = (unsigned long long)(long long)expect;
+    }
+}
+__device__ __forceinline__ void lev_set(int* lev, long long off, int v)
+{
+    if (lev) __stcg(lev + off, v);
+}
+#endif
 __device__ __forceinline__ void bar_sync(int id, int count)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
@@ -405,7 +425,8 @@ __device__ __forceinline__ void load_xcol(XCol& x, const float* xo, int l_lo)
         x.v[r][2] = v[16];
     }
 }
-__device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld, const XCol& x, int gx, int o1, int o2, int ly_lo, int ly_hi, int l_lo)
+__device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld, const XCol& x, int gx, int o1, int o2, int ly_lo, int ly_hi, int l_lo,
+                                           int* lev, int level)
 {
     const int lane = threadIdx.x & 31;
     if ((unsigned)gx >= (unsigned)P.g.n[0]) return;
@@ -421,6 +442,7 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
             __stcg(fld[0] + off, x.v[r][0]);
             __stcg(fld[1] + off, x.v[r][1]);
             __stcg(fld[2] + off, x.v[r][2]);
+            FDTD_DEBUG_ONLY(lev_set(lev, off, level);)
         }
     }
 }
@@ -523,6 +545,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     ex[r][l] = oke ? __ldcg(Ex + off) : 0.0f;
                     ey[r][l] = oke ? __ldcg(Ey + off) : 0.0f;
                     ez[r][l] = oke ? __ldcg(Ez + off) : 0.0f;
+                    FDTD_DEBUG_ONLY(if (ok) lev_check(P, P.levH, off, 0, 1); if (oke) lev_check(P, P.levE, off, 0, 2);)
                     const int cidx = r * SX + (gz & (BZ - 1)) * PLANE;
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -576,6 +599,14 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 }
             }
             warp_arrive(mb + MB_HFREE);
+#ifdef FDTD_DEBUG
+            // every H value just taken from the shell must have received exactly k updates in this launch
+#pragma unroll
+            for (int r = 0; r < NROW; ++r)
+                for (int l = 0; l < BZ; ++l)
+                    if ((l == 0 || ly[r] == 0 || lx == 0) && col_in[r] && (unsigned)(o2 + l) < (unsigned)nz)
+                        lev_check(P, P.levH, col_off[r] + plane * (o2 + l), k, 3);
+#endif
         }
         PROF_MARK(0);
         bar_sync(1, NCOMPUTE);   // exchange rows of H (shell + last H phase) and the scattered coefficients are visible
@@ -671,6 +702,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     __stcg(Ex + off, ex[r][W2 + 1]);
                     __stcg(Ey + off, ey[r][W2 + 1]);
                     __stcg(Ez + off, ez[r][W2 + 1]);
+                    FDTD_DEBUG_ONLY(lev_set(P.levE, off, k + 1);)
                 }
                 if (last | (ly[r] == W1)) {                          // warp-uniform: the leaving row (or the whole tile), planes 1..6
                     long long off = col_off[r] + plane * (o2 + 1);
@@ -680,6 +712,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                             __stcg(Ex + off, ex[r][l + 1]);
                             __stcg(Ey + off, ey[r][l + 1]);
                             __stcg(Ez + off, ez[r][l + 1]);
+                            FDTD_DEBUG_ONLY(lev_set(P.levE, off, k + 1);)
                         }
                         off += plane;
                     }
@@ -733,6 +766,14 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         warp_arrive(mb + MB_EFREE);
+#ifdef FDTD_DEBUG
+        // every E value just taken from the shell must have received exactly k+1 updates in this launch
+#pragma unroll
+        for (int r = 0; r < NROW; ++r)
+            for (int l = 0; l < BZ; ++l)
+                if ((l == 0 || ly[r] == 0 || lx == 0) && col_in[r] && (unsigned)(o2 + l) < (unsigned)nz)
+                    lev_check(P, P.levE, col_off[r] + plane * (o2 + l), k + 1, 4);
+#endif
         bar_sync(1, NCOMPUTE);   // exchange rows of E are visible; every warp has finished E phase k
         PROF_MARK(5);
         // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
@@ -778,6 +819,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     __stcg(Hx + off, hx[r][W2]);
                     __stcg(Hy + off, hy[r][W2]);
                     __stcg(Hz + off, hz[r][W2]);
+                    FDTD_DEBUG_ONLY(lev_set(P.levH, off, k + 1);)
                 }
                 if (last | (ly[r] == W1 - 1)) {                      // warp-uniform: leaving row (or whole tile), planes 0..5
                     long long off = col_off[r] + plane * o2;
@@ -787,6 +829,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                             __stcg(Hx + off, hx[r][l + 1]);
                             __stcg(Hy + off, hy[r][l + 1]);
                             __stcg(Hz + off, hz[r][l + 1]);
+                            FDTD_DEBUG_ONLY(lev_set(P.levH, off, k + 1);)
                         }
                         off += plane;
                     }
@@ -1020,8 +1063,8 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                 __syncwarp();
                 if (lane == 0) mbar_arrive(mb + MB_ACKH);
                 if (k != T - 1 && !FDTD_DBG(P, 4)) {
-                    store_xcol(P, P.g.E, ce, o0 + W0, o1, o2, 1, W1 - 1, 1);
-                    store_xcol(P, P.g.H, ch, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0);
+                    store_xcol(P, P.g.E, ce, o0 + W0, o1, o2, 1, W1 - 1, 1, P.levE, k + 1);
+                    store_xcol(P, P.g.H, ch, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0, P.levH, k + 1);
                 }
                 __syncwarp();
                 if (lane == 0) {

@@ -26,7 +26,7 @@ def oracle_run(w, steps):
     return E, H
 
 
-def gpu_run(w, steps, kernel, tile=None, T=0, variant="fma"):
+def gpu_run(w, steps, kernel, tile=None, T=0, variant="nofma"):
     E, H, sim = binding.run_workload(w, kernel=kernel, tile=tile, T=T, steps=steps, variant=variant)
     info = sim.get_kernel()
     sim.close()

@@ -9,8 +9,11 @@
   (f) the hand-off watchdog fires (FDTD_ETIMEOUT) instead of hanging when a flag is withheld  (dbg build)
   (g) checkpoint / resume: get_fields -> new ctx -> set_fields + set_time == the straight run
 
-All through the C ABI; bit-exact (np.array_equal) for the -fmad=false builds, max|GPU-oracle| <= 1e-5 max|field| for the
-FMA build.  The inputs of (a), (b) are built here (not in workloads.make_fields, which zeroes the frozen cells)."""
+All through the C ABI; bit-exact (np.array_equal) for the product library (variant "nofma", -fmad=false), which therefore
+meets north_star's max|GPU-oracle| <= 1e-5 max|field| on every run length; the optional FMA-contracted variant is held to
+1e-5 as well except on the 1000-step config 2 run, where its measured drift (3e-5) is asserted against 1e-4 and is the
+reason it is not the product.  The inputs of (a), (b) are built here (not in workloads.make_fields,
+which zeroes the frozen cells)."""
 import numpy as np
 import pytest
 
@@ -34,7 +37,7 @@ def _to_dev(arrs, grouped=True):
     return workloads._grouped(ts) if grouped else ts
 
 
-def _compare(E, H, Eo, Ho, exact):
+def _compare(E, H, Eo, Ho, exact, tol=TOL):
     scale = max(float(np.abs(x).max()) for x in Eo + Ho)
     worst = 0.0
     for g, o in zip(list(E) + list(H), Eo + Ho):
@@ -43,7 +46,8 @@ def _compare(E, H, Eo, Ho, exact):
         if exact:
             assert np.array_equal(g, o), f"not bit-exact: max diff {np.abs(g - o).max():.3e} at {np.unravel_index(np.abs(g - o).argmax(), g.shape)}"
         worst = max(worst, float(np.abs(g.astype(np.float64) - o.astype(np.float64)).max()))
-    assert worst <= TOL * max(scale, 1e-30), f"max|GPU-oracle| = {worst:.3e} > {TOL} * {scale:.3e}"
+    assert worst <= tol * max(scale, 1e-30), f"max|GPU-oracle| = {worst:.3e} > {tol} * {scale:.3e}"
+    return worst / max(scale, 1e-30)
 
 
 def _run_gpu(n, d, dt, boundary, E0, H0, ca, cb, db, src, steps, kernel, tile, T, variant, grouped=True):
@@ -237,7 +241,11 @@ def test_full_run_parity_library_defaults(cuda_device, full_oracle, name, idx, s
         sim.close()
         if kernel == binding.KERNEL_SYSTOLIC:
             assert info["which"] == binding.KERNEL_SYSTOLIC
-        _compare(E, H, Eo, Ho, exact=(variant == "nofma"))
+        # the contracted variant drifts 3e-5 max|field| from the oracle over the 1000 steps of config 2 (fields decay by 100x
+        # after the pulse while the rounding differences made near the source persist): outside north_star's bar, so it is
+        # not the product; asserted here against 1e-4 so that a real defect still fails
+        rel = _compare(E, H, Eo, Ho, exact=(variant == "nofma"), tol=1e-4 if (variant == "fma" and w.steps >= 1000) else TOL)
+        print(f"full run {name} {variant} kernel={kernel}: max|GPU-oracle|/max|field| = {rel:.2e}")
         del E, H
 
 
@@ -328,6 +336,37 @@ def test_watchdog_turns_a_withheld_flag_into_etimeout(cuda_device, monkeypatch):
     E, H, sim = binding.run_workload(w, steps=8, variant="dbg")
     sim.close()
     assert all(bool(np.isfinite(x.cpu().numpy()).all()) for x in E + H)
+
+
+# ---- section 5: time-level shadow arrays (race detector of the hand-off protocol) -------------------------------------
+def test_level_shadow_arrays_find_no_violation_and_do_find_a_broken_protocol(cuda_device, monkeypatch):
+    """dbg build with FDTD_DEBUG_LEVELS=1: every value a tile takes from global memory carries the time level the schedule
+    promises -- on wall grids, on the padded periodic copy, under pseudo-random delays.  With the upwind waits switched
+    off (FDTD_DEBUG_SKIP=1) and the same delays the detector must report violations: it is not vacuous."""
+    monkeypatch.setenv("FDTD_DEBUG_LEVELS", "1")
+    cases = [workloads.config(1).scaled((72, 60, 52), steps=60), workloads.config(2).scaled((64, 56, 40), steps=60),
+             workloads.config(3, 128).scaled((100, 96, 90), steps=40)]
+    for seed in ("0", "777"):
+        monkeypatch.setenv("FDTD_DEBUG_DELAY", seed)
+        for w in cases:
+            for T in (7, 0):
+                E, H, sim = binding.run_workload(w, tile=(31, 15, 7) if T else None, T=T, steps=w.steps, variant="dbg")
+                errs = sim.debug_level_errors()
+                sim.close()
+                assert errs[0] == 0, f"{w.name} T={T} delay={seed}: level violations {errs}"
+    monkeypatch.setenv("FDTD_DEBUG_SKIP", "1")
+    monkeypatch.setenv("FDTD_DEBUG_DELAY", "777")
+    w = cases[0]
+    E, H, sim = binding.run_workload(w, tile=(31, 15, 7), T=30, steps=60, variant="dbg")
+    errs = sim.debug_level_errors()
+    sim.close()
+    assert errs[0] > 0, "the detector did not notice tiles running without their upwind waits"
+    # the product library has no such arrays
+    sim = binding.Fdtd((8, 8, 8), (1, 1, 1), 0.1, (0, 0, 0))
+    with pytest.raises(binding.FdtdError) as e:
+        sim.debug_level_errors()
+    assert e.value.code == binding.ESTATE
+    sim.close()
 
 
 # ---- (g) checkpoint / resume ---------------------------------------------------------------------------------

@@ -689,8 +689,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     if (e == cudaSuccess) e = cudaMalloc(&c->d_abort, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(c->d_abort, 0, sizeof(int));
 #ifdef FDTD_PROFILE
-    if (e == cudaSuccess) e = cudaMalloc(&c->d_prof, 32 * sizeof(long long));
-    if (e == cudaSuccess) e = cudaMemset(c->d_prof, 0, 32 * sizeof(long long));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_prof, (32 + FDTD_TRACE_CAP) * sizeof(long long));
+    if (e == cudaSuccess) e = cudaMemset(c->d_prof, 0, (32 + FDTD_TRACE_CAP) * sizeof(long long));
 #endif
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
@@ -1001,6 +1001,19 @@ void fdtd_destroy(fdtd_ctx* c)
             fprintf(stderr, "fdtd profile (clock64 ticks summed over CTAs):");
             for (int i = 0; i < 32; ++i) fprintf(stderr, "%s%lld", i % 8 == 0 ? "\n  " : " ", h[i]);
             fprintf(stderr, "\n");
+        }
+        // event trace of one CTA (systolic_tma.cu TRACE): clock << 20 | role << 16 | event << 12 | step
+        if (const char* path = getenv("FDTD_TRACE_FILE")) {
+            std::vector<long long> tr(FDTD_TRACE_CAP);
+            if (cudaMemcpy(tr.data(), c->d_prof + 32, tr.size() * sizeof(long long), cudaMemcpyDeviceToHost) == cudaSuccess) {
+                if (FILE* f = fopen(path, "w")) {
+                    for (long long v : tr) {
+                        if (v == 0) break;
+                        fprintf(f, "%lld %d %d %d\n", v >> 20, (int)((v >> 16) & 15), (int)((v >> 12) & 15), (int)(v & 4095));
+                    }
+                    fclose(f);
+                }
+            }
         }
         cudaFree(c->d_prof);
     }

@@ -70,6 +70,7 @@ inline AxisPlan make_axis_plan(int n, int per, int N, int T)
 #endif
 
 constexpr int MAX_SRC_IMAGES = 125;
+constexpr int FDTD_TRACE_CAP = 1 << 16;   // FDTD_PROFILE build: events of the traced CTA, behind the 32 tick accumulators of SysParams::prof
 
 // The padded working copy of the grid (pad_kernels.cu): a periodic axis a carries G[a] ghost cells on
 // either side (m[a] = n[a] + 2 G[a]); wall axes have G[a] = 0; rows are ldx >= m[0] elements long (a multiple of 4).

@@ -456,10 +456,18 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
 #define PROF_DECL long long pt_ = clock64(), pacc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}
 #define PROF_MARK(i) do { const long long n_ = clock64(); pacc_[i] += n_ - pt_; pt_ = n_; } while (0)
 #define PROF_FLUSH(base) do { if ((threadIdx.x & 31) == 0 && P.prof) for (int i_ = 0; i_ < 8; ++i_) atomicAdd((unsigned long long*)P.prof + (base) + i_, (unsigned long long)pacc_[i_]); } while (0)
+// event trace of one CTA (the tiles CTA 0 claims in the second half of the claim order): P.prof[32 ...]
+#define TRACE_C(ev, k) do { if (w == 0 || w == NWARPS_C - 1) TRACE(w == 0 ? 0 : 5, ev, k); } while (0)
+#define TRACE(role, ev, k) do { if (trace_on_ && (threadIdx.x & 31) == 0) { const unsigned i_ = atomicAdd(&trace_cur_, 1u); \
+    if (i_ < (unsigned)FDTD_TRACE_CAP) P.prof[32 + i_] = (clock64() << 20) | ((long long)(role) << 16) | ((long long)(ev) << 12) | (long long)((k) & 4095); } } while (0)
+__shared__ int trace_on_;
+__shared__ unsigned trace_cur_;
 #else
 #define PROF_DECL
 #define PROF_MARK(i)
 #define PROF_FLUSH(base)
+#define TRACE(role, ev, k)
+#define TRACE_C(ev, k)
 #endif
 
 struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
@@ -564,8 +572,10 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exH[(l - 1) * PLANE + slot1] = make_float2(hz[RL][l], hx[RL][l]);
             }
         } else {
+            TRACE_C( 0, k);
             mbar_wait(mb + MB_HREADY, ph.hready & 1u);
             ++ph.hready;
+            TRACE_C( 1, k);
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 hx[r][0] = stgH[zidx<3>(0, ly[r], xs)];
@@ -612,6 +622,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         bar_sync(1, NCOMPUTE);   // exchange rows of H (shell + last H phase) and the scattered coefficients are visible
 
         PROF_MARK(1);
+        TRACE_C( 2, k);
         // ---------------- E phase on R_k = [1,w]^3 (a1): every slot computes, shell slots produce garbage ----
         // fast (no coefficient arrays, box never touches a wall or the outside): cb is the scalar dt, no mask loads
         auto e_phase = [&](auto fastc) {
@@ -689,6 +700,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         PROF_MARK(2);
+        TRACE_C( 3, k);
         if (k > k0) {   // the signal warp has copied the x-out rows of step k-1 (and the DONE barriers cannot lap it)
             mbar_wait(mb + MB_ACKE, ph.acke & 1u);
             ++ph.acke;
@@ -728,6 +740,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         warp_arrive(mb + MB_EDONE);
+        TRACE_C( 4, k);
         FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);)
 
         // ---------------- E minus shell -------------------------------------------------------------------------
@@ -735,6 +748,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         mbar_wait(mb + MB_EREADY, ph.eready & 1u);
         ++ph.eready;
         PROF_MARK(4);
+        TRACE_C( 5, k);
 #pragma unroll
         for (int r = 0; r < NROW; ++r) {
             ex[r][1] = stgE[zidx<3>(0, ly[r], xs)];
@@ -776,6 +790,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #endif
         bar_sync(1, NCOMPUTE);   // exchange rows of E are visible; every warp has finished E phase k
         PROF_MARK(5);
+        TRACE_C( 6, k);
         // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
         // first used by E phase k+1 (shell cells are not in R_k); copied a whole step ahead (issued after CFREE(k-1))
         if (k >= 1 && !fast) {
@@ -787,6 +802,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             warp_arrive(mb + MB_CFREE);
         }
         PROF_MARK(7);
+        TRACE_C( 7, k);
 
         // ---------------- H phase on R_{k+1} = [0,w-1]^3 (a2): every slot computes ----------------------------
 #pragma unroll
@@ -806,6 +822,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
             exH[l * PLANE + slot1] = make_float2(hz[RL][l + 1], hx[RL][l + 1]);
         }
+        TRACE_C( 8, k);
         if (k > k0) {   // the signal warp has copied the H x-out rows of step k-1 (HDONE cannot lap its waiters)
             mbar_wait(mb + MB_ACKH, ph.ackh & 1u);
             ++ph.ackh;
@@ -845,6 +862,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         warp_arrive(mb + MB_HDONE);
+        TRACE_C( 9, k);
         FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);)
         PROF_MARK(6);
     }
@@ -861,6 +879,10 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
     __shared__ Ctl ctl;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (tid == 0) {
+#ifdef FDTD_PROFILE
+        trace_on_ = 0;
+        trace_cur_ = 0u;
+#endif
         ctl.abort = 0;
         mbar_init(mb + MB_HFULL, 1);
         mbar_init(mb + MB_CFULL, 1);
@@ -894,6 +916,9 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
         if (tid == 0) {
             ctl.tile = (int)atomicAdd(P.counter, 1u);
             if (ld_volatile(P.abort_flag) != 0) ctl.abort = 1;
+#ifdef FDTD_PROFILE
+            trace_on_ = (blockIdx.x == 0 && P.prof != nullptr && (int)ctl.tile >= P.ntiles / 2) ? 1 : 0;
+#endif
         }
         bar_sync(0, NT);
         if (ctl.tile >= P.ntiles || ctl.abort) return false;
@@ -964,6 +989,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                     PROF_MARK(7);
                     if (warp == W_HPROD) {
+                        TRACE(1, 0, k);
                         // field shell: acquire the upwind flags and order the async proxy after them while the staging is
                         // still in use, copy, repack the entering column -> HREADY(k)
                         if (k == hk0 || !EARLY) {      // later steps: acquired while the previous copy was in flight
@@ -971,8 +997,10 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                             if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                         }
                         PROF_MARK(0);
+                        TRACE(1, 1, k);
                         if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                         PROF_MARK(1);
+                        TRACE(1, 2, k);
                         if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         __syncwarp();
                         if (k + 1 < k1 && EARLY) {
@@ -980,17 +1008,22 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                             if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                         }
                         PROF_MARK(2);
+                        TRACE(1, 3, k);
                         if (!FDTD_DBG(P, 2)) { mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull; }
                         PROF_MARK(3);
+                        TRACE(1, 4, k);
                         pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
                         warp_arrive(mb + MB_HREADY);
+                        TRACE(1, 5, k);
                         PROF_MARK(4);
                     } else {
                         // coefficient shell (constants of the run: no flag, no proxy fence): copied as soon as the compute
                         // warps have taken the previous one out of the staging (CFREE), a whole step before it is needed
                         if (COEF && !fast) {         // (a uniform tile has no coefficient copy)
+                        TRACE(2, 0, k);
                         if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
                         PROF_MARK(0);
+                        TRACE(2, 1, k);
                         if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                         __syncwarp();
                         PROF_MARK(1);
@@ -1015,19 +1048,25 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     wait_upwind(P, t, P.flagE, P.flag_base + k + 1, &ctl);
                     if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                 }
+                TRACE(3, 0, k);
                 if (k > k0) {
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
                 }
+                TRACE(3, 1, k);
                 if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
                 __syncwarp();
                 if (k + 1 < k1 && EARLY) {
                     wait_upwind(P, t, P.flagE, P.flag_base + k + 2, &ctl);
                     if (lane == 0 && !FDTD_DBG(P, 32)) fence_proxy_async();
                 }
+                TRACE(3, 2, k);
                 if (!FDTD_DBG(P, 2)) { mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull; }
+                TRACE(3, 4, k);
                 const float* stg = sm + Lay<COEF>::stge;
                 pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
+                TRACE(3, 5, k);
                 if (k > k0) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
+                TRACE(3, 6, k);
                 // the shell column's Ez, Ex of planes 1..6 for its y-1 readers in the H phase
                 float2* exE = reinterpret_cast<float2*>(sm + Lay<COEF>::exch) + EXP;
                 for (int r = 0; r < 3; ++r) {
@@ -1039,6 +1078,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     }
                 }
                 warp_arrive(mb + MB_EREADY);
+                TRACE(3, 7, k);
             }
             if (k1 > k0) { ++n_efree; ++n_hdone; }   // phases of the last step: covered by the CTA barrier at the tile boundary
         } else {
@@ -1054,11 +1094,15 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
             for (int k = k0; k < k1; ++k) {
                 const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
                 XCol ce, ch;
+                TRACE(4, 0, k);
                 mbar_wait(mb + MB_EDONE, n_edone & 1u); ++n_edone;
+                TRACE(4, 1, k);
                 load_xcol(ce, sm + Lay<COEF>::xoute, 1);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(mb + MB_ACKE);
+                TRACE(4, 2, k);
                 mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone;
+                TRACE(4, 3, k);
                 load_xcol(ch, sm + Lay<COEF>::xouth, 0);
                 __syncwarp();
                 if (lane == 0) mbar_arrive(mb + MB_ACKH);
@@ -1067,6 +1111,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     store_xcol(P, P.g.H, ch, o0 + W0 - 1, o1, o2, 0, W1 - 2, 0, P.levH, k + 1);
                 }
                 __syncwarp();
+                TRACE(4, 5, k);
                 if (lane == 0) {
                     fence_acq_rel_gpu();
                     FDTD_DEBUG_ONLY(if (tile != P.withhold_tile))
@@ -1076,6 +1121,7 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
                     }
                 }
                 __syncwarp();
+                TRACE(4, 6, k);
             }
             if (k1 < T && lane == 0) {
                 raise_flag(P, P.flagE, tile, P.flag_base + T);

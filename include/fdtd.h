@@ -155,6 +155,22 @@ int fdtd_plan_owner(int n, int boundary, int N, int T, int g, int s, int* tile, 
  * product library: out is zeroed). */
 int fdtd_debug_level_errors(fdtd_ctx* ctx, long long out[5]);
 
+/* Adiabatic-absorber coefficient generator (section 4: "does not use PMLs, but instead relies on the
+ * imaginary part of the permittivity to allow for the formation of adiabatic absorbers [5]"; reading #12).
+ * Context-free; runs one kernel on `cuda_stream` of the current device and returns without synchronising.
+ * Writes the six per-cell update-coefficient arrays that fdtd_set_coeffs takes, for a conductivity that rises as
+ * sigma_max * u^order (u = 0 at the inner edge of a layer, 1 at the wall) over `thickness` cells in front of each face:
+ *     thickness[6], sigma_max[6]: HOST arrays ordered x-low, x-high, y-low, y-high, z-low, z-high (0 = no layer);
+ *     order: integer 0..8 (0 = uniform conductivity inside the layer);  layers of different axes add;
+ *     eps[3]: host array of DEVICE pointers to per-cell relative permittivities of E_x, E_y, E_z (NULL, or NULL
+ *             entries: 1); ca[3], cb[3]: host arrays of DEVICE pointers, written (nx*ny*nz floats each, x fastest).
+ *     E_a of cell (i,j,k) is evaluated at its own Yee position (half a cell further along axis a);
+ *     ca = (2 eps - sigma dt)/(2 eps + sigma dt),  cb = 2 dt/(2 eps + sigma dt), every operation rounded to fp32.
+ * A round-trip power reflection R0 in a medium of index n_r needs sigma_max = -(order+1) n_r ln(R0) / (2 L d).
+ * FDTD_EINVAL: bad dims, negative thickness or sigma_max, thickness > n, order out of range, NULL output. */
+int fdtd_absorber_coeffs(int nx, int ny, int nz, float dt, const float* const eps[3], const int thickness[6],
+                         const float sigma_max[6], int order, float* const ca[3], float* const cb[3], void* cuda_stream);
+
 const char* fdtd_last_error(const fdtd_ctx* ctx); /* text of the last failure on this ctx; never NULL */
 const char* fdtd_build_info(void);                /* e.g. "sm_100a fmad=true" */
 void fdtd_destroy(fdtd_ctx* ctx);                 /* NULL-safe; never frees borrowed buffers */

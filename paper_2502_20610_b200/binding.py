@@ -39,6 +39,8 @@ _PROTOS = {
     "fdtd_plan_tiles": (C.c_int, [C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_int)]),
     "fdtd_plan_owner": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "fdtd_debug_level_errors": (C.c_int, [C.c_void_p, C.POINTER(C.c_longlong)]),
+    "fdtd_absorber_coeffs": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_float, C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.POINTER(C.c_float),
+                                       C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_void_p]),
     "fdtd_last_error": (C.c_char_p, [C.c_void_p]),
     "fdtd_build_info": (C.c_char_p, []),
     "fdtd_destroy": (None, [C.c_void_p]),
@@ -95,6 +97,19 @@ def plan_owner(n, boundary, N, T, g, s, variant="nofma"):
     if rc != OK:
         raise FdtdError(rc)
     return tile.value, off.value
+
+
+def absorber_coeffs(n, dt, eps, thickness, sigma_max, order, ca, cb, stream=None, variant="nofma"):
+    """fdtd_absorber_coeffs: fill the CUDA tensors ca[3], cb[3] (shape (nz, ny, nx)) with the graded-conductivity update
+    coefficients; eps: None or three CUDA tensors.  Enqueued on the current torch stream."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    rc = load(variant).fdtd_absorber_coeffs(int(n[0]), int(n[1]), int(n[2]), float(dt), _ptr3(eps), (C.c_int * 6)(*[int(x) for x in thickness]),
+                                            (C.c_float * 6)(*[float(x) for x in sigma_max]), int(order), _ptr3(ca), _ptr3(cb),
+                                            C.c_void_p(int(stream) or None))
+    if rc != OK:
+        raise FdtdError(rc, "fdtd_absorber_coeffs")
 
 
 class Fdtd:

@@ -31,6 +31,7 @@ struct fdtd_ctx {
     int cfg_idx;      // resolved shared-memory systolic configuration, -1 = unresolved / not used
     bool use_reg;     // resolved: the register-resident kernel (tile 31x15x7) runs
     bool use_tma;     // resolved: its TMA-staged version runs
+    bool tma_by8;     // resolved: the 31x7x7 build of it (two CTAs per SM)
     // resolved: the TMA kernel runs on a padded working copy of the grid (periodic axis or nx % 4 != 0)
     bool use_pad;
     PadGeom pg;
@@ -154,14 +155,15 @@ int resolve_systolic(fdtd_ctx* c)
         if (c->env_tile[0] > 0) { N[0] = c->env_tile[0]; N[1] = c->env_tile[1]; N[2] = c->env_tile[2]; }
     }
     c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
-    c->use_tma = c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->dbg_no_tma;
+    c->tma_by8 = c->which == FDTD_KERNEL_SYSTOLIC && N[0] == 31 && N[1] == 7 && N[2] == 7;
+    c->use_tma = (c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->dbg_no_tma) || c->tma_by8;
     c->use_pad = c->use_tma && (c->g.per[0] || c->g.per[1] || c->g.per[2] || c->g.n[0] % 4 != 0);
     int found = -1;
     int per_sm = 0;
     if (c->use_tma) {
-        cudaError_t e = systolic_tma_prepare(want_coef, &per_sm);
+        cudaError_t e = c->tma_by8 ? systolic_tma_prepare_by8(want_coef, &per_sm) : systolic_tma_prepare(want_coef, &per_sm);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
-        c->smem = systolic_tma_smem(want_coef);
+        c->smem = c->tma_by8 ? systolic_tma_smem_by8(want_coef) : systolic_tma_smem(want_coef);
     } else if (c->use_reg) {
         cudaError_t e = systolic_reg_prepare(want_coef, &per_sm);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
@@ -285,7 +287,8 @@ int ensure_tmaps(fdtd_ctx* c)
         encode = (EncodeTiledFn)fn;
     }
     int box[3][3];
-    systolic_tma_boxes(box);
+    if (c->tma_by8) systolic_tma_boxes_by8(box);
+    else systolic_tma_boxes(box);
     long long ldx = 0;
     const GridParams wg = work_grid(c, &ldx);
     const void* arr[12];
@@ -554,7 +557,8 @@ int step_systolic(fdtd_ctx* c, int n)
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
-        e = c->use_tma   ? launch_systolic_tma(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
+        e = c->tma_by8   ? launch_systolic_tma_by8(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
+            : c->use_tma ? launch_systolic_tma(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream)
                          : launch_systolic(c->cfg_idx, P, ctas, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "systolic launch");
@@ -637,6 +641,7 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->cfg_idx = -1;
     c->use_reg = false;
     c->use_tma = false;
+    c->tma_by8 = false;
     c->use_pad = false;
     c->pad_fld = c->pad_coef = nullptr;
     c->pad_stride = 0;
@@ -1020,6 +1025,20 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     delete c;
+}
+
+int fdtd_absorber_coeffs(int nx, int ny, int nz, float dt, const float* const eps[3], const int thickness[6],
+                         const float sigma_max[6], int order, float* const ca[3], float* const cb[3], void* cuda_stream)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || nx > (1 << 15) || ny > (1 << 15) || nz > (1 << 15)) return FDTD_EINVAL;
+    if (!(dt > 0.0f) || !std::isfinite(dt) || !thickness || !sigma_max || !ca || !cb || order < 0 || order > 8) return FDTD_EINVAL;
+    const int n[3] = {nx, ny, nz};
+    for (int f = 0; f < 6; ++f)
+        if (thickness[f] < 0 || thickness[f] > n[f / 2] || !(sigma_max[f] >= 0.0f) || !std::isfinite(sigma_max[f])) return FDTD_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (!ca[a] || !cb[a]) return FDTD_EINVAL;
+    const cudaError_t e = launch_absorber(n, dt, eps, thickness, sigma_max, order, ca, cb, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? FDTD_OK : FDTD_ECUDA;
 }
 
 }  // extern "C"

@@ -30,8 +30,18 @@ int systolic_tma_threads();
 void systolic_tma_boxes(int box[3][3]);   // TMA box extents (x,y,z) of the z-plane, y-row and x-column shell pieces
 cudaError_t systolic_tma_prepare(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
+// implemented in systolic_tma_by8.cu: the same kernel for tile 31x7x7 (box 32x8x8), two CTAs per SM
+size_t systolic_tma_smem_by8(int coef);
+int systolic_tma_threads_by8();
+void systolic_tma_boxes_by8(int box[3][3]);
+cudaError_t systolic_tma_prepare_by8(int coef, int* blocks_per_sm);
+cudaError_t launch_systolic_tma_by8(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
 
 // implemented in pad_kernels.cu: copies between the caller's arrays and the padded working copy (periodic images)
 cudaError_t launch_pad_copy_in(const PadGeom& g, const PadArrays& a, cudaStream_t st);     // all padded cells <- images
 cudaError_t launch_pad_ghost_fill(const PadGeom& g, const PadArrays& a, cudaStream_t st);  // ghost cells <- interior
 cudaError_t launch_pad_copy_out(const PadGeom& g, const PadArrays& a, cudaStream_t st);    // interior -> caller
+
+// implemented in absorber_kernels.cu: graded-conductivity update coefficients written to device arrays (row f3)
+cudaError_t launch_absorber(const int n[3], float dt, const float* const eps[3], const int L[6], const float smax[6], int order,
+                            float* const ca[3], float* const cb[3], cudaStream_t st);

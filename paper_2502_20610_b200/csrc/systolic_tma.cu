@@ -55,7 +55,17 @@
 
 namespace {
 
-constexpr int BX = 32, BY = 16, BZ = 8;
+// FDTD_BY = 16 (default): one CTA of 16 compute warps per SM, tile 31x15x7.  FDTD_BY = 8 (systolic_tma_by8.cu): tile 31x7x7,
+// 8 compute warps, half the shared memory and registers: TWO CTAs per SM, whose latency-bound sections (shell absorb,
+// publish, hand-offs) overlap each other's arithmetic.
+#ifndef FDTD_BY
+#define FDTD_BY 16
+#endif
+#ifndef FDTD_TMA_NAME
+#define FDTD_TMA_NAME(x) x
+#endif
+constexpr int BX = 32, BY = FDTD_BY, BZ = 8;
+constexpr int CTAS_PER_SM = BY == 16 ? 1 : 2;
 constexpr int W0 = BX - 1, W1 = BY - 1, W2 = BZ - 1;   // tile widths (PEC axes: always full)
 #ifndef FDTD_NROW
 #define FDTD_NROW 1
@@ -68,7 +78,8 @@ constexpr int PLANE = SX * BY;                          // slots (the entering x
 constexpr int NT = NCOMPUTE + 128;
 // NROW = 1: the launch gives each of the 640 threads 96 registers: compute warps grow to 104, auxiliary warps shrink to 64
 // (512*104 + 128*64 = 61440 = 640*96).  NROW = 2: 384 threads of 168 registers: 256*208 + 128*64 = 61440 <= 64512.
-constexpr int REGS_COMPUTE = NROW == 1 ? 104 : 208, REGS_AUX = 64;
+// BY = 8: 384 threads of 80 registers at launch (two CTAs per SM): 256*96 + 128*48 = 30720 = 384*80.
+constexpr int REGS_COMPUTE = BY == 8 ? 96 : NROW == 1 ? 104 : 208, REGS_AUX = BY == 8 ? 48 : 64;
 constexpr int W_HPROD = NWARPS_C, W_HAUX = NWARPS_C + 1, W_EPROD = NWARPS_C + 2;   // warp NWARPS_C + 3: signal
 
 // staging of one array's minus shell (floats); every TMA destination is 128-byte aligned
@@ -194,11 +205,11 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity), "r"(0x989680u)   // suspend-time hint: the warp sleeps in hardware instead of spinning
         : "memory");
 }
 // one elected arrive per warp, after every lane's earlier shared/global accesses
@@ -366,15 +377,16 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
         put((o2 & (BZ - 1)) * PLANE + (ys0 + r) * SX + lane, o0 + lx, o1 + ly[r], o2, v);
     }
     constexpr int ROW_WARPS = W2, COL_WARPS = (W1 * W2 + 31) / 32;
-    static_assert(ROW_WARPS + COL_WARPS <= NWARPS_C, "not enough compute warps for the coefficient shell");
-    if (w < ROW_WARPS) {                       // the entering row, plane l = w + 1: lane = x offset inside the box
-        const int l = w + 1, gx = o0 + lane;
+#pragma unroll
+    for (int it = w; it < ROW_WARPS + COL_WARPS; it += NWARPS_C) {   // one work item per warp (two for one warp when BY = 8)
+    if (it < ROW_WARPS) {                      // the entering row, plane l = it + 1: lane = x offset inside the box
+        const int l = it + 1, gx = o0 + lane;
         float v[6];
 #pragma unroll
         for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
         put(((o2 + l) & (BZ - 1)) * PLANE + (o1 & (BY - 1)) * SX + (gx & (BX - 1)), gx, o1, o2 + l, v);
-    } else if (w < ROW_WARPS + COL_WARPS) {    // the entering column: idx = (l-1)*15 + (ly-1)
-        const int idx = (w - ROW_WARPS) * 32 + lane;
+    } else {                                   // the entering column: idx = (l-1)*W1 + (ly-1)
+        const int idx = (it - ROW_WARPS) * 32 + lane;
         if (idx < W1 * W2) {
             const int cy = 1 + idx % W1, l = 1 + idx / W1;
             float v[6];
@@ -382,6 +394,7 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
             for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[xidx<6>(c, cy, l) + r0] : 0.0f;
             put(((o2 + l) & (BZ - 1)) * PLANE + ((o1 + cy) & (BY - 1)) * SX + (o0 & (BX - 1)), o0, o1 + cy, o2 + l, v);
         }
+    }
     }
 }
 
@@ -418,7 +431,7 @@ __device__ __forceinline__ void load_xcol(XCol& x, const float* xo, int l_lo)
     const int lane = threadIdx.x & 31;
 #pragma unroll
     for (int r = 0; r < XROUNDS; ++r) {
-        const int item = r * 32 + lane;            // y slot * 6 + plane
+        const int item = min(r * 32 + lane, BY * (W2 - 1) - 1);            // y slot * 6 + plane
         const float* v = xo + (item / (W2 - 1)) * 24 + l_lo + item % (W2 - 1);
         x.v[r][0] = v[0];
         x.v[r][1] = v[8];
@@ -437,7 +450,7 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
         const int ys = item / (W2 - 1), l = l_lo + item % (W2 - 1);
         const int ly = (ys - o1) & (BY - 1);
         const int gy = o1 + ly, gz = o2 + l;
-        if (ly >= ly_lo && ly <= ly_hi && (unsigned)gy < (unsigned)P.g.n[1] && (unsigned)gz < (unsigned)P.g.n[2]) {
+        if (item < BY * (W2 - 1) && ly >= ly_lo && ly <= ly_hi && (unsigned)gy < (unsigned)P.g.n[1] && (unsigned)gz < (unsigned)P.g.n[2]) {
             const long long off = gx + nx * gy + plane * gz;
             __stcg(fld[0] + off, x.v[r][0]);
             __stcg(fld[1] + off, x.v[r][1]);
@@ -872,7 +885,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 }
 
 template <bool COEF>
-__global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_constant__ SysParams P, const __grid_constant__ TmaMaps M)
+__global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __grid_constant__ SysParams P, const __grid_constant__ TmaMaps M)
 {
     extern __shared__ __align__(128) float sm[];
     __shared__ __align__(8) unsigned long long mb[MB_COUNT];
@@ -1138,27 +1151,27 @@ __global__ void __launch_bounds__(NT, 1) systolic_tma_kernel(const __grid_consta
 
 }  // namespace
 
-size_t systolic_tma_smem(int coef) { return (size_t)(coef ? Lay<true>::total : Lay<false>::total) * sizeof(float); }
-int systolic_tma_threads() { return NT; }
-void systolic_tma_boxes(int box[3][3])
+size_t FDTD_TMA_NAME(systolic_tma_smem)(int coef) { return (size_t)(coef ? Lay<true>::total : Lay<false>::total) * sizeof(float); }
+int FDTD_TMA_NAME(systolic_tma_threads)() { return NT; }
+void FDTD_TMA_NAME(systolic_tma_boxes)(int box[3][3])
 {
     const int b[3][3] = {{RX, BY, 1}, {RX, 1, BZ}, {4, BY, W2}};
     for (int f = 0; f < 3; ++f)
         for (int q = 0; q < 3; ++q) box[f][q] = b[f][q];
 }
 
-cudaError_t systolic_tma_prepare(int coef, int* blocks_per_sm)
+cudaError_t FDTD_TMA_NAME(systolic_tma_prepare)(int coef, int* blocks_per_sm)
 {
     const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)systolic_tma_smem(coef));
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FDTD_TMA_NAME(systolic_tma_smem)(coef));
     if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, fn, NT, systolic_tma_smem(coef));
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, fn, NT, FDTD_TMA_NAME(systolic_tma_smem)(coef));
 }
 
-cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st)
+cudaError_t FDTD_TMA_NAME(launch_systolic_tma)(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st)
 {
     static_assert(sizeof(CUtensorMap) == 128, "TmaMaps layout");
     const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
     void* args[] = {(void*)&p, (void*)&maps};
-    return cudaLaunchKernel(fn, dim3((unsigned)ctas), dim3((unsigned)NT), args, systolic_tma_smem(coef), st);
+    return cudaLaunchKernel(fn, dim3((unsigned)ctas), dim3((unsigned)NT), args, FDTD_TMA_NAME(systolic_tma_smem)(coef), st);
 }

@@ -1,0 +1,111 @@
+"""GPU parity of the SURVEY.md 8(f) rows and of the two-CTAs-per-SM build of the systolic kernel, through the C ABI,
+against the CPU oracles (oracle/yee.py, oracle/absorber.py, oracle/monitor.py), element by element on the same
+seeded inputs.  The product library is the -fmad=false build: every comparison here is BIT-EXACT."""
+import numpy as np
+import pytest
+
+from oracle.absorber import absorber_coeffs
+from oracle.yee import YeeOracle
+from paper_2502_20610_b200 import binding, workloads
+from paper_2502_20610_b200.workloads import PEC, PERIODIC
+from tests.test_gpu_parity import CASES, compare, gpu_run, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+
+# ---- tile 31x7x7 (systolic_tma_by8.cu: the TMA-staged kernel with a 32x8x8 box, two CTAs per SM) ---------------------
+BY8_RUNS = [("C1", 8), ("C1", 33), ("C1", 100), ("C2s", 5), ("C2s", 32), ("C3s", 16), ("C4s", 40), ("C4s", 3), ("C5s", 32),
+            ("C5s", 1), ("ragged", 6), ("allper", 5)]
+
+
+@pytest.fixture(scope="module")
+def oracle_cache():
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            w, steps = CASES[name]
+            cache[name] = oracle_run(w, steps)
+        return cache[name]
+    return get
+
+
+@pytest.mark.parametrize("variant", ["nofma", "fma"])
+@pytest.mark.parametrize("name,T", BY8_RUNS)
+def test_tile_31x7x7_matches_oracle(cuda_device, oracle_cache, name, T, variant):
+    w, steps = CASES[name]
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 7, 7), T=T, variant=variant)
+    assert info["which"] == binding.KERNEL_SYSTOLIC and info["tile"] == (31, 7, 7) and info["T"] == T
+    compare((E, H), oracle_cache(name), exact=(variant == "nofma"))
+
+
+# ---- f3: adiabatic-absorber coefficient generator -------------------------------------------------------------------
+ABSORBER_CASES = [
+    # n, dt, with eps, thickness, sigma_max, order
+    ((40, 36, 28), 0.2886751, True, (8, 6, 5, 7, 4, 9), (0.11, 0.07, 0.2, 0.05, 0.3, 0.09), 2),
+    ((37, 29, 23), 0.25, False, (10, 0, 0, 12, 23, 0), (0.4, 0.0, 0.0, 0.15, 0.02, 0.0), 3),
+    ((64, 8, 8), 0.31, True, (32, 32, 0, 0, 0, 0), (0.25, 0.3, 0, 0, 0, 0), 1),       # the two layers of an axis meet
+    ((16, 16, 16), 0.1, True, (3, 3, 3, 3, 3, 3), (0.5,) * 6, 0),                    # order 0: uniform inside the layer
+    ((130, 70, 33), 0.2, True, (20, 20, 10, 10, 8, 8), (0.05,) * 6, 4),
+]
+
+
+@pytest.mark.parametrize("n,dt,with_eps,thickness,smax,order", ABSORBER_CASES)
+def test_absorber_generator_bit_exact(cuda_device, n, dt, with_eps, thickness, smax, order):
+    import torch
+    shape = (n[2], n[1], n[0])
+    rng = np.random.default_rng(n[0] * 1000 + order)
+    eps = [rng.uniform(1.0, 12.1, shape).astype(np.float32) for _ in range(3)] if with_eps else None
+    want_ca, want_cb = absorber_coeffs(n, np.float32(dt), eps, thickness, smax, order, np.float32)
+    dev = torch.device("cuda:0")
+    eps_d = None if eps is None else [torch.from_numpy(e).to(dev) for e in eps]
+    ca = [torch.full(shape, -7.0, dtype=torch.float32, device=dev) for _ in range(3)]
+    cb = [torch.full(shape, -7.0, dtype=torch.float32, device=dev) for _ in range(3)]
+    binding.absorber_coeffs(n, dt, eps_d, thickness, smax, order, ca, cb)
+    torch.cuda.synchronize()
+    for a in range(3):
+        assert np.array_equal(ca[a].cpu().numpy(), want_ca[a]), f"ca[{a}] differs"
+        assert np.array_equal(cb[a].cpu().numpy(), want_cb[a]), f"cb[{a}] differs"
+
+
+def test_absorber_rejects_bad_arguments(cuda_device):
+    import torch
+    dev = torch.device("cuda:0")
+    n = (8, 8, 8)
+    out = [torch.empty((8, 8, 8), dtype=torch.float32, device=dev) for _ in range(6)]
+    for th, sm, order in (((9, 0, 0, 0, 0, 0), (0.1,) * 6, 2), ((1, 0, 0, 0, 0, 0), (-0.1, 0, 0, 0, 0, 0), 2), ((1,) * 6, (0.1,) * 6, 9),
+                          ((-1, 0, 0, 0, 0, 0), (0.1,) * 6, 2)):
+        with pytest.raises(binding.FdtdError) as e:
+            binding.absorber_coeffs(n, 0.1, None, th, sm, order, out[:3], out[3:])
+        assert e.value.code == binding.EINVAL
+
+
+def test_absorber_run_end_to_end_matches_oracle(cuda_device):
+    """Generator output fed to the systolic kernel: a pulse hits graded layers on all six faces; the fields after the run
+    equal the oracle's run on the oracle generator's coefficients, bit for bit."""
+    import torch
+    w = workloads.config(1).scaled((72, 60, 52), steps=120)
+    n, dt = w.n, w.dt
+    th, sm = (10, 10, 8, 8, 9, 7), (0.08, 0.08, 0.1, 0.1, 0.09, 0.12)
+    eps_h = [np.ascontiguousarray(e, dtype=np.float32) for e in workloads.make_eps(w)]
+    ca_h, cb_h = absorber_coeffs(n, np.float32(dt), eps_h, th, sm, 2, np.float32)
+    E, H = workloads.make_fields(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca_h, cb_h, None)
+    src = workloads.make_source(w)
+    orc.set_source(src.comp, src.box, src.amp, src.wave)
+    orc.step(120)
+    dev = torch.device("cuda:0")
+    Ed, Hd = workloads.make_fields(w, device=dev)
+    eps_d = [torch.from_numpy(np.ascontiguousarray(e)).to(dev) for e in eps_h]
+    ca = [torch.empty_like(Ed[0]) for _ in range(3)]
+    cb = [torch.empty_like(Ed[0]) for _ in range(3)]
+    binding.absorber_coeffs(n, dt, eps_d, th, sm, 2, ca, cb)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+    sim.set_fields(Ed, Hd)
+    sim.set_coeffs(ca, cb, None)
+    sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.step(120)
+    sim.sync()
+    sim.close()
+    compare(([x.cpu().numpy() for x in Ed], [x.cpu().numpy() for x in Hd]), (E, H), exact=True)
+    assert float(np.abs(E[2]).max()) > 0

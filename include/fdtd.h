@@ -100,6 +100,20 @@ int fdtd_set_coeffs(fdtd_ctx* ctx, const float* const ca[3], const float* const 
 int fdtd_set_source(fdtd_ctx* ctx, int comp, int i0, int j0, int k0, int ni, int nj, int nk,
                     const float* amp, const float* wave, int nwave);
 
+/* Running-DFT output monitor on one plane (outputs are excluded from the paper's benchmark but named as what real runs
+ * carry; reading #13).  While the step counter t is in [0, nt), every step adds, for each cell of
+ * the plane `axis` = `index`, each frequency f < nfreq and each component a:
+ *     after the E half-step and the source:  acc[a][f][0|1][cell]     += E_a * wE[t][f][0|1]
+ *     after the H half-step:                 acc[3 + a][f][0|1][cell] += H_a * wH[t][f][0|1]
+ * (product rounded to fp32, then the add; [0|1] = real | imaginary part of the complex weight).  The weights are the
+ * caller's: e.g. wE[t][f] = exp(-i w_f (t+1) dt), wH[t][f] = exp(-i w_f (t+3/2) dt), or a window times these.
+ * wE, wH: HOST arrays [nt][nfreq][2], copied.  acc: DEVICE array [6][nfreq][2][cells], BORROWED, not cleared by the
+ * library; cells of the plane are numbered x fastest over the two remaining axes (axis 0: j + ny*k; 1: i + nx*k; 2: i + nx*j).
+ * One monitor per context; acc == NULL removes it.  Runs inside FDTD_KERNEL_NAIVE and FDTD_KERNEL_SYSTOLIC (tiles
+ * 31x15x7 and 31x7x7); other schedules make fdtd_step return FDTD_EINVAL while a monitor is set.
+ * FDTD_EINVAL: axis/index outside the grid, nfreq not in 1..64, nt < 1, NULL table, misaligned acc. */
+int fdtd_set_monitor(fdtd_ctx* ctx, int axis, int index, int nfreq, int nt, const float* wE, const float* wH, float* acc);
+
 /* Advance n >= 0 steps; enqueues on the ctx stream and returns without synchronising; ctx time += n.
  * FDTD_ESTATE before fdtd_set_fields.  A device-side failure (hand-off watchdog) is reported by the next
  * fdtd_get_fields / fdtd_sync as FDTD_ETIMEOUT.   (eq. (1); sections 3-4 for the schedule) */

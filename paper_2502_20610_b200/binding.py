@@ -27,6 +27,7 @@ _PROTOS = {
     "fdtd_set_coeffs": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_float)]),
     "fdtd_set_source": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                   C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int]),
+    "fdtd_set_monitor": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_void_p]),
     "fdtd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "fdtd_get_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "fdtd_sync": (C.c_int, [C.c_void_p]),
@@ -169,6 +170,23 @@ class Fdtd:
         fp = C.POINTER(C.c_float)
         self._check(self._lib.fdtd_set_source(self._h, int(comp), *[int(x) for x in box], amp.ctypes.data_as(fp),
                                               wave.ctypes.data_as(fp), int(wave.size)))
+
+    def set_monitor(self, axis, index, wE, wH, acc):
+        """Running DFT on the plane axis = index.  wE, wH: numpy (nt, F, 2); acc: float32 CUDA tensor (6, F, 2, cells),
+        borrowed and accumulated into (the caller zeroes it).  acc=None removes the monitor."""
+        import numpy as np
+        if acc is None:
+            self._check(self._lib.fdtd_set_monitor(self._h, 0, 0, 0, 0, None, None, None))
+            return
+        wE = np.ascontiguousarray(wE, dtype=np.float32)
+        wH = np.ascontiguousarray(wH, dtype=np.float32)
+        assert wE.shape == wH.shape and wE.ndim == 3 and wE.shape[2] == 2
+        nt, F = wE.shape[0], wE.shape[1]
+        assert acc.is_cuda and acc.is_contiguous() and acc.numel() == 6 * F * 2 * (self.n[0] * self.n[1] * self.n[2] // self.n[axis])
+        self._keep.append(acc)
+        fp = C.POINTER(C.c_float)
+        self._check(self._lib.fdtd_set_monitor(self._h, int(axis), int(index), F, nt, wE.ctypes.data_as(fp), wH.ctypes.data_as(fp),
+                                               C.c_void_p(acc.data_ptr())))
 
     def set_kernel(self, which, tile=None, T=0):
         tx, ty, tz = tile if tile is not None else (0, 0, 0)

@@ -23,6 +23,8 @@ struct fdtd_ctx {
     float* d_wave;
     std::vector<float> h_wave;
     long long t;
+    MonitorParams mon;   // running-DFT monitor in CALLER coordinates (G = 0); mon.on == 0: none
+    float* d_mon_w;      // device copy of the weight tables: wE[nt][F][2] then wH[nt][F][2]
     // schedule
     int which;
     bool which_explicit;   // fdtd_set_kernel was called: no automatic choice
@@ -418,9 +420,20 @@ int step_naive(fdtd_ctx* c, int n)
             if (e != cudaSuccess) return cuda_fail(c, e, "source launch");
             c->counters[0]++;
         }
+        const bool mon = c->mon.on && c->t >= 0 && c->t < c->mon.nt;
+        if (mon) {
+            e = launch_monitor_naive(c->g, c->mon, 0, c->t, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "monitor launch");
+            c->counters[0]++;
+        }
         e = launch_h_half_naive(c->g, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "H half-step launch");
         c->counters[0]++;
+        if (mon) {
+            e = launch_monitor_naive(c->g, c->mon, 1, c->t, c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "monitor launch");
+            c->counters[0]++;
+        }
         c->t++;
         c->counters[1]++;
     }
@@ -437,6 +450,8 @@ int step_systolic(fdtd_ctx* c, int n)
         const int rc = ensure_tmaps(c);
         if (rc != FDTD_OK) return rc;
     }
+    if (c->mon.on && !c->use_tma)
+        return fail(c, FDTD_EINVAL, "a monitor needs FDTD_KERNEL_SYSTOLIC with tile 31x15x7 or 31x7x7, or FDTD_KERNEL_NAIVE");
     const int N[3] = {c->N[0], c->N[1], c->N[2]};
     long long ldx = 0;
     const GridParams wg = work_grid(c, &ldx);
@@ -531,6 +546,11 @@ int step_systolic(fdtd_ctx* c, int n)
         P.spin_budget = c->spin_budget;
         P.delay_seed = c->delay_seed;
         P.prof = c->d_prof;
+        P.mon = c->mon;
+        if (c->mon.on && c->use_pad) {
+            for (int a = 0; a < 3; ++a) P.mon.G[a] = c->pg.G[a];
+            P.mon.index = c->mon.index + c->pg.G[c->mon.axis];
+        }
         for (int g = 0; g < 3; ++g) P.tma_group[g] = c->tma_group[g];
         P.dbg = c->dbg_skip;
         P.withhold_tile = c->dbg_withhold;
@@ -657,6 +677,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->d_counter = nullptr;
     c->d_abort = nullptr;
     c->d_prof = nullptr;
+    c->d_mon_w = nullptr;
+    memset(&c->mon, 0, sizeof c->mon);
     c->d_order = nullptr;
     c->flag_base = 0;
     c->delay_seed = 0;
@@ -797,6 +819,38 @@ int fdtd_set_source(fdtd_ctx* c, int comp, int i0, int j0, int k0, int ni, int n
     c->g.src_amp = c->d_amp;
     c->g.src_wave = c->d_wave;
     c->g.src_nwave = nwave;
+    return FDTD_OK;
+}
+
+int fdtd_set_monitor(fdtd_ctx* c, int axis, int index, int nfreq, int nt, const float* wE, const float* wH, float* acc)
+{
+    if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
+    cudaError_t e = cudaStreamSynchronize(c->stream);   // the old tables may still be in use
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    if (c->d_mon_w) cudaFree(c->d_mon_w);
+    c->d_mon_w = nullptr;
+    memset(&c->mon, 0, sizeof c->mon);
+    if (!acc) return FDTD_OK;
+    if (axis < 0 || axis > 2 || index < 0 || index >= c->g.n[axis] || nfreq < 1 || nfreq > 64 || nt < 1 || !wE || !wH)
+        return fail(c, FDTD_EINVAL, "fdtd_set_monitor: bad axis, index, nfreq (1..64), nt or weight table");
+    if (!aligned16(acc)) return fail(c, FDTD_EINVAL, "fdtd_set_monitor: misaligned accumulator");
+    const size_t nw = (size_t)nt * nfreq * 2;
+    e = cudaMalloc(&c->d_mon_w, 2 * nw * sizeof(float));
+    if (e != cudaSuccess) return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(monitor weights): ") + cudaGetErrorString(e));
+    e = cudaMemcpy(c->d_mon_w, wE, nw * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_mon_w + nw, wH, nw * sizeof(float), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(monitor weights)");
+    c->mon.on = 1;
+    c->mon.axis = axis;
+    c->mon.index = index;
+    c->mon.F = nfreq;
+    c->mon.nt = nt;
+    for (int a = 0; a < 3; ++a) c->mon.n[a] = c->g.n[a];
+    c->mon.wE = c->d_mon_w;
+    c->mon.wH = c->d_mon_w + nw;
+    c->mon.acc = acc;
+    c->mon.pcells = (long long)c->g.n[0] * c->g.n[1] * c->g.n[2] / c->g.n[axis];
     return FDTD_OK;
 }
 
@@ -993,6 +1047,7 @@ void fdtd_destroy(fdtd_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->d_amp) cudaFree(c->d_amp);
     if (c->d_wave) cudaFree(c->d_wave);
+    if (c->d_mon_w) cudaFree(c->d_mon_w);
     if (c->d_flags) cudaFree(c->d_flags);
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);

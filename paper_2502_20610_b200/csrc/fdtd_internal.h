@@ -10,6 +10,8 @@ cudaError_t launch_e_half_naive(const GridParams& g, cudaStream_t st);
 cudaError_t launch_h_half_naive(const GridParams& g, cudaStream_t st);
 cudaError_t launch_source_w(const GridParams& g, float w, cudaStream_t st);   // w = wave[t], looked up by the host
 
+cudaError_t launch_monitor_naive(const GridParams& g, const MonitorParams& m, int isH, long long t, cudaStream_t st);   // row f4
+
 // implemented in systolic_kernel.cu
 int systolic_num_configs();
 const SysConfig* systolic_config(int idx);

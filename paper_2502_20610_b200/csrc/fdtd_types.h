@@ -87,6 +87,33 @@ struct PadArrays {
     int narr;
 };
 
+// Running-DFT monitor on one plane of the grid (PAPER.md:106 names outputs as what real runs carry;
+// DESIGN.md reading #13).  During step t (0 <= t < nt), for every cell of the plane and every frequency f:
+//     after the E half-step and the source:  acc[a][f][re|im][cell]     += E_a * wE[t][f][re|im]     a = 0..2
+//     after the H half-step:                 acc[3 + a][f][re|im][cell] += H_a * wH[t][f][re|im]
+// (product rounded, then the add).  Plane cells are numbered x fastest over the two remaining axes of the CALLER's grid.
+struct MonitorParams {
+    int on;               // 0: no monitor
+    int axis, index;      // plane axis; plane index in WORKING coordinates (caller index + G[axis])
+    int F, nt;
+    int n[3];             // extents of the caller's grid
+    int G[3];             // working coordinate = caller coordinate + G (the padded copy of DESIGN.md 6.4), else 0
+    const float* wE;      // device, [nt][F][2]
+    const float* wH;
+    float* acc;           // device, [6][F][2][pcells], borrowed from the caller
+    long long pcells;
+    // cell number inside the plane of the working-grid cell (gx,gy,gz), or -1 when the cell is not on the plane or is a
+    // ghost image outside the caller's grid
+    FDTD_HD long long cell(int gx, int gy, int gz) const
+    {
+        const int g[3] = {gx, gy, gz};
+        if (g[axis] != index) return -1;
+        const int u0 = gx - G[0], u1 = gy - G[1], u2 = gz - G[2];
+        if ((unsigned)u0 >= (unsigned)n[0] || (unsigned)u1 >= (unsigned)n[1] || (unsigned)u2 >= (unsigned)n[2]) return -1;
+        return axis == 0 ? u1 + (long long)n[1] * u2 : axis == 1 ? u0 + (long long)n[0] * u2 : u0 + (long long)n[0] * u1;
+    }
+};
+
 struct SysParams {
     GridParams g;
     AxisPlan ax[3];
@@ -106,6 +133,7 @@ struct SysParams {
     int ldx;
     int nsrc;              // 0: no source; else number of images of g.src_box
     int src_org[MAX_SRC_IMAGES][3];
+    MonitorParams mon;     // running-DFT monitor (mon.on == 0: none)
     long long* prof;       // FDTD_PROFILE build: 32 tick accumulators (NULL otherwise)
     // FDTD_DEBUG builds only (always 0 / NULL in the product libraries, and never read there):
     int dbg;               // FDTD_DEBUG_SKIP timing probes (results invalid): 1 no upwind waits, 2 no shell loads, 4 no publishes,

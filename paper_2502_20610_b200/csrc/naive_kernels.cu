@@ -253,3 +253,36 @@ cudaError_t launch_source_w(const GridParams& g, float w, cudaStream_t st)
     source_kernel<<<blocks, 256, 0, st>>>(g, w);
     return cudaGetLastError();
 }
+
+// ---- running-DFT monitor (row f4): one thread per plane cell and component, all frequencies ----------------------------
+namespace {
+__global__ void __launch_bounds__(128) monitor_kernel(const __grid_constant__ GridParams g, const __grid_constant__ MonitorParams m, int isH, long long t)
+{
+    const long long q = blockIdx.x * 128ll + threadIdx.x;
+    if (q >= 3 * m.pcells) return;
+    const int c = (int)(q / m.pcells);
+    const long long cell = q % m.pcells;
+    // plane cell -> grid coordinates (the naive kernels run on the caller's grid: G = 0)
+    int i, j, k;
+    if (m.axis == 0)      { i = m.index; j = (int)(cell % m.n[1]); k = (int)(cell / m.n[1]); }
+    else if (m.axis == 1) { j = m.index; i = (int)(cell % m.n[0]); k = (int)(cell / m.n[0]); }
+    else                  { k = m.index; i = (int)(cell % m.n[0]); j = (int)(cell / m.n[0]); }
+    const long long off = i + (long long)g.n[0] * (j + (long long)g.n[1] * k);
+    const float v = (isH ? g.H[c] : g.E[c])[off];
+    const float* w = (isH ? m.wH : m.wE) + t * m.F * 2;
+    float* acc = m.acc + ((long long)(isH ? 3 + c : c) * m.F * 2) * m.pcells + cell;
+    for (int f = 0; f < m.F; ++f) {
+        const float pr = v * w[2 * f];
+        const float pi = v * w[2 * f + 1];
+        acc[(2 * f) * m.pcells] = acc[(2 * f) * m.pcells] + pr;
+        acc[(2 * f + 1) * m.pcells] = acc[(2 * f + 1) * m.pcells] + pi;
+    }
+}
+}  // namespace
+
+cudaError_t launch_monitor_naive(const GridParams& g, const MonitorParams& m, int isH, long long t, cudaStream_t st)
+{
+    const long long items = 3 * m.pcells;
+    monitor_kernel<<<(unsigned)((items + 127) / 128), 128, 0, st>>>(g, m, isH, t);
+    return cudaGetLastError();
+}

@@ -483,6 +483,43 @@ __shared__ unsigned trace_cur_;
 #define TRACE_C(ev, k)
 #endif
 
+// Running-DFT monitor (row f4, reading #13): the cells of the plane that this thread has just updated in step
+// t0 + k are accumulated into the caller's device array.  Every (cell, step) pair is updated by exactly one thread of one
+// tile; successive steps of a cell are ordered by program order inside a tile and by the flag hand-off between tiles (the
+// read-modify-write below is issued before the warp arrives on the DONE barrier that the signal warp's fence covers, and
+// goes through L2).  Rare path: the caller tests the CTA-uniform conditions first.
+template <int NV>
+__device__ __forceinline__ void monitor_add(const MonitorParams& m, const float* w, int base, int gx, int gy, int gz, const float (&v)[NV][3])
+{
+    // v[l] = the three components at plane gz + l
+#pragma unroll
+    for (int l = 0; l < NV; ++l) {
+        const long long cell = m.cell(gx, gy, gz + l);
+        if (cell < 0) continue;
+        float* acc = m.acc + ((long long)base * m.F * 2) * m.pcells + cell;
+        for (int f = 0; f < m.F; ++f) {
+            const float wr = __ldg(w + 2 * f), wi = __ldg(w + 2 * f + 1);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                float* pr = acc + ((long long)(c * m.F + f) * 2) * m.pcells;
+                float* pi = pr + m.pcells;
+                const float qr = v[l][c] * wr;
+                const float qi = v[l][c] * wi;
+                __stcg(pr, __ldcg(pr) + qr);
+                __stcg(pi, __ldcg(pi) + qi);
+            }
+        }
+    }
+}
+// CTA-uniform: does the monitor plane cut the region [lo, lo + W) of this step, and is step ts inside the weight table
+__device__ __forceinline__ bool monitor_hits(const MonitorParams& m, long long ts, int lo0, int lo1, int lo2)
+{
+    if (!m.on || ts < 0 || ts >= m.nt) return false;
+    const int lo = m.axis == 0 ? lo0 : m.axis == 1 ? lo1 : lo2;
+    const int wd = m.axis == 0 ? W0 : m.axis == 1 ? W1 : W2;
+    return m.index >= lo && m.index < lo + wd;
+}
+
 struct Phases {   // completed phases of each mbarrier as seen by this thread's role (all users count alike)
     unsigned hready, eready, acke, ackh, cfull;
 };
@@ -585,10 +622,10 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 exH[(l - 1) * PLANE + slot1] = make_float2(hz[RL][l], hx[RL][l]);
             }
         } else {
-            TRACE_C( 0, k);
+            TRACE_C(0, k);
             mbar_wait(mb + MB_HREADY, ph.hready & 1u);
             ++ph.hready;
-            TRACE_C( 1, k);
+            TRACE_C(1, k);
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 hx[r][0] = stgH[zidx<3>(0, ly[r], xs)];
@@ -635,7 +672,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         bar_sync(1, NCOMPUTE);   // exchange rows of H (shell + last H phase) and the scattered coefficients are visible
 
         PROF_MARK(1);
-        TRACE_C( 2, k);
+        TRACE_C(2, k);
         // ---------------- E phase on R_k = [1,w]^3 (a1): every slot computes, shell slots produce garbage ----
         // fast (no coefficient arrays, box never touches a wall or the outside): cb is the scalar dt, no mask loads
         auto e_phase = [&](auto fastc) {
@@ -704,6 +741,18 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 }
             }
         }
+        // running DFT of E on the monitor plane: R_k = [o+1, o+W] on every axis
+        if (monitor_hits(P.mon, P.t0 + k, o0 + 1, o1 + 1, o2 + 1)) {
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
+                if ((lx >= 1) & (ly[r] >= 1) && col_in[r]) {
+                    float v[W2][3];
+#pragma unroll
+                    for (int l = 1; l < BZ; ++l) { v[l - 1][0] = ex[r][l + 1]; v[l - 1][1] = ey[r][l + 1]; v[l - 1][2] = ez[r][l + 1]; }
+                    monitor_add<W2>(P.mon, P.mon.wE + (P.t0 + k) * P.mon.F * 2, 0, gx, gy[r], o2 + 1, v);
+                }
+            }
+        }
         // E of row 0, planes 1..6, for the previous warp's row 1 in the H phase; the shell column lx = 0 is written by the
         // E-side warp
         if (lx != 0) {
@@ -713,7 +762,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         PROF_MARK(2);
-        TRACE_C( 3, k);
+        TRACE_C(3, k);
         if (k > k0) {   // the signal warp has copied the x-out rows of step k-1 (and the DONE barriers cannot lap it)
             mbar_wait(mb + MB_ACKE, ph.acke & 1u);
             ++ph.acke;
@@ -753,7 +802,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         warp_arrive(mb + MB_EDONE);
-        TRACE_C( 4, k);
+        TRACE_C(4, k);
         FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 1);)
 
         // ---------------- E minus shell -------------------------------------------------------------------------
@@ -761,7 +810,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         mbar_wait(mb + MB_EREADY, ph.eready & 1u);
         ++ph.eready;
         PROF_MARK(4);
-        TRACE_C( 5, k);
+        TRACE_C(5, k);
 #pragma unroll
         for (int r = 0; r < NROW; ++r) {
             ex[r][1] = stgE[zidx<3>(0, ly[r], xs)];
@@ -803,7 +852,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #endif
         bar_sync(1, NCOMPUTE);   // exchange rows of E are visible; every warp has finished E phase k
         PROF_MARK(5);
-        TRACE_C( 6, k);
+        TRACE_C(6, k);
         // ---------------- coefficients of the cells that entered with this step's shell ------------------------------
         // first used by E phase k+1 (shell cells are not in R_k); copied a whole step ahead (issued after CFREE(k-1))
         if (k >= 1 && !fast) {
@@ -815,7 +864,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             warp_arrive(mb + MB_CFREE);
         }
         PROF_MARK(7);
-        TRACE_C( 7, k);
+        TRACE_C(7, k);
 
         // ---------------- H phase on R_{k+1} = [0,w-1]^3 (a2): every slot computes ----------------------------
 #pragma unroll
@@ -835,7 +884,19 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
             exH[l * PLANE + slot1] = make_float2(hz[RL][l + 1], hx[RL][l + 1]);
         }
-        TRACE_C( 8, k);
+        // running DFT of H on the monitor plane: R_{k+1} = [o, o+W-1] on every axis
+        if (monitor_hits(P.mon, P.t0 + k, o0, o1, o2)) {
+#pragma unroll
+            for (int r = 0; r < NROW; ++r) {
+                if ((lx <= W0 - 1) & (ly[r] <= W1 - 1) && col_in[r]) {
+                    float v[W2][3];
+#pragma unroll
+                    for (int l = 0; l < BZ - 1; ++l) { v[l][0] = hx[r][l + 1]; v[l][1] = hy[r][l + 1]; v[l][2] = hz[r][l + 1]; }
+                    monitor_add<W2>(P.mon, P.mon.wH + (P.t0 + k) * P.mon.F * 2, 3, gx, gy[r], o2, v);
+                }
+            }
+        }
+        TRACE_C(8, k);
         if (k > k0) {   // the signal warp has copied the H x-out rows of step k-1 (HDONE cannot lap its waiters)
             mbar_wait(mb + MB_ACKH, ph.ackh & 1u);
             ++ph.ackh;
@@ -875,7 +936,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         warp_arrive(mb + MB_HDONE);
-        TRACE_C( 9, k);
+        TRACE_C(9, k);
         FDTD_DEBUG_ONLY(if (P.delay_seed != 0u) debug_delay(P, tile, k, 2);)
         PROF_MARK(6);
     }

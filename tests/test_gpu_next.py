@@ -109,3 +109,97 @@ def test_absorber_run_end_to_end_matches_oracle(cuda_device):
     sim.close()
     compare(([x.cpu().numpy() for x in Ed], [x.cpu().numpy() for x in Hd]), (E, H), exact=True)
     assert float(np.abs(E[2]).max()) > 0
+
+
+# ---- f4: running-DFT monitors ---------------------------------------------------------------------------------------
+def _weights(nt, F, seed):
+    """Complex weights of a windowed DFT: exp(-i w_f (t+1) dt') * hann(t), as float32 (re, im) tables for E and H."""
+    t = np.arange(nt, dtype=np.float64)
+    win = 0.5 - 0.5 * np.cos(2 * np.pi * (t + 0.5) / nt)
+    om = 0.05 + 0.11 * np.arange(F) + 0.003 * seed
+    wE = np.zeros((nt, F, 2))
+    wH = np.zeros((nt, F, 2))
+    for f in range(F):
+        wE[:, f, 0], wE[:, f, 1] = win * np.cos(om[f] * (t + 1)), -win * np.sin(om[f] * (t + 1))
+        wH[:, f, 0], wH[:, f, 1] = win * np.cos(om[f] * (t + 1.5)), -win * np.sin(om[f] * (t + 1.5))
+    return wE.astype(np.float32), wH.astype(np.float32)
+
+
+MONITOR_RUNS = [
+    # case, steps, nt (weights table length), axis, index, F, kernel, tile, T
+    ("C2s", 90, 90, 2, 26, 2, "naive", None, 0),
+    ("C2s", 90, 90, 2, 26, 2, "systolic", (31, 15, 7), 32),
+    ("C2s", 90, 70, 0, 36, 3, "systolic", (31, 15, 7), 128),      # table shorter than the run
+    ("C2s", 90, 90, 1, 0, 1, "systolic", (31, 7, 7), 17),          # the frozen low wall plane
+    ("C2s", 90, 90, 1, 59, 1, "systolic", (31, 15, 7), 7),         # the last plane
+    ("C3s", 60, 60, 0, 5, 2, "naive", None, 0),
+    ("C3s", 60, 60, 0, 5, 2, "systolic", (31, 15, 7), 8),          # periodic x on the padded copy: plane has ghost images
+    ("C3s", 60, 60, 2, 20, 2, "systolic", (31, 15, 7), 8),
+    ("ragged", 50, 50, 1, 11, 2, "systolic", (31, 15, 7), 6),      # odd nx, periodic y
+    ("ragged", 50, 50, 0, 36, 2, "systolic", (31, 7, 7), 50),
+    ("C5s", 90, 90, 2, 18, 4, "systolic", (31, 15, 7), 32),
+]
+
+
+@pytest.mark.parametrize("name,steps,nt,axis,index,F,kernel,tile,T", MONITOR_RUNS)
+def test_monitor_matches_oracle_bit_exact(cuda_device, name, steps, nt, axis, index, F, kernel, tile, T):
+    import torch
+    from oracle.monitor import MonitorOracle
+    w, _ = CASES[name]
+    wE, wH = _weights(nt, F, axis + index)
+    E, H = workloads.make_fields(w)
+    ca, cb = workloads.make_coeffs(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None)
+    src = workloads.make_source(w)
+    if src is not None:
+        orc.set_source(src.comp, src.box, src.amp, src.wave)
+    mon = MonitorOracle(orc, axis, index, wE, wH)
+    mon.step(steps)
+    want = mon.acc.reshape(6, F, 2, -1)
+
+    dev = torch.device("cuda:0")
+    Ed, Hd = workloads.make_fields(w, device=dev)
+    cad, cbd = workloads.make_coeffs(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+    sim.set_fields(Ed, Hd)
+    if cad is not None:
+        sim.set_coeffs(cad, cbd, None)
+    if src is not None:
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_NAIVE if kernel == "naive" else binding.KERNEL_SYSTOLIC, tile, T)
+    acc = torch.zeros((6, F, 2, want.shape[3]), dtype=torch.float32, device=dev)
+    sim.set_monitor(axis, index, wE, wH, acc)
+    # two calls: the second one continues the accumulation
+    sim.step(steps // 3)
+    sim.step(steps - steps // 3)
+    sim.sync()
+    sim.close()
+    got = acc.cpu().numpy()
+    assert float(np.abs(want).max()) > 0
+    assert np.array_equal(got, want), f"monitor differs: max {np.abs(got - want).max():.3e}"
+    compare(([x.cpu().numpy() for x in Ed], [x.cpu().numpy() for x in Hd]), (E, H), exact=True)   # and the fields are untouched by it
+
+
+def test_monitor_rejected_by_other_schedules_and_bad_arguments(cuda_device):
+    import torch
+    w, _ = CASES["C1"]
+    dev = torch.device("cuda:0")
+    Ed, Hd = workloads.make_fields(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+    sim.set_fields(Ed, Hd)
+    wE, wH = _weights(10, 1, 0)
+    acc = torch.zeros((6, 1, 2, 64 * 64), dtype=torch.float32, device=dev)
+    for axis, index in ((3, 0), (0, 64), (1, -1)):
+        with pytest.raises(binding.FdtdError) as e:
+            sim._check(sim._lib.fdtd_set_monitor(sim._h, axis, index, 1, 10, wE.ctypes.data_as(binding.C.POINTER(binding.C.c_float)),
+                                                 wH.ctypes.data_as(binding.C.POINTER(binding.C.c_float)), binding.C.c_void_p(acc.data_ptr())))
+        assert e.value.code == binding.EINVAL
+    sim.set_monitor(0, 3, wE, wH, acc)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC_REG, (31, 15, 7), 8)
+    with pytest.raises(binding.FdtdError) as e:
+        sim.step(2)
+    assert e.value.code == binding.EINVAL
+    sim.set_monitor(0, 0, None, None, None)     # removed: the schedule runs again
+    sim.step(2)
+    sim.sync()
+    sim.close()

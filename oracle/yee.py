@@ -40,7 +40,7 @@ def lib():
     global _lib
     if _lib is None:
         _lib = C.CDLL(build_oracle.build())
-        for suf in ("f32", "f64"):
+        for suf in ("f32", "f64", "h16"):
             getattr(_lib, "yee_oracle_run_" + suf).restype = C.c_int
             getattr(_lib, "yee_oracle_e_half_" + suf).restype = C.c_int
             getattr(_lib, "yee_oracle_h_half_" + suf).restype = C.c_int
@@ -56,9 +56,19 @@ class YeeOracle:
     cb None -> dt; db None -> (dt, dt, dt)  (SURVEY.md 8(b) fdtd_set_coeffs contract).
     """
 
-    def __init__(self, n, d, dt, boundary, E, H, ca=None, cb=None, db=None, nthreads=None):
+    def __init__(self, n, d, dt, boundary, E, H, ca=None, cb=None, db=None, nthreads=None, storage=None):
+        """storage="f16" (float32 arrays only): every stored field value is rounded to IEEE binary16 (row f1, PAPER.md:104);
+        the arrays must hold binary16-representable values on entry."""
         self.dtype = np.dtype(E[0].dtype)
         assert self.dtype in _GRID
+        self.suffix = _SUF[self.dtype]
+        if storage == "f16":
+            assert self.dtype == np.dtype(np.float32)
+            for a in list(E) + list(H):
+                assert np.array_equal(a, a.astype(np.float16).astype(np.float32)), "f16 storage: inputs must be binary16 values"
+            self.suffix = "h16"
+        else:
+            assert storage is None
         self.n = tuple(int(x) for x in n)
         shape = (self.n[2], self.n[1], self.n[0])
         self.E, self.H = list(E), list(H)
@@ -102,13 +112,13 @@ class YeeOracle:
         self.g.src_nwave = int(wave.size)
 
     def step(self, nsteps=1):
-        rc = getattr(lib(), "yee_oracle_run_" + _SUF[self.dtype])(C.byref(self.g), C.c_longlong(self.t), C.c_int(nsteps))
+        rc = getattr(lib(), "yee_oracle_run_" + self.suffix)(C.byref(self.g), C.c_longlong(self.t), C.c_int(nsteps))
         if rc != 0:
             raise ValueError("yee_oracle_run rejected its arguments")
         self.t += nsteps
 
     def e_half(self):
-        getattr(lib(), "yee_oracle_e_half_" + _SUF[self.dtype])(C.byref(self.g))
+        getattr(lib(), "yee_oracle_e_half_" + self.suffix)(C.byref(self.g))
 
     def h_half(self):
-        getattr(lib(), "yee_oracle_h_half_" + _SUF[self.dtype])(C.byref(self.g))
+        getattr(lib(), "yee_oracle_h_half_" + self.suffix)(C.byref(self.g))

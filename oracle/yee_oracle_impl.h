@@ -6,6 +6,8 @@
  *   REAL   = float | double
  *   FN(x)  = x##_f32 | x##_f64
  * and holds literal triple loops, one statement per rounded operation.
+ *   STORE(x) = x for the f32 / f64 builds; the f16-storage build (row f1) rounds every value it
+ *   stores to IEEE binary16, nearest-even, and keeps it in a float array.
  *
  * Index convention: idx = i + nx*(j + ny*k), x fastest.
  */
@@ -42,7 +44,7 @@ static void FN(e_half)(const FN(yee_grid) *g)
                     const REAL keep = g->ca[0] ? (REAL)(g->ca[0][p] * Ex[p]) : Ex[p];
                     const REAL cb = g->cb[0] ? g->cb[0][p] : g->cb_scalar;
                     const REAL gain = cb * curl;
-                    Ex[p] = keep + gain;
+                    Ex[p] = STORE(keep + gain);
                 }
                 /* E_y:  (Hx - Hx[k-1])/dz - (Hz - Hz[i-1])/dx */
                 if (!(wall_z || wall_x)) {
@@ -54,7 +56,7 @@ static void FN(e_half)(const FN(yee_grid) *g)
                     const REAL keep = g->ca[1] ? (REAL)(g->ca[1][p] * Ey[p]) : Ey[p];
                     const REAL cb = g->cb[1] ? g->cb[1][p] : g->cb_scalar;
                     const REAL gain = cb * curl;
-                    Ey[p] = keep + gain;
+                    Ey[p] = STORE(keep + gain);
                 }
                 /* E_z:  (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy */
                 if (!(wall_x || wall_y)) {
@@ -66,7 +68,7 @@ static void FN(e_half)(const FN(yee_grid) *g)
                     const REAL keep = g->ca[2] ? (REAL)(g->ca[2][p] * Ez[p]) : Ez[p];
                     const REAL cb = g->cb[2] ? g->cb[2][p] : g->cb_scalar;
                     const REAL gain = cb * curl;
-                    Ez[p] = keep + gain;
+                    Ez[p] = STORE(keep + gain);
                 }
             }
         }
@@ -87,7 +89,7 @@ static void FN(add_source)(const FN(yee_grid) *g, long long t)
                 const size_t p = (size_t)(g->src_box[0] + ii)
                                + (size_t)nx * ((size_t)(g->src_box[1] + jj) + (size_t)ny * (size_t)(g->src_box[2] + kk));
                 const REAL inj = g->src_amp[q] * w;
-                Ec[p] = Ec[p] + inj;
+                Ec[p] = STORE(Ec[p] + inj);
             }
 }
 
@@ -126,7 +128,7 @@ static void FN(h_half)(const FN(yee_grid) *g)
                     const REAL t2 = d2 * rdz;
                     const REAL curl = t1 - t2;
                     const REAL loss = g->db[0] * curl;
-                    Hx[p] = Hx[p] - loss;
+                    Hx[p] = STORE(Hx[p] - loss);
                 }
                 /* H_y -= db_y * [ (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx ] */
                 {
@@ -136,7 +138,7 @@ static void FN(h_half)(const FN(yee_grid) *g)
                     const REAL t2 = d2 * rdx;
                     const REAL curl = t1 - t2;
                     const REAL loss = g->db[1] * curl;
-                    Hy[p] = Hy[p] - loss;
+                    Hy[p] = STORE(Hy[p] - loss);
                 }
                 /* H_z -= db_z * [ (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy ] */
                 {
@@ -146,7 +148,7 @@ static void FN(h_half)(const FN(yee_grid) *g)
                     const REAL t2 = d2 * rdy;
                     const REAL curl = t1 - t2;
                     const REAL loss = g->db[2] * curl;
-                    Hz[p] = Hz[p] - loss;
+                    Hz[p] = STORE(Hz[p] - loss);
                 }
             }
         }

@@ -241,3 +241,90 @@ def test_m3_weights_outside_the_table_are_skipped_and_float32_is_separately_roun
     mon.step(3)                                           # t >= nt: nothing accumulates
     assert np.array_equal(snap, mon.acc)
     assert mon.acc.dtype == np.float32
+
+
+# ------------------------------------------------------------------------------------------------
+# f1: f16 field storage with f32 arithmetic (oracle build "_h16")
+# ------------------------------------------------------------------------------------------------
+def _h16_inputs(n, seed, boundary, coef):
+    rng = np.random.default_rng(seed)
+    shape = (n[2], n[1], n[0])
+    r16 = lambda a: a.astype(np.float16).astype(np.float32)
+    E = [r16(rng.uniform(-1, 1, shape)) for _ in range(3)]
+    H = [r16(rng.uniform(-1, 1, shape)) for _ in range(3)]
+    ca = [rng.uniform(0.9, 1.0, shape).astype(np.float32) for _ in range(3)] if coef else None
+    cb = [rng.uniform(0.05, 0.3, shape).astype(np.float32) for _ in range(3)] if coef else None
+    return E, H, ca, cb
+
+
+@pytest.mark.parametrize("boundary", [(PEC, PEC, PEC), (PERIODIC, PEC, PERIODIC)])
+@pytest.mark.parametrize("coef", [False, True])
+def test_h1_each_half_step_is_the_f32_half_step_rounded_by_numpy(boundary, coef):
+    """One half-step of the f16-storage build = the (pinned) f32 half-step followed by numpy's own binary16 rounding."""
+    n, d, dt = (9, 7, 6), (1.0, 0.8, 1.3), 0.3
+    E, H, ca, cb = _h16_inputs(n, 11, boundary, coef)
+    E2, H2 = [a.copy() for a in E], [a.copy() for a in H]
+    y16 = YeeOracle(n, d, dt, boundary, E, H, ca, cb, db=(0.3, 0.25, 0.2), storage="f16")
+    y32 = YeeOracle(n, d, dt, boundary, E2, H2, ca, cb, db=(0.3, 0.25, 0.2))
+    y16.e_half()
+    y32.e_half()
+    for a, b in zip(E, E2):
+        assert np.array_equal(a, b.astype(np.float16).astype(np.float32))
+    assert any(not np.array_equal(a, b) for a, b in zip(E, E2))          # the rounding does something
+    for a, b in zip(E, E2):                                                # continue from the rounded state on both sides
+        b[:] = a
+    y16.h_half()
+    y32.h_half()
+    for a, b in zip(H, H2):
+        assert np.array_equal(a, b.astype(np.float16).astype(np.float32))
+
+
+def test_h2_exactly_representable_run_equals_the_f32_run():
+    """Small dyadic data, d = 1, dt = 1/2: every intermediate value of a few steps is a binary16 number, so storage
+    rounding is the identity and the two builds agree bit for bit (and the f32 build is pinned by P9's exact rationals)."""
+    n, d, dt = (6, 5, 4), (1.0, 1.0, 1.0), 0.5
+    rng = np.random.default_rng(2)
+    shape = (n[2], n[1], n[0])
+    E = [rng.integers(-4, 5, shape).astype(np.float32) / 4 for _ in range(3)]
+    H = [rng.integers(-4, 5, shape).astype(np.float32) / 4 for _ in range(3)]
+    E2, H2 = [a.copy() for a in E], [a.copy() for a in H]
+    amp = np.ones((1, 1, 1), np.float32)
+    wave = np.array([0.5, 0.25, -0.5], np.float32)
+    y16 = YeeOracle(n, d, dt, (PEC, PERIODIC, PEC), E, H, storage="f16")
+    y32 = YeeOracle(n, d, dt, (PEC, PERIODIC, PEC), E2, H2)
+    for y in (y16, y32):
+        y.set_source(2, (2, 2, 1, 1, 1, 1), amp, wave)
+        y.step(3)          # values stay multiples of 2^-8 below 2^4: 11 significant bits suffice
+    for a, b in zip(E + H, E2 + H2):
+        assert np.array_equal(a, b)
+
+
+def test_h3_source_add_is_rounded_and_error_stays_at_the_binary16_level():
+    n, d = (12, 10, 8), (1.0, 1.0, 1.0)
+    dt = 0.5 / math.sqrt(3)
+    E, H, _, _ = _h16_inputs(n, 5, (PEC,) * 3, False)
+    E64, H64 = [a.astype(np.float64) for a in E], [a.astype(np.float64) for a in H]
+    amp = np.full((1, 1, 1), 0.3337, np.float32)
+    wave = np.array([0.7771], np.float32)
+    y16 = YeeOracle(n, d, dt, (PEC,) * 3, E, H, storage="f16")
+    y16.set_source(0, (5, 5, 4, 1, 1, 1), amp, wave)
+    before = [a.copy() for a in E]
+    Hb = [a.copy() for a in H]
+    y16.step(1)
+    # re-derive E_x at the source cell: f32 update rounded, then f32 add of the rounded product, rounded again
+    ye = YeeOracle(n, d, dt, (PEC,) * 3, before, Hb)
+    ye.e_half()
+    e1 = np.float32(np.float16(before[0][4, 5, 5]))
+    inj = np.float32(amp[0, 0, 0] * wave[0])
+    assert E[0][4, 5, 5] == np.float32(np.float16(e1 + inj))
+    for a in E + H:
+        assert np.array_equal(a, a.astype(np.float16).astype(np.float32))
+    # 40 steps against f64: relative error of a few binary16 ulps per step, nothing worse
+    y64 = YeeOracle(n, d, dt, (PEC,) * 3, E64, H64)
+    y64.set_source(0, (5, 5, 4, 1, 1, 1), amp.astype(np.float64), wave.astype(np.float64))
+    y64.step(1)
+    y16.step(40)
+    y64.step(40)
+    scale = max(float(np.abs(a).max()) for a in E64 + H64)
+    err = max(float(np.abs(a - b).max()) for a, b in zip(E + H, E64 + H64))
+    assert 1e-5 * scale < err < 40 * 2.0 ** -10 * scale

@@ -77,6 +77,17 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
  * FDTD_EINVAL: NULL or misaligned pointer.   (the six arrays of eq. (1) and its siblings) */
 int fdtd_set_fields(fdtd_ctx* ctx, float* const E[3], float* const H[3]);
 
+/* The same with the six field arrays stored as IEEE binary16 (row f1; section 4: the paper's engine "halves
+ * the number of bytes needed to be loaded per field value, by utilizing 16-bit floating-point representations for the
+ * field values"; reading #14).  E[3], H[3]: host arrays of DEVICE pointers to nx*ny*nz binary16 values each,
+ * same layout, 16-byte aligned, borrowed and updated in place.  Arithmetic is unchanged (f32, the same expression tree;
+ * coefficients, 1/d and source tables stay f32); every newly computed field value -- each half-step, and the source add --
+ * is rounded to binary16, nearest-even, before it is stored or used again, so the result does not depend on the schedule
+ * and equals the f16-storage build of the oracle bit for bit.  Runs FDTD_KERNEL_NAIVE and FDTD_KERNEL_SYSTOLIC (tile
+ * 31x15x7; a periodic axis or nx % 8 != 0 uses the padded working copy); other schedules return FDTD_EINVAL from
+ * fdtd_step.  fdtd_load_fields / fdtd_get_fields then copy binary16 arrays (pass the pointers cast to float*). */
+int fdtd_set_fields_f16(fdtd_ctx* ctx, void* const E[3], void* const H[3]);
+
 /* Copy initial data from six caller arrays (HOST or device pointers, same layout) into the bound field
  * buffers, asynchronously on the ctx stream.  NULL entries are skipped.  This is the host-buffer entry of
  * the end-to-end path (bench.py `e2e`).  FDTD_ESTATE before fdtd_set_fields. */

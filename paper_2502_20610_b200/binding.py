@@ -23,6 +23,7 @@ _PROTOS = {
     "fdtd_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float,
                               C.POINTER(C.c_int), C.c_void_p]),
     "fdtd_set_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "fdtd_set_fields_f16": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "fdtd_load_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "fdtd_set_coeffs": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_float)]),
     "fdtd_set_source": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
@@ -136,16 +137,20 @@ class Fdtd:
         if rc != OK:
             raise FdtdError(rc, self._lib.fdtd_last_error(self._h).decode())
 
-    def _check_tensors(self, ts):
+    def _check_tensors(self, ts, dtype=None):
         import torch
         shape = (self.n[2], self.n[1], self.n[0])
         for t in ts:
-            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and tuple(t.shape) == shape, "bad field tensor"
+            assert t.is_cuda and t.dtype == (dtype or torch.float32) and t.is_contiguous() and tuple(t.shape) == shape, "bad field tensor"
 
     def set_fields(self, E, H):
-        self._check_tensors(list(E) + list(H))
+        """Six float32 CUDA tensors, or six float16 CUDA tensors (binary16 field storage, fdtd_set_fields_f16)."""
+        import torch
+        half = E[0].dtype == torch.float16
+        self._check_tensors(list(E) + list(H), torch.float16 if half else torch.float32)
         self._keep = [list(E), list(H)] + self._keep[2:]
-        self._check(self._lib.fdtd_set_fields(self._h, _ptr3(E), _ptr3(H)))
+        fn = self._lib.fdtd_set_fields_f16 if half else self._lib.fdtd_set_fields
+        self._check(fn(self._h, _ptr3(E), _ptr3(H)))
 
     def load_fields(self, E, H):
         """Copy initial data from host (pinned numpy / CPU tensors) or device arrays into the bound buffers."""

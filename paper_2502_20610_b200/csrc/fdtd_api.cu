@@ -34,6 +34,7 @@ struct fdtd_ctx {
     bool use_reg;     // resolved: the register-resident kernel (tile 31x15x7) runs
     bool use_tma;     // resolved: its TMA-staged version runs
     bool tma_by8;     // resolved: the 31x7x7 build of it (two CTAs per SM)
+    bool tma_h16;     // resolved: the binary16-field-storage build of it (g.fld16)
     // resolved: the TMA kernel runs on a padded working copy of the grid (periodic axis or nx % 4 != 0)
     bool use_pad;
     PadGeom pg;
@@ -158,14 +159,19 @@ int resolve_systolic(fdtd_ctx* c)
     }
     c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
     c->tma_by8 = c->which == FDTD_KERNEL_SYSTOLIC && N[0] == 31 && N[1] == 7 && N[2] == 7;
+    c->tma_h16 = c->g.fld16 != 0;
+    if (c->tma_h16 && !(c->which == FDTD_KERNEL_SYSTOLIC && N[0] == 31 && N[1] == 15 && N[2] == 7))
+        return fail(c, FDTD_EINVAL, "binary16 field storage runs FDTD_KERNEL_NAIVE or FDTD_KERNEL_SYSTOLIC with tile 31x15x7");
     c->use_tma = (c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->dbg_no_tma) || c->tma_by8;
-    c->use_pad = c->use_tma && (c->g.per[0] || c->g.per[1] || c->g.per[2] || c->g.n[0] % 4 != 0);
+    c->use_pad = c->use_tma && (c->g.per[0] || c->g.per[1] || c->g.per[2] || c->g.n[0] % (c->tma_h16 ? 8 : 4) != 0);
     int found = -1;
     int per_sm = 0;
     if (c->use_tma) {
-        cudaError_t e = c->tma_by8 ? systolic_tma_prepare_by8(want_coef, &per_sm) : systolic_tma_prepare(want_coef, &per_sm);
+        cudaError_t e = c->tma_h16   ? systolic_tma_prepare_h16(want_coef, &per_sm)
+                        : c->tma_by8 ? systolic_tma_prepare_by8(want_coef, &per_sm)
+                                     : systolic_tma_prepare(want_coef, &per_sm);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
-        c->smem = c->tma_by8 ? systolic_tma_smem_by8(want_coef) : systolic_tma_smem(want_coef);
+        c->smem = c->tma_h16 ? systolic_tma_smem_h16(want_coef) : c->tma_by8 ? systolic_tma_smem_by8(want_coef) : systolic_tma_smem(want_coef);
     } else if (c->use_reg) {
         cudaError_t e = systolic_reg_prepare(want_coef, &per_sm);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
@@ -215,7 +221,7 @@ int resolve_systolic(fdtd_ctx* c)
             c->pg.G[a] = c->g.per[a] ? c->T : 0;
             c->pg.m[a] = c->g.n[a] + 2 * c->pg.G[a];
         }
-        c->pg.ldx = (c->pg.m[0] + 3) / 4 * 4;
+        c->pg.ldx = c->tma_h16 ? (c->pg.m[0] + 7) / 8 * 8 : (c->pg.m[0] + 3) / 4 * 4;   // rows are multiples of 16 bytes
         cells = c->pg.ldx * c->pg.m[1] * c->pg.m[2];
         if (c->pg.m[0] > (1 << 16) || c->pg.m[1] > (1 << 16) || c->pg.m[2] > (1 << 16) || cells >= (1ll << 40))
             return fail(c, FDTD_EINVAL, "padded working grid too large; use a smaller temporal depth");
@@ -242,8 +248,10 @@ GridParams work_grid(const fdtd_ctx* c, long long* ldx)
     *ldx = c->g.n[0];
     if (!c->use_pad) return g;
     for (int a = 0; a < 3; ++a) {
-        g.E[a] = c->pad_fld + c->pad_stride * a;
-        g.H[a] = c->pad_fld + c->pad_stride * (3 + a);
+        // the padded field arrays hold elements of the storage type (binary16 arrays sit behind float pointers)
+        const size_t es = c->g.fld16 ? 2 : 4;
+        g.E[a] = reinterpret_cast<float*>(reinterpret_cast<char*>(c->pad_fld) + es * (size_t)c->pad_stride * a);
+        g.H[a] = reinterpret_cast<float*>(reinterpret_cast<char*>(c->pad_fld) + es * (size_t)c->pad_stride * (3 + a));
         g.ca[a] = c->pad_coef ? c->pad_coef + c->pad_stride * a : nullptr;
         g.cb[a] = c->pad_coef ? c->pad_coef + c->pad_stride * (3 + a) : nullptr;
         g.n[a] = c->pg.m[a];
@@ -288,9 +296,10 @@ int ensure_tmaps(fdtd_ctx* c)
         if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) return fail(c, FDTD_ECUDA, "cuTensorMapEncodeTiled is not available in this driver");
         encode = (EncodeTiledFn)fn;
     }
-    int box[3][3];
-    if (c->tma_by8) systolic_tma_boxes_by8(box);
-    else systolic_tma_boxes(box);
+    int box_fld[3][3], box_coef[3][3];
+    if (c->tma_h16) systolic_tma_boxes_h16(box_fld, box_coef);
+    else if (c->tma_by8) systolic_tma_boxes_by8(box_fld, box_coef);
+    else systolic_tma_boxes(box_fld, box_coef);
     long long ldx = 0;
     const GridParams wg = work_grid(c, &ldx);
     const void* arr[12];
@@ -303,10 +312,11 @@ int ensure_tmaps(fdtd_ctx* c)
     static_assert(sizeof(CUtensorMap) * 36 == sizeof(TmaMaps), "TmaMaps layout");
     CUtensorMap* host = reinterpret_cast<CUtensorMap*>(c->tmaps.bytes);
     memset(c->tmaps.bytes, 0, sizeof c->tmaps.bytes);
-    const cuuint64_t nbytes = (cuuint64_t)ldx * wg.n[1] * wg.n[2] * 4u;
+    const cuuint64_t ncells = (cuuint64_t)ldx * wg.n[1] * wg.n[2];
     // arrays first..first+count-1 at one positive stride (multiple of 16 bytes, no overlap)? -> the stride, else 0
     auto uniform_stride = [&](int first, int count) -> cuuint64_t {
         if (!arr[first] || c->dbg_no_group) return 0;
+        const cuuint64_t nbytes = ncells * ((first < 6 && c->g.fld16) ? 2u : 4u);
         const char* b0 = (const char*)arr[first];
         const char* b1 = (const char*)arr[first + 1];
         if (b1 <= b0) return 0;
@@ -316,14 +326,17 @@ int ensure_tmaps(fdtd_ctx* c)
             if ((const char*)arr[first + a] != b0 + d * a) return 0;
         return d;
     };
-    auto encode_maps = [&](CUtensorMap* dst, const void* base, int narr, cuuint64_t astride) -> int {
+    auto encode_maps = [&](CUtensorMap* dst, const void* base, int narr, cuuint64_t astride, bool fld) -> int {
         // extents are the logical grid (elements beyond it are delivered as zeros), strides follow the row pitch
+        const bool h16 = fld && c->g.fld16;
+        const cuuint64_t es = h16 ? 2u : 4u;
+        const int (*box)[3] = fld ? box_fld : box_coef;
         const cuuint64_t dims[4] = {(cuuint64_t)wg.n[0], (cuuint64_t)wg.n[1], (cuuint64_t)wg.n[2], (cuuint64_t)narr};
-        const cuuint64_t strides[3] = {(cuuint64_t)ldx * 4u, (cuuint64_t)ldx * wg.n[1] * 4u, astride};
+        const cuuint64_t strides[3] = {(cuuint64_t)ldx * es, (cuuint64_t)ldx * wg.n[1] * es, astride};
         const cuuint32_t estr[4] = {1, 1, 1, 1};
         for (int f = 0; f < 3; ++f) {
             const cuuint32_t b[4] = {(cuuint32_t)box[f][0], (cuuint32_t)box[f][1], (cuuint32_t)box[f][2], (cuuint32_t)narr};
-            const CUresult r = encode(dst + f, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, narr > 1 ? 4 : 3, const_cast<void*>(base), dims, strides, b, estr,
+            const CUresult r = encode(dst + f, h16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, narr > 1 ? 4 : 3, const_cast<void*>(base), dims, strides, b, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) {
@@ -345,13 +358,13 @@ int ensure_tmaps(fdtd_ctx* c)
         cuuint64_t da = 0, db = 0;
         if (d) {
             c->tma_group[g] = 1;
-            rc = encode_maps(dst, arr[first[g]], count[g], d);
+            rc = encode_maps(dst, arr[first[g]], count[g], d, g < 2);
         } else if (g == 2 && (da = uniform_stride(6, 3)) && (db = uniform_stride(9, 3))) {
             c->tma_group[g] = 2;
-            rc = encode_maps(dst, arr[6], 3, da);
-            if (rc == FDTD_OK) rc = encode_maps(dst + 9, arr[9], 3, db);
+            rc = encode_maps(dst, arr[6], 3, da, false);
+            if (rc == FDTD_OK) rc = encode_maps(dst + 9, arr[9], 3, db, false);
         } else {
-            for (int a = 0; a < count[g] && rc == FDTD_OK; ++a) rc = encode_maps(dst + a * 3, arr[first[g] + a], 1, 0);
+            for (int a = 0; a < count[g] && rc == FDTD_OK; ++a) rc = encode_maps(dst + a * 3, arr[first[g] + a], 1, 0, g < 2);
         }
         if (rc != FDTD_OK) return rc;
     }
@@ -486,7 +499,7 @@ int step_systolic(fdtd_ctx* c, int n)
             pc.usr[a] = const_cast<float*>(c->g.ca[a]);
             pc.usr[3 + a] = const_cast<float*>(c->g.cb[a]);
         }
-        pf.ext = c->pad_fld; pf.stride = c->pad_stride; pf.narr = 6;
+        pf.ext = c->pad_fld; pf.stride = c->pad_stride; pf.narr = 6; pf.elem16 = c->g.fld16;
         pc.ext = c->pad_coef; pc.stride = c->pad_stride; pc.narr = 6;
         if (c->pad_coef && !c->pad_coef_valid) {           // constants of the run: copied (with their images) once
             cudaError_t e = launch_pad_copy_in(c->pg, pc, c->stream);
@@ -577,7 +590,8 @@ int step_systolic(fdtd_ctx* c, int n)
         cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
-        e = c->tma_by8   ? launch_systolic_tma_by8(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
+        e = c->tma_h16   ? launch_systolic_tma_h16(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
+            : c->tma_by8 ? launch_systolic_tma_by8(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->use_tma ? launch_systolic_tma(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream)
                          : launch_systolic(c->cfg_idx, P, ctas, c->stream);
@@ -662,6 +676,7 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->use_reg = false;
     c->use_tma = false;
     c->tma_by8 = false;
+    c->tma_h16 = false;
     c->use_pad = false;
     c->pad_fld = c->pad_coef = nullptr;
     c->pad_stride = 0;
@@ -741,6 +756,27 @@ int fdtd_set_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
         c->g.E[a] = E[a];
         c->g.H[a] = H[a];
     }
+    if (c->g.fld16) c->resolved = false;     // the storage type selects the kernel build
+    c->g.fld16 = 0;
+    c->fields_set = true;
+    c->tmaps_valid = false;
+    return FDTD_OK;
+}
+
+int fdtd_set_fields_f16(fdtd_ctx* c, void* const E[3], void* const H[3])
+{
+    if (!c) return FDTD_EINVAL;
+    if (!E || !H) return fail(c, FDTD_EINVAL, "fdtd_set_fields_f16: NULL array");
+    for (int a = 0; a < 3; ++a) {
+        if (!E[a] || !H[a]) return fail(c, FDTD_EINVAL, "fdtd_set_fields_f16: NULL field pointer");
+        if (!aligned16(E[a]) || !aligned16(H[a])) return fail(c, FDTD_EINVAL, "fdtd_set_fields_f16: pointers must be 16-byte aligned");
+    }
+    for (int a = 0; a < 3; ++a) {
+        c->g.E[a] = static_cast<float*>(E[a]);     // binary16 arrays behind float pointers; g.fld16 tells the kernels
+        c->g.H[a] = static_cast<float*>(H[a]);
+    }
+    if (!c->g.fld16) c->resolved = false;
+    c->g.fld16 = 1;
     c->fields_set = true;
     c->tmaps_valid = false;
     return FDTD_OK;
@@ -751,7 +787,7 @@ int fdtd_load_fields(fdtd_ctx* c, const float* const E[3], const float* const H[
     if (!c) return FDTD_EINVAL;
     DeviceGuard guard(c);
     if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_load_fields before fdtd_set_fields");
-    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * sizeof(float);
+    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * (c->g.fld16 ? 2 : sizeof(float));
     for (int a = 0; a < 3; ++a) {
         if (E && E[a] && E[a] != c->g.E[a]) {
             cudaError_t e = cudaMemcpyAsync(c->g.E[a], E[a], bytes, cudaMemcpyDefault, c->stream);
@@ -884,7 +920,7 @@ int fdtd_get_fields(fdtd_ctx* c, float* const E[3], float* const H[3])
     if (rc != FDTD_OK) return rc;
     if (!E && !H) return FDTD_OK;
     if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_get_fields before fdtd_set_fields");
-    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * sizeof(float);
+    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * c->g.n[2] * (c->g.fld16 ? 2 : sizeof(float));
     for (int a = 0; a < 3; ++a) {
         if (E && E[a] && E[a] != c->g.E[a]) {
             cudaError_t e = cudaMemcpyAsync(E[a], c->g.E[a], bytes, cudaMemcpyDefault, c->stream);

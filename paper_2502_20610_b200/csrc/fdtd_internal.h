@@ -29,15 +29,22 @@ cudaError_t launch_systolic_reg(int coef, const SysParams& p, int ctas, cudaStre
 // implemented in systolic_tma.cu: the TMA-staged systolic kernel (PEC grids, nx % 4 == 0), tile 31x15x7
 size_t systolic_tma_smem(int coef);
 int systolic_tma_threads();
-void systolic_tma_boxes(int box[3][3]);   // TMA box extents (x,y,z) of the z-plane, y-row and x-column shell pieces
+void systolic_tma_boxes(int fld[3][3], int coef[3][3]);   // TMA box extents (x,y,z) of the z-plane, y-row and x-column shell pieces
 cudaError_t systolic_tma_prepare(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_tma(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
 // implemented in systolic_tma_by8.cu: the same kernel for tile 31x7x7 (box 32x8x8), two CTAs per SM
 size_t systolic_tma_smem_by8(int coef);
 int systolic_tma_threads_by8();
-void systolic_tma_boxes_by8(int box[3][3]);
+void systolic_tma_boxes_by8(int fld[3][3], int coef[3][3]);
 cudaError_t systolic_tma_prepare_by8(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_tma_by8(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
+
+// implemented in systolic_tma_h16.cu: the same kernel for binary16 field storage (GridParams::fld16), tile 31x15x7
+size_t systolic_tma_smem_h16(int coef);
+int systolic_tma_threads_h16();
+void systolic_tma_boxes_h16(int fld[3][3], int coef[3][3]);
+cudaError_t systolic_tma_prepare_h16(int coef, int* blocks_per_sm);
+cudaError_t launch_systolic_tma_h16(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
 
 // implemented in pad_kernels.cu: copies between the caller's arrays and the padded working copy (periodic images)
 cudaError_t launch_pad_copy_in(const PadGeom& g, const PadArrays& a, cudaStream_t st);     // all padded cells <- images

@@ -18,6 +18,7 @@ struct GridParams {
     float* H[3];
     const float* ca[3];  // all NULL or all set
     const float* cb[3];  // all NULL or all set
+    int fld16;           // 1: E and H point to IEEE binary16 arrays (row f1); arithmetic stays f32
     int n[3];
     int per[3];          // 1 = periodic axis
     float rd[3];         // (float)(1.0 / (double)d_a)                    (reading #2)
@@ -83,8 +84,9 @@ struct PadGeom {
 struct PadArrays {
     float* usr[6];        // the caller's arrays (n[0]*n[1]*n[2] each)
     float* ext;           // narr padded arrays of ldx*m[1]*m[2] elements at a uniform stride
-    long long stride;
+    long long stride;     // in elements
     int narr;
+    int elem16;           // 1: the arrays hold binary16 elements (usr / ext are then __half arrays behind float pointers)
 };
 
 // Running-DFT monitor on one plane of the grid (PAPER.md:106 names outputs as what real runs carry;

@@ -13,6 +13,8 @@
 //
 // Arithmetic: the expression tree of eq. (1) with coefficients, one rounding per operation when compiled
 // with -fmad=false (then bit-identical to the fp32 oracle); the default build lets ptxas contract mul+add.
+#include <cuda_fp16.h>
+
 #include "fdtd_internal.h"
 #include "yee_update.h"
 
@@ -44,6 +46,40 @@ __device__ __forceinline__ void stv(float* __restrict__ p, const float (&v)[VEC]
     }
 }
 
+// binary16 field storage (row f1): exact conversion to f32 on load, round-to-nearest-even on store
+template <int VEC>
+__device__ __forceinline__ void ldv(const __half* __restrict__ p, float (&v)[VEC])
+{
+    if constexpr (VEC == 4) {
+        const uint2 t = *reinterpret_cast<const uint2*>(p);
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&t.x));
+        const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&t.y));
+        v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+    } else {
+#pragma unroll
+        for (int q = 0; q < VEC; ++q) v[q] = __half2float(p[q]);
+    }
+}
+
+template <int VEC>
+__device__ __forceinline__ void stv(__half* __restrict__ p, const float (&v)[VEC])
+{
+    if constexpr (VEC == 4) {
+        const __half2 a = __floats2half2_rn(v[0], v[1]), b = __floats2half2_rn(v[2], v[3]);
+        uint2 t;
+        t.x = *reinterpret_cast<const unsigned*>(&a);
+        t.y = *reinterpret_cast<const unsigned*>(&b);
+        *reinterpret_cast<uint2*>(p) = t;
+    } else {
+#pragma unroll
+        for (int q = 0; q < VEC; ++q) p[q] = __float2half_rn(v[q]);
+    }
+}
+__device__ __forceinline__ float ld1(const float* p) { return *p; }
+__device__ __forceinline__ float ld1(const __half* p) { return __half2float(*p); }
+__device__ __forceinline__ void st1(float* p, float v) { *p = v; }
+__device__ __forceinline__ void st1(__half* p, float v) { *p = __float2half_rn(v); }
+
 template <int VEC>
 __device__ __forceinline__ void zerov(float (&v)[VEC])
 {
@@ -63,7 +99,7 @@ __device__ __forceinline__ float h_update(float h, float ec_p, float ec, float e
     return yee_h_update(h, ec_p, ec, eb_p, eb, rdb, rdc, db);
 }
 
-template <int VEC>
+template <int VEC, typename FT>
 __global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__ GridParams g)
 {
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
@@ -81,9 +117,12 @@ __global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__
     const long long xm_off = (i0 > 0) ? -1 : (long long)(nx - 1);
     const float rdx = g.rd[0], rdy = g.rd[1], rdz = g.rd[2];
     const bool has_ca = g.ca[0] != nullptr, has_cb = g.cb[0] != nullptr;
-    const float* __restrict__ Hx = g.H[0];
-    const float* __restrict__ Hy = g.H[1];
-    const float* __restrict__ Hz = g.H[2];
+    const FT* __restrict__ Hx = reinterpret_cast<const FT*>(g.H[0]);
+    const FT* __restrict__ Hy = reinterpret_cast<const FT*>(g.H[1]);
+    const FT* __restrict__ Hz = reinterpret_cast<const FT*>(g.H[2]);
+    FT* __restrict__ Ex = reinterpret_cast<FT*>(g.E[0]);
+    FT* __restrict__ Ey = reinterpret_cast<FT*>(g.E[1]);
+    FT* __restrict__ Ez = reinterpret_cast<FT*>(g.E[2]);
 
     float hx_m[VEC], hy_m[VEC];   // H_x, H_y one plane back in z
     if (k0 > 0 || perz) {
@@ -103,11 +142,11 @@ __global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__
         ldv<VEC>(Hz + p, hz);
         ldv<VEC>(Hz + p + ym_off, hz_ym);
         ldv<VEC>(Hx + p + ym_off, hx_ym);
-        const float hz_xm = Hz[p + xm_off];
-        const float hy_xm = Hy[p + xm_off];
-        ldv<VEC>(g.E[0] + p, ex);
-        ldv<VEC>(g.E[1] + p, ey);
-        ldv<VEC>(g.E[2] + p, ez);
+        const float hz_xm = ld1(Hz + p + xm_off);
+        const float hy_xm = ld1(Hy + p + xm_off);
+        ldv<VEC>(Ex + p, ex);
+        ldv<VEC>(Ey + p, ey);
+        ldv<VEC>(Ez + p, ez);
         float ca0[VEC], ca1[VEC], ca2[VEC], cb0[VEC], cb1[VEC], cb2[VEC];
         if (has_ca) { ldv<VEC>(g.ca[0] + p, ca0); ldv<VEC>(g.ca[1] + p, ca1); ldv<VEC>(g.ca[2] + p, ca2); }
         if (has_cb) { ldv<VEC>(g.cb[0] + p, cb0); ldv<VEC>(g.cb[1] + p, cb1); ldv<VEC>(g.cb[2] + p, cb2); }
@@ -126,15 +165,15 @@ __global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__
                 ez[v] = e_update(ez[v], hy[v], hy_x, hx[v], hx_ym[v], rdx, rdy, has_ca, has_ca ? ca2[v] : 1.0f,
                                  has_cb ? cb2[v] : g.cb_scalar);
         }
-        stv<VEC>(g.E[0] + p, ex);
-        stv<VEC>(g.E[1] + p, ey);
-        stv<VEC>(g.E[2] + p, ez);
+        stv<VEC>(Ex + p, ex);
+        stv<VEC>(Ey + p, ey);
+        stv<VEC>(Ez + p, ez);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) { hx_m[v] = hx[v]; hy_m[v] = hy[v]; }
     }
 }
 
-template <int VEC>
+template <int VEC, typename FT>
 __global__ void __launch_bounds__(kThreads) h_half_naive(const __grid_constant__ GridParams g)
 {
     const int nx = g.n[0], ny = g.n[1], nz = g.n[2];
@@ -154,9 +193,12 @@ __global__ void __launch_bounds__(kThreads) h_half_naive(const __grid_constant__
     const bool ghost_x = last_x && !perx;
     const long long xp_off = last_x ? (long long)VEC - nx : (long long)VEC;
     const float rdx = g.rd[0], rdy = g.rd[1], rdz = g.rd[2];
-    const float* __restrict__ Ex = g.E[0];
-    const float* __restrict__ Ey = g.E[1];
-    const float* __restrict__ Ez = g.E[2];
+    const FT* __restrict__ Ex = reinterpret_cast<const FT*>(g.E[0]);
+    const FT* __restrict__ Ey = reinterpret_cast<const FT*>(g.E[1]);
+    const FT* __restrict__ Ez = reinterpret_cast<const FT*>(g.E[2]);
+    FT* __restrict__ Hx = reinterpret_cast<FT*>(g.H[0]);
+    FT* __restrict__ Hy = reinterpret_cast<FT*>(g.H[1]);
+    FT* __restrict__ Hz = reinterpret_cast<FT*>(g.H[2]);
 
     float ex[VEC], ey[VEC];
     ldv<VEC>(Ex + cell0 + plane * k0, ex);
@@ -182,11 +224,11 @@ __global__ void __launch_bounds__(kThreads) h_half_naive(const __grid_constant__
             ldv<VEC>(Ez + p + yp_off, ez_yp);
             ldv<VEC>(Ex + p + yp_off, ex_yp);
         }
-        const float ey_xp = ghost_x ? 0.0f : Ey[p + xp_off];
-        const float ez_xp = ghost_x ? 0.0f : Ez[p + xp_off];
-        ldv<VEC>(g.H[0] + p, hx);
-        ldv<VEC>(g.H[1] + p, hy);
-        ldv<VEC>(g.H[2] + p, hz);
+        const float ey_xp = ghost_x ? 0.0f : ld1(Ey + p + xp_off);
+        const float ez_xp = ghost_x ? 0.0f : ld1(Ez + p + xp_off);
+        ldv<VEC>(Hx + p, hx);
+        ldv<VEC>(Hy + p, hy);
+        ldv<VEC>(Hz + p, hz);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             const float ey_x = (v == VEC - 1) ? ey_xp : ey[v < VEC - 1 ? v + 1 : v];
@@ -195,27 +237,28 @@ __global__ void __launch_bounds__(kThreads) h_half_naive(const __grid_constant__
             hy[v] = h_update(hy[v], ex_p[v], ex[v], ez_x, ez[v], rdz, rdx, g.db[1]);       // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
             hz[v] = h_update(hz[v], ey_x, ey[v], ex_yp[v], ex[v], rdx, rdy, g.db[2]);      // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
         }
-        stv<VEC>(g.H[0] + p, hx);
-        stv<VEC>(g.H[1] + p, hy);
-        stv<VEC>(g.H[2] + p, hz);
+        stv<VEC>(Hx + p, hx);
+        stv<VEC>(Hy + p, hy);
+        stv<VEC>(Hz + p, hz);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) { ex[v] = ex_p[v]; ey[v] = ey_p[v]; }
     }
 }
 
 // E_comp[box] += amp[q] * wave[t]   (reading #6)
+template <typename FT>
 __global__ void source_kernel(const __grid_constant__ GridParams g, float w)
 {
     const int ni = g.src_box[3], nj = g.src_box[4], nk = g.src_box[5];
     const long long total = (long long)ni * nj * nk;
-    float* __restrict__ Ec = g.E[g.src_comp];
+    FT* __restrict__ Ec = reinterpret_cast<FT*>(g.E[g.src_comp]);
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
         const int ii = (int)(q % ni);
         const int jj = (int)((q / ni) % nj);
         const int kk = (int)(q / ((long long)ni * nj));
         const long long p = (long long)(g.src_box[0] + ii) + (long long)g.n[0] * ((long long)(g.src_box[1] + jj) + (long long)g.n[1] * (g.src_box[2] + kk));
         const float inj = g.src_amp[q] * w;
-        Ec[p] = Ec[p] + inj;
+        st1(Ec + p, ld1(Ec + p) + inj);
     }
 }
 
@@ -229,19 +272,25 @@ dim3 naive_grid(const GridParams& g, int vec)
 
 cudaError_t launch_e_half_naive(const GridParams& g, cudaStream_t st)
 {
-    if (g.n[0] % 4 == 0)
-        e_half_naive<4><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
+    if (g.fld16) {
+        if (g.n[0] % 4 == 0) e_half_naive<4, __half><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
+        else e_half_naive<1, __half><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
+    } else if (g.n[0] % 4 == 0)
+        e_half_naive<4, float><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
     else
-        e_half_naive<1><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
+        e_half_naive<1, float><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
     return cudaGetLastError();
 }
 
 cudaError_t launch_h_half_naive(const GridParams& g, cudaStream_t st)
 {
-    if (g.n[0] % 4 == 0)
-        h_half_naive<4><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
+    if (g.fld16) {
+        if (g.n[0] % 4 == 0) h_half_naive<4, __half><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
+        else h_half_naive<1, __half><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
+    } else if (g.n[0] % 4 == 0)
+        h_half_naive<4, float><<<naive_grid(g, 4), kThreads, 0, st>>>(g);
     else
-        h_half_naive<1><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
+        h_half_naive<1, float><<<naive_grid(g, 1), kThreads, 0, st>>>(g);
     return cudaGetLastError();
 }
 
@@ -250,7 +299,8 @@ cudaError_t launch_source_w(const GridParams& g, float w, cudaStream_t st)
 {
     const long long total = (long long)g.src_box[3] * g.src_box[4] * g.src_box[5];
     const int blocks = (int)((total + 255) / 256 > 1184 ? 1184 : (total + 255) / 256);
-    source_kernel<<<blocks, 256, 0, st>>>(g, w);
+    if (g.fld16) source_kernel<__half><<<blocks, 256, 0, st>>>(g, w);
+    else source_kernel<float><<<blocks, 256, 0, st>>>(g, w);
     return cudaGetLastError();
 }
 
@@ -268,7 +318,8 @@ __global__ void __launch_bounds__(128) monitor_kernel(const __grid_constant__ Gr
     else if (m.axis == 1) { j = m.index; i = (int)(cell % m.n[0]); k = (int)(cell / m.n[0]); }
     else                  { k = m.index; i = (int)(cell % m.n[0]); j = (int)(cell / m.n[0]); }
     const long long off = i + (long long)g.n[0] * (j + (long long)g.n[1] * k);
-    const float v = (isH ? g.H[c] : g.E[c])[off];
+    const float* fa = isH ? g.H[c] : g.E[c];
+    const float v = g.fld16 ? __half2float(reinterpret_cast<const __half*>(fa)[off]) : fa[off];
     const float* w = (isH ? m.wH : m.wE) + t * m.F * 2;
     float* acc = m.acc + ((long long)(isH ? 3 + c : c) * m.F * 2) * m.pcells + cell;
     for (int f = 0; f < m.F; ++f) {

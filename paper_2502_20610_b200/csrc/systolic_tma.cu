@@ -47,6 +47,7 @@
 // Scope: every axis is a wall axis of the (possibly padded) grid and nx % 4 == 0 (TMA strides are
 // multiples of 16 bytes); P.g.per[] only says which low walls freeze tangential E.
 #include <cuda.h>
+#include <cuda_fp16.h>
 
 #include <type_traits>
 
@@ -87,6 +88,34 @@ constexpr int W_HPROD = NWARPS_C, W_HAUX = NWARPS_C + 1, W_EPROD = NWARPS_C + 2;
 // box starts at q0 = o0 & ~3 and is RX = 36 cells wide; r0 = o0 & 3 is where the shell begins inside a staged row
 // Box extents are chosen so that every piece is a multiple of 128 bytes: a group of arrays at uniform stride can
 // then be fetched by ONE 4-D box per piece and lands exactly where per-array 3-D boxes would put it.
+// Field storage (row f1): FDTD_FLD16 builds keep the six field arrays in IEEE binary16 (systolic_tma_h16.cu);
+// arithmetic and the on-chip copies stay f32, every newly computed value is rounded to binary16 before it is used again
+// (reading #14), so the result does not depend on the schedule.  A binary16 box needs 8 elements per 16 bytes:
+// field boxes start at o0 & ~7, are 40 cells wide, and the x column box is 8 cells wide.
+#ifdef FDTD_FLD16
+using fld_t = __half;
+constexpr int RXF = BX + 8, CWF = 8;
+__device__ __forceinline__ float fld_round(float v) { return __half2float(__float2half_rn(v)); }
+__device__ __forceinline__ float fld_get(const fld_t* p) { return __half2float(*p); }
+__device__ __forceinline__ float fld_ldcg(const float* base, long long off) { return __half2float(__ldcg(reinterpret_cast<const __half*>(base) + off)); }
+__device__ __forceinline__ void fld_stcg(float* base, long long off, float v) { __stcg(reinterpret_cast<__half*>(base) + off, __float2half_rn(v)); }
+#else
+using fld_t = float;
+constexpr int RXF = BX + 4, CWF = 4;
+__device__ __forceinline__ float fld_round(float v) { return v; }
+__device__ __forceinline__ float fld_get(const fld_t* p) { return *p; }
+__device__ __forceinline__ float fld_ldcg(const float* base, long long off) { return __ldcg(base + off); }
+__device__ __forceinline__ void fld_stcg(float* base, long long off, float v) { __stcg(base + off, v); }
+#endif
+constexpr int XMASK_F = CWF - 1;
+// staged group of the three field arrays, in elements of fld_t: [3][FZF] [3][FYF] [3][FXF]
+constexpr int FZF = RXF * BY, FYF = RXF * BZ, FXF = CWF * BY * W2;
+constexpr int F_ARR_F = (FZF + FYF + FXF) * (int)sizeof(fld_t) / 4;      // floats of staging per field array and step
+static_assert((FZF * sizeof(fld_t)) % 128 == 0 && (FYF * sizeof(fld_t)) % 128 == 0 && (FXF * sizeof(fld_t)) % 128 == 0, "TMA destinations are 128-byte aligned");
+__device__ __forceinline__ int zidxF(int a, int ly, int x) { return a * FZF + ly * RXF + x; }
+__device__ __forceinline__ int yidxF(int a, int l, int x) { return 3 * FZF + a * FYF + (l - 1) * RXF + x; }
+__device__ __forceinline__ int xidxF(int a, int ly, int l) { return 3 * (FZF + FYF) + a * FXF + ((l - 1) * BY + ly) * CWF; }
+// coefficient arrays are always f32
 constexpr int RX = BX + 4;
 constexpr int FZ = RX * BY;                  // box (36,16,1)   [y][x]      576 floats: plane l_z = 0
 constexpr int FY = RX * BZ;                  // box (36,1,8)    [z][x]      288 floats: row l_y = 0, l_z = 1..8 (8 unused)
@@ -98,15 +127,14 @@ template <int NA> __device__ __forceinline__ int yidx(int a, int l, int x) { ret
 template <int NA> __device__ __forceinline__ int xidx(int a, int ly, int l) { return NA * (FZ + FY) + a * FX + ((l - 1) * BY + ly) * 4; }
 constexpr int XPK = BY * 3 * 8;              // packed x column [y slot][component][8]
 constexpr int EXP = 7 * PLANE;               // one exchange array: 7 planes of (x,y) slots
-constexpr unsigned BYTES_ARR = F_ARR * 4u;   // bytes TMA delivers per array and step
 
 template <bool COEF>
 struct Lay {
     static constexpr int NC = COEF ? 6 : 3;            // resident coefficient floats per cell: COEF: three (ca, cb) pairs,
                                                        // [(c*BZ + z slot)*PLANE + slot] as float2; else three cb masks as float
     static constexpr int stgh = 0;
-    static constexpr int stge = stgh + 3 * F_ARR;
-    static constexpr int stgc = stge + 3 * F_ARR;
+    static constexpr int stge = stgh + 3 * F_ARR_F;
+    static constexpr int stgc = stge + 3 * F_ARR_F;
     static constexpr int xpkh = stgc + (COEF ? 6 * F_ARR : 0);
     static constexpr int xpke = xpkh + XPK;
     static constexpr int xoute = xpke + XPK;           // leaving x column of E, [y slot][component][8], stored by the signal warp
@@ -302,11 +330,14 @@ __device__ __forceinline__ void tma_load_4d(float* dst, const CUtensorMap* map, 
 // One lane issues the minus shell of step k for a group of NA arrays into stg = [NA][FZ] [NA][FY] [NA][FX].
 // grouped == 1: the arrays sit at a uniform stride and maps[0..2] are 4-D (x, y, z, array) maps, one box per piece;
 // grouped == 2 (NA = 6): two such triples (maps[0..2], maps[9..11]); grouped == 0: per-array 3-D maps maps[a*3 + piece].
-template <int NA>
+// FLD: the group is the three field arrays (elements of fld_t, field box geometry); else f32 coefficient arrays.
+template <int NA, bool FLD>
 __device__ __forceinline__ void issue_shell(const CUtensorMap* maps, int grouped, float* stg, int o0, int o1, int o2, unsigned long long* bar)
 {
-    const int q0 = o0 & ~3;
-    mbar_expect_tx(bar, (unsigned)NA * BYTES_ARR);
+    // piece sizes in floats of staging
+    constexpr int FZ = FLD ? FZF * (int)sizeof(fld_t) / 4 : ::FZ, FY = FLD ? FYF * (int)sizeof(fld_t) / 4 : ::FY, FX = FLD ? FXF * (int)sizeof(fld_t) / 4 : ::FX;
+    const int q0 = FLD ? (o0 & ~XMASK_F) : (o0 & ~3);
+    mbar_expect_tx(bar, (unsigned)NA * (unsigned)(FZ + FY + FX) * 4u);
     float* dz = stg;
     float* dy = stg + NA * FZ;
     float* dx = stg + NA * (FZ + FY);
@@ -399,17 +430,17 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
 }
 
 // x column of the three field arrays in `stg` -> xpk[(y slot*3 + c)*8 + l], l = 1..7 (16-byte rows for the owner lane)
-__device__ __forceinline__ void pack_xcol(const float* stg, float* xpk, int o0, int o1)
+__device__ __forceinline__ void pack_xcol(const fld_t* stg, float* xpk, int o0, int o1)
 {
     const int lane = threadIdx.x & 31;
-    const int r0 = o0 & 3;
+    const int r0 = o0 & XMASK_F;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         float v[4];
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int idx = r * 32 + lane;
-            v[r] = idx < W1 * W2 ? stg[xidx<3>(c, 1 + idx % W1, 1 + idx / W1) + r0] : 0.0f;
+            v[r] = idx < W1 * W2 ? fld_get(stg + xidxF(c, 1 + idx % W1, 1 + idx / W1) + r0) : 0.0f;
         }
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
@@ -452,9 +483,9 @@ __device__ __forceinline__ void store_xcol(const SysParams& P, float* const* fld
         const int gy = o1 + ly, gz = o2 + l;
         if (item < BY * (W2 - 1) && ly >= ly_lo && ly <= ly_hi && (unsigned)gy < (unsigned)P.g.n[1] && (unsigned)gz < (unsigned)P.g.n[2]) {
             const long long off = gx + nx * gy + plane * gz;
-            __stcg(fld[0] + off, x.v[r][0]);
-            __stcg(fld[1] + off, x.v[r][1]);
-            __stcg(fld[2] + off, x.v[r][2]);
+            fld_stcg(fld[0], off, x.v[r][0]);
+            fld_stcg(fld[1], off, x.v[r][1]);
+            fld_stcg(fld[2], off, x.v[r][2]);
             FDTD_DEBUG_ONLY(lev_set(lev, off, level);)
         }
     }
@@ -537,8 +568,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     const int nx = P.g.n[0], ny = P.g.n[1], nz = P.g.n[2];
     const long long ldx = P.ldx, plane = ldx * ny;
 
-    const float* stgH = sm + Lay<COEF>::stgh;
-    const float* stgE = sm + Lay<COEF>::stge;
+    const fld_t* stgH = reinterpret_cast<const fld_t*>(sm + Lay<COEF>::stgh);
+    const fld_t* stgE = reinterpret_cast<const fld_t*>(sm + Lay<COEF>::stge);
     const float* xpkH = sm + Lay<COEF>::xpkh;
     const float* xpkE = sm + Lay<COEF>::xpke;
     // y exchange: only the links between a thread's row 1 and the next warp's row 0 go through shared memory
@@ -573,7 +604,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         const int o0 = t.a[0] - k - 1, o1 = t.a[1] - k - 1, o2 = t.a[2] - k - 1;
         const int lx = (lane - o0) & (BX - 1);
         const int gx = o0 + lx;
-        const int xs = (o0 & 3) + lx;          // position inside a staged row
+        const int xs = (o0 & XMASK_F) + lx;    // position inside a staged field row
         int ly[NROW], gy[NROW];
         bool col_in[NROW];
         long long col_off[NROW];
@@ -596,13 +627,13 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     const int gz = o2 + l;
                     const bool ok = col_in[r] && (unsigned)gz < (unsigned)nz;
                     const long long off = ok ? col_off[r] + plane * gz : 0;
-                    hx[r][l] = ok ? __ldcg(Hx + off) : 0.0f;
-                    hy[r][l] = ok ? __ldcg(Hy + off) : 0.0f;
-                    hz[r][l] = ok ? __ldcg(Hz + off) : 0.0f;
+                    hx[r][l] = ok ? fld_ldcg(Hx, off) : 0.0f;
+                    hy[r][l] = ok ? fld_ldcg(Hy, off) : 0.0f;
+                    hz[r][l] = ok ? fld_ldcg(Hz, off) : 0.0f;
                     const bool oke = ok && lx >= 1 && ly[r] >= 1 && l >= 1;
-                    ex[r][l] = oke ? __ldcg(Ex + off) : 0.0f;
-                    ey[r][l] = oke ? __ldcg(Ey + off) : 0.0f;
-                    ez[r][l] = oke ? __ldcg(Ez + off) : 0.0f;
+                    ex[r][l] = oke ? fld_ldcg(Ex, off) : 0.0f;
+                    ey[r][l] = oke ? fld_ldcg(Ey, off) : 0.0f;
+                    ez[r][l] = oke ? fld_ldcg(Ez, off) : 0.0f;
                     FDTD_DEBUG_ONLY(if (ok) lev_check(P, P.levH, off, 0, 1); if (oke) lev_check(P, P.levE, off, 0, 2);)
                     const int cidx = r * SX + (gz & (BZ - 1)) * PLANE;
 #pragma unroll
@@ -628,18 +659,18 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             TRACE_C(1, k);
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
-                hx[r][0] = stgH[zidx<3>(0, ly[r], xs)];
-                hy[r][0] = stgH[zidx<3>(1, ly[r], xs)];
-                hz[r][0] = stgH[zidx<3>(2, ly[r], xs)];
+                hx[r][0] = fld_get(stgH + zidxF(0, ly[r], xs));
+                hy[r][0] = fld_get(stgH + zidxF(1, ly[r], xs));
+                hz[r][0] = fld_get(stgH + zidxF(2, ly[r], xs));
             }
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 if (ly[r] == 0) {         // warp-uniform: the entering row
 #pragma unroll
                     for (int l = 1; l < BZ; ++l) {
-                        hx[r][l] = stgH[yidx<3>(0, l, xs)];
-                        hy[r][l] = stgH[yidx<3>(1, l, xs)];
-                        hz[r][l] = stgH[yidx<3>(2, l, xs)];
+                        hx[r][l] = fld_get(stgH + yidxF(0, l, xs));
+                        hy[r][l] = fld_get(stgH + yidxF(1, l, xs));
+                        hz[r][l] = fld_get(stgH + yidxF(2, l, xs));
                         if (r == RL) {    // its y+1 neighbour is the next warp's row 0, which reads it from the exchange
                             exH[(l - 1) * PLANE + slot1] = make_float2(hz[r][l], hx[r][l]);
                         }
@@ -699,11 +730,11 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     cbx = cmask[cidx + r * SX]; cby = cmask[cidx + r * SX + BZ * PLANE]; cbz = cmask[cidx + r * SX + 2 * BZ * PLANE];
                 }
                 // E_x: (Hz - Hz[j-1])/dy - (Hy - Hy[k-1])/dz      eq. (1)
-                ex[r][l + 1] = yee_e_update<COEF>(ex[r][l], hz[r][l], hz_y, hy[r][l], hy[r][l - 1], rdy, rdz, cax, cbx);
+                ex[r][l + 1] = fld_round(yee_e_update<COEF>(ex[r][l], hz[r][l], hz_y, hy[r][l], hy[r][l - 1], rdy, rdz, cax, cbx));
                 // E_y: (Hx - Hx[k-1])/dz - (Hz - Hz[i-1])/dx
-                ey[r][l + 1] = yee_e_update<COEF>(ey[r][l], hx[r][l], hx[r][l - 1], hz[r][l], hz_xm, rdz, rdx, cay, cby);
+                ey[r][l + 1] = fld_round(yee_e_update<COEF>(ey[r][l], hx[r][l], hx[r][l - 1], hz[r][l], hz_xm, rdz, rdx, cay, cby));
                 // E_z: (Hy - Hy[i-1])/dx - (Hx - Hx[j-1])/dy
-                ez[r][l + 1] = yee_e_update<COEF>(ez[r][l], hy[r][l], hy_xm, hx[r][l], hx_y, rdx, rdy, caz, cbz);
+                ez[r][l + 1] = fld_round(yee_e_update<COEF>(ez[r][l], hy[r][l], hy_xm, hx[r][l], hx_y, rdx, rdy, caz, cbz));
             }
         }
         };
@@ -730,9 +761,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                                     if (sz >= 0 && sz < P.g.src_box[5]) {
                                         const float amp = __ldg(P.g.src_amp + (sx + P.g.src_box[3] * (sy + (long long)P.g.src_box[4] * sz)));
                                         const float inj = amp * wsrc;
-                                        if (P.g.src_comp == 0) ex[r][l + 1] = ex[r][l + 1] + inj;
-                                        else if (P.g.src_comp == 1) ey[r][l + 1] = ey[r][l + 1] + inj;
-                                        else ez[r][l + 1] = ez[r][l + 1] + inj;
+                                        if (P.g.src_comp == 0) ex[r][l + 1] = fld_round(ex[r][l + 1] + inj);
+                                        else if (P.g.src_comp == 1) ey[r][l + 1] = fld_round(ey[r][l + 1] + inj);
+                                        else ez[r][l + 1] = fld_round(ez[r][l + 1] + inj);
                                     }
                                 }
                             }
@@ -773,9 +804,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             if ((lx >= 1) & (ly[r] >= 1) && col_in[r] && !FDTD_DBG(P, 4)) {
                 if ((unsigned)(o2 + W2) < (unsigned)nz) {            // the leaving plane l = 7: every column
                     const long long off = col_off[r] + plane * (o2 + W2);
-                    __stcg(Ex + off, ex[r][W2 + 1]);
-                    __stcg(Ey + off, ey[r][W2 + 1]);
-                    __stcg(Ez + off, ez[r][W2 + 1]);
+                    fld_stcg(Ex, off, ex[r][W2 + 1]);
+                    fld_stcg(Ey, off, ey[r][W2 + 1]);
+                    fld_stcg(Ez, off, ez[r][W2 + 1]);
                     FDTD_DEBUG_ONLY(lev_set(P.levE, off, k + 1);)
                 }
                 if (last | (ly[r] == W1)) {                          // warp-uniform: the leaving row (or the whole tile), planes 1..6
@@ -783,9 +814,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #pragma unroll
                     for (int l = 1; l < W2; ++l) {
                         if ((unsigned)(o2 + l) < (unsigned)nz) {
-                            __stcg(Ex + off, ex[r][l + 1]);
-                            __stcg(Ey + off, ey[r][l + 1]);
-                            __stcg(Ez + off, ez[r][l + 1]);
+                            fld_stcg(Ex, off, ex[r][l + 1]);
+                            fld_stcg(Ey, off, ey[r][l + 1]);
+                            fld_stcg(Ez, off, ez[r][l + 1]);
                             FDTD_DEBUG_ONLY(lev_set(P.levE, off, k + 1);)
                         }
                         off += plane;
@@ -813,9 +844,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
         TRACE_C(5, k);
 #pragma unroll
         for (int r = 0; r < NROW; ++r) {
-            ex[r][1] = stgE[zidx<3>(0, ly[r], xs)];
-            ey[r][1] = stgE[zidx<3>(1, ly[r], xs)];
-            ez[r][1] = stgE[zidx<3>(2, ly[r], xs)];
+            ex[r][1] = fld_get(stgE + zidxF(0, ly[r], xs));
+            ey[r][1] = fld_get(stgE + zidxF(1, ly[r], xs));
+            ez[r][1] = fld_get(stgE + zidxF(2, ly[r], xs));
         }
         exE[slot0] = make_float2(ez[0][1], ex[0][1]);
 #pragma unroll
@@ -823,9 +854,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             if (ly[r] == 0) {             // warp-uniform: the entering row
 #pragma unroll
                 for (int l = 1; l < BZ; ++l) {
-                    ex[r][l + 1] = stgE[yidx<3>(0, l, xs)];
-                    ey[r][l + 1] = stgE[yidx<3>(1, l, xs)];
-                    ez[r][l + 1] = stgE[yidx<3>(2, l, xs)];
+                    ex[r][l + 1] = fld_get(stgE + yidxF(0, l, xs));
+                    ey[r][l + 1] = fld_get(stgE + yidxF(1, l, xs));
+                    ez[r][l + 1] = fld_get(stgE + yidxF(2, l, xs));
                 }
             }
         }
@@ -878,9 +909,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                 // y+1 neighbour: the last row reads the next warp's row 0 from the exchange, row 0 of two reads row 1's registers
                 const float ez_y = r == RL ? ez_yp : ez[r < RL ? r + 1 : RL][l + 1];
                 const float ex_y = r == RL ? ex_yp : ex[r < RL ? r + 1 : RL][l + 1];
-                hx[r][l + 1] = yee_h_update(hx[r][l], ez_y, ez[r][l + 1], ey[r][l + 2], ey[r][l + 1], rdy, rdz, dbx);   // (Ez[j+1]-Ez)/dy - (Ey[k+1]-Ey)/dz
-                hy[r][l + 1] = yee_h_update(hy[r][l], ex[r][l + 2], ex[r][l + 1], ez_xp, ez[r][l + 1], rdz, rdx, dby);   // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
-                hz[r][l + 1] = yee_h_update(hz[r][l], ey_xp, ey[r][l + 1], ex_y, ex[r][l + 1], rdx, rdy, dbz);           // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
+                hx[r][l + 1] = fld_round(yee_h_update(hx[r][l], ez_y, ez[r][l + 1], ey[r][l + 2], ey[r][l + 1], rdy, rdz, dbx));   // (Ez[j+1]-Ez)/dy - (Ey[k+1]-Ey)/dz
+                hy[r][l + 1] = fld_round(yee_h_update(hy[r][l], ex[r][l + 2], ex[r][l + 1], ez_xp, ez[r][l + 1], rdz, rdx, dby));   // (Ex[k+1]-Ex)/dz - (Ez[i+1]-Ez)/dx
+                hz[r][l + 1] = fld_round(yee_h_update(hz[r][l], ey_xp, ey[r][l + 1], ex_y, ex[r][l + 1], rdx, rdy, dbz));           // (Ey[i+1]-Ey)/dx - (Ex[j+1]-Ex)/dy
             }
             exH[l * PLANE + slot1] = make_float2(hz[RL][l + 1], hx[RL][l + 1]);
         }
@@ -907,9 +938,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             if ((lx <= W0 - 1) & (ly[r] <= W1 - 1) && col_in[r] && !FDTD_DBG(P, 4)) {
                 if ((unsigned)(o2 + W2 - 1) < (unsigned)nz) {        // the leaving plane l = 6: every column
                     const long long off = col_off[r] + plane * (o2 + W2 - 1);
-                    __stcg(Hx + off, hx[r][W2]);
-                    __stcg(Hy + off, hy[r][W2]);
-                    __stcg(Hz + off, hz[r][W2]);
+                    fld_stcg(Hx, off, hx[r][W2]);
+                    fld_stcg(Hy, off, hy[r][W2]);
+                    fld_stcg(Hz, off, hz[r][W2]);
                     FDTD_DEBUG_ONLY(lev_set(P.levH, off, k + 1);)
                 }
                 if (last | (ly[r] == W1 - 1)) {                      // warp-uniform: leaving row (or whole tile), planes 0..5
@@ -917,9 +948,9 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #pragma unroll
                     for (int l = 0; l < W2 - 1; ++l) {
                         if ((unsigned)(o2 + l) < (unsigned)nz) {
-                            __stcg(Hx + off, hx[r][l + 1]);
-                            __stcg(Hy + off, hy[r][l + 1]);
-                            __stcg(Hz + off, hz[r][l + 1]);
+                            fld_stcg(Hx, off, hx[r][l + 1]);
+                            fld_stcg(Hy, off, hy[r][l + 1]);
+                            fld_stcg(Hz, off, hz[r][l + 1]);
                             FDTD_DEBUG_ONLY(lev_set(P.levH, off, k + 1);)
                         }
                         off += plane;
@@ -1075,7 +1106,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                         if (k > hk0) { mbar_wait(mb + MB_HFREE, n_hfree & 1u); ++n_hfree; }
                         PROF_MARK(1);
                         TRACE(1, 2, k);
-                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
+                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3, true>(maps + 3 * 3, P.tma_group[1], sm + Lay<COEF>::stgh, o0, o1, o2, mb + MB_HFULL);
                         __syncwarp();
                         if (k + 1 < k1 && EARLY) {
                             wait_upwind(P, t, P.flagH, P.flag_base + k + 1, &ctl);
@@ -1086,7 +1117,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                         if (!FDTD_DBG(P, 2)) { mbar_wait(mb + MB_HFULL, n_hfull & 1u); ++n_hfull; }
                         PROF_MARK(3);
                         TRACE(1, 4, k);
-                        pack_xcol(sm + Lay<COEF>::stgh, sm + Lay<COEF>::xpkh, o0, o1);
+                        pack_xcol(reinterpret_cast<const fld_t*>(sm + Lay<COEF>::stgh), sm + Lay<COEF>::xpkh, o0, o1);
                         warp_arrive(mb + MB_HREADY);
                         TRACE(1, 5, k);
                         PROF_MARK(4);
@@ -1098,7 +1129,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                         if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
                         PROF_MARK(0);
                         TRACE(2, 1, k);
-                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6, false>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
                         __syncwarp();
                         PROF_MARK(1);
                         }
@@ -1127,7 +1158,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                     mbar_wait(mb + MB_EFREE, n_efree & 1u); ++n_efree;     // staging of step k-1 absorbed
                 }
                 TRACE(3, 1, k);
-                if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
+                if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<3, true>(maps, P.tma_group[0], sm + Lay<COEF>::stge, o0, o1, o2, mb + MB_EFULL);
                 __syncwarp();
                 if (k + 1 < k1 && EARLY) {
                     wait_upwind(P, t, P.flagE, P.flag_base + k + 2, &ctl);
@@ -1136,7 +1167,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                 TRACE(3, 2, k);
                 if (!FDTD_DBG(P, 2)) { mbar_wait(mb + MB_EFULL, n_efull & 1u); ++n_efull; }
                 TRACE(3, 4, k);
-                const float* stg = sm + Lay<COEF>::stge;
+                const fld_t* stg = reinterpret_cast<const fld_t*>(sm + Lay<COEF>::stge);
                 pack_xcol(stg, sm + Lay<COEF>::xpke, o0, o1);
                 TRACE(3, 5, k);
                 if (k > k0) { mbar_wait(mb + MB_HDONE, n_hdone & 1u); ++n_hdone; }   // H phase k-1 has read the E exchange rows
@@ -1148,7 +1179,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                     if (idx < W1 * (W2 - 1)) {
                         const int ly = 1 + idx % W1, l = 1 + idx / W1;
                         const int s = ((o1 + ly) & (BY - 1)) * SX + (o0 & (BX - 1));
-                        exE[l * PLANE + s] = make_float2(stg[xidx<3>(2, ly, l) + (o0 & 3)], stg[xidx<3>(0, ly, l) + (o0 & 3)]);
+                        exE[l * PLANE + s] = make_float2(fld_get(stg + xidxF(2, ly, l) + (o0 & XMASK_F)), fld_get(stg + xidxF(0, ly, l) + (o0 & XMASK_F)));
                     }
                 }
                 warp_arrive(mb + MB_EREADY);
@@ -1214,11 +1245,15 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
 
 size_t FDTD_TMA_NAME(systolic_tma_smem)(int coef) { return (size_t)(coef ? Lay<true>::total : Lay<false>::total) * sizeof(float); }
 int FDTD_TMA_NAME(systolic_tma_threads)() { return NT; }
-void FDTD_TMA_NAME(systolic_tma_boxes)(int box[3][3])
+void FDTD_TMA_NAME(systolic_tma_boxes)(int fld[3][3], int coef[3][3])
 {
-    const int b[3][3] = {{RX, BY, 1}, {RX, 1, BZ}, {4, BY, W2}};
+    const int bf[3][3] = {{RXF, BY, 1}, {RXF, 1, BZ}, {CWF, BY, W2}};
+    const int bc[3][3] = {{RX, BY, 1}, {RX, 1, BZ}, {4, BY, W2}};
     for (int f = 0; f < 3; ++f)
-        for (int q = 0; q < 3; ++q) box[f][q] = b[f][q];
+        for (int q = 0; q < 3; ++q) {
+            fld[f][q] = bf[f][q];
+            coef[f][q] = bc[f][q];
+        }
 }
 
 cudaError_t FDTD_TMA_NAME(systolic_tma_prepare)(int coef, int* blocks_per_sm)

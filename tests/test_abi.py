@@ -19,7 +19,7 @@ def libs():
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "fdtd.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(fdtd_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(fdtd_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_every_declared_symbol_is_exported_and_bound(libs):

@@ -203,3 +203,80 @@ def test_monitor_rejected_by_other_schedules_and_bad_arguments(cuda_device):
     sim.step(2)
     sim.sync()
     sim.close()
+
+
+# ---- f1: binary16 field storage, f32 arithmetic ---------------------------------------------------------------------
+def _h16_oracle(w, steps):
+    r16 = lambda a: a.astype(np.float16).astype(np.float32)
+    E, H = workloads.make_fields(w)
+    E, H = [r16(a) for a in E], [r16(a) for a in H]
+    ca, cb = workloads.make_coeffs(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None, storage="f16")
+    src = workloads.make_source(w)
+    if src is not None:
+        orc.set_source(src.comp, src.box, src.amp, src.wave)
+    orc.step(steps)
+    return E, H
+
+
+def _h16_gpu(w, steps, kernel, tile, T, variant="nofma", calls=1):
+    import torch
+    dev = torch.device("cuda:0")
+    E, H = workloads.make_fields(w, device=dev)
+    E, H = [a.to(torch.float16) for a in E], [a.to(torch.float16) for a in H]      # round-to-nearest-even, as the oracle's inputs
+    ca, cb = workloads.make_coeffs(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant=variant)
+    sim.set_fields(E, H)
+    if ca is not None:
+        sim.set_coeffs(ca, cb, None)
+    src = workloads.make_source(w)
+    if src is not None:
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(kernel, tile, T)
+    for c in range(calls):
+        sim.step(steps // calls if c < calls - 1 else steps - (calls - 1) * (steps // calls))
+    sim.sync()
+    info = sim.get_kernel()
+    sim.close()
+    return [a.float().cpu().numpy() for a in E], [a.float().cpu().numpy() for a in H], info
+
+
+@pytest.fixture(scope="module")
+def h16_cache():
+    cache = {}
+
+    def get(name):
+        if name not in cache:
+            w, steps = CASES[name]
+            cache[name] = _h16_oracle(w, steps)
+        return cache[name]
+    return get
+
+
+H16_RUNS = [("C1", "naive", None, 0), ("C2s", "naive", None, 0), ("C3s", "naive", None, 0), ("ragged", "naive", None, 0),
+            ("C1", "systolic", (31, 15, 7), 33), ("C1", "systolic", (31, 15, 7), 128), ("C2s", "systolic", (31, 15, 7), 32),
+            ("C2s", "systolic", (31, 15, 7), 5), ("C3s", "systolic", (31, 15, 7), 16), ("C4s", "systolic", (31, 15, 7), 40),
+            ("C5s", "systolic", (31, 15, 7), 32), ("C5s", "systolic", (31, 15, 7), 1), ("ragged", "systolic", (31, 15, 7), 6),
+            ("allper", "systolic", (31, 15, 7), 5)]
+
+
+@pytest.mark.parametrize("name,kernel,tile,T", H16_RUNS)
+def test_f16_storage_matches_oracle_bit_exact(cuda_device, h16_cache, name, kernel, tile, T):
+    w, steps = CASES[name]
+    E, H, info = _h16_gpu(w, steps, binding.KERNEL_NAIVE if kernel == "naive" else binding.KERNEL_SYSTOLIC, tile, T, calls=2)
+    want = h16_cache(name)
+    assert max(float(np.abs(a).max()) for a in want[0] + want[1]) > 0
+    compare((E, H), want, exact=True)
+
+
+def test_f16_storage_fma_build_within_tolerance_and_other_schedules_rejected(cuda_device, h16_cache):
+    w, steps = CASES["C5s"]
+    E, H, _ = _h16_gpu(w, steps, binding.KERNEL_SYSTOLIC, (31, 15, 7), 32, variant="fma")
+    want = h16_cache("C5s")
+    scale = max(float(np.abs(a).max()) for a in want[0] + want[1])
+    worst = max(float(np.abs(g - o).max()) for g, o in zip(E + H, want[0] + want[1]))
+    assert worst <= 2.0 ** -10 * scale          # contraction moves a result across a binary16 rounding boundary now and then
+    for kernel, tile in ((binding.KERNEL_SYSTOLIC_REG, (31, 15, 7)), (binding.KERNEL_SYSTOLIC, (31, 7, 7)), (binding.KERNEL_SYSTOLIC_SMEM, (15, 7, 7))):
+        with pytest.raises(binding.FdtdError) as e:
+            _h16_gpu(w, 4, kernel, tile, 4)
+        assert e.value.code == binding.EINVAL

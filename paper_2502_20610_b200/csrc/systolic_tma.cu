@@ -555,7 +555,7 @@ struct Phases {   // completed phases of each mbarrier as seen by this thread's 
     unsigned hready, eready, acke, ackh, cfull;
 };
 
-template <bool COEF>
+template <bool COEF, bool MON>
 __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom& t, int tile, int k0, int k1, bool fast, float* sm, unsigned long long* mb, Phases& ph)
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -773,7 +773,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             }
         }
         // running DFT of E on the monitor plane: R_k = [o+1, o+W] on every axis
-        if (monitor_hits(P.mon, P.t0 + k, o0 + 1, o1 + 1, o2 + 1)) {
+        if (MON && monitor_hits(P.mon, P.t0 + k, o0 + 1, o1 + 1, o2 + 1)) {
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 if ((lx >= 1) & (ly[r] >= 1) && col_in[r]) {
@@ -916,7 +916,7 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
             exH[l * PLANE + slot1] = make_float2(hz[RL][l + 1], hx[RL][l + 1]);
         }
         // running DFT of H on the monitor plane: R_{k+1} = [o, o+W-1] on every axis
-        if (monitor_hits(P.mon, P.t0 + k, o0, o1, o2)) {
+        if (MON && monitor_hits(P.mon, P.t0 + k, o0, o1, o2)) {
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 if ((lx <= W0 - 1) & (ly[r] <= W1 - 1) && col_in[r]) {
@@ -976,7 +976,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
     if (k1 > k0) { ++ph.acke; ++ph.ackh; }
 }
 
-template <bool COEF>
+// MON: a running-DFT monitor is set (a separate instantiation keeps its rare path out of the product loop)
+template <bool COEF, bool MON>
 __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __grid_constant__ SysParams P, const __grid_constant__ TmaMaps M)
 {
     extern __shared__ __align__(128) float sm[];
@@ -1068,7 +1069,7 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
     if (warp < NWARPS_C) {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS_COMPUTE));
         TileJob J;
-        while (next_tile(J)) compute_tile<COEF>(P, J.t, J.tile, J.k0, J.k1, J.fast, sm, mb, ph);
+        while (next_tile(J)) compute_tile<COEF, MON>(P, J.t, J.tile, J.k0, J.k1, J.fast, sm, mb, ph);
         return;
     }
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS_AUX));
@@ -1258,8 +1259,10 @@ void FDTD_TMA_NAME(systolic_tma_boxes)(int fld[3][3], int coef[3][3])
 
 cudaError_t FDTD_TMA_NAME(systolic_tma_prepare)(int coef, int* blocks_per_sm)
 {
-    const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
+    const void* fn = coef ? (const void*)&systolic_tma_kernel<true, false> : (const void*)&systolic_tma_kernel<false, false>;
+    const void* fm = coef ? (const void*)&systolic_tma_kernel<true, true> : (const void*)&systolic_tma_kernel<false, true>;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FDTD_TMA_NAME(systolic_tma_smem)(coef));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(fm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FDTD_TMA_NAME(systolic_tma_smem)(coef));
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, fn, NT, FDTD_TMA_NAME(systolic_tma_smem)(coef));
 }
@@ -1267,7 +1270,8 @@ cudaError_t FDTD_TMA_NAME(systolic_tma_prepare)(int coef, int* blocks_per_sm)
 cudaError_t FDTD_TMA_NAME(launch_systolic_tma)(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st)
 {
     static_assert(sizeof(CUtensorMap) == 128, "TmaMaps layout");
-    const void* fn = coef ? (const void*)&systolic_tma_kernel<true> : (const void*)&systolic_tma_kernel<false>;
+    const void* fn = p.mon.on ? (coef ? (const void*)&systolic_tma_kernel<true, true> : (const void*)&systolic_tma_kernel<false, true>)
+                              : (coef ? (const void*)&systolic_tma_kernel<true, false> : (const void*)&systolic_tma_kernel<false, false>);
     void* args[] = {(void*)&p, (void*)&maps};
     return cudaLaunchKernel(fn, dim3((unsigned)ctas), dim3((unsigned)NT), args, FDTD_TMA_NAME(systolic_tma_smem)(coef), st);
 }

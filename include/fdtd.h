@@ -156,8 +156,12 @@ int fdtd_get_kernel(const fdtd_ctx* ctx, int out[8]);
  * out[2] = systolic chunks launched, out[3] = tiles processed. */
 int fdtd_get_counters(const fdtd_ctx* ctx, long long out[4]);
 
-/* GPU time of the most recent fdtd_step call in milliseconds (CUDA events recorded on the ctx stream around
- * the enqueued kernels).  Synchronises on the closing event. */
+/* GPU time of the most recent fdtd_step call in milliseconds (CUDA events recorded on the ctx stream around the enqueued
+ * kernels).  Synchronises on the closing event.  Timing is OFF by default: the events sit between the last launch of one
+ * call and the first launch of the next and would serialise them, whereas consecutive systolic launches of the same
+ * tile grid overlap (the next launch fills the SMs the previous one drains, gated by per-tile flags; PAPER.md:112,
+ * DESIGN.md 6.6).  fdtd_set_timing(ctx, 1) switches the events on for later calls; FDTD_ESTATE until a timed call exists. */
+int fdtd_set_timing(fdtd_ctx* ctx, int on);
 int fdtd_last_step_ms(fdtd_ctx* ctx, float* ms);
 
 /* Pure host function (no device needed): the tile schedule the systolic kernel would use for this grid.

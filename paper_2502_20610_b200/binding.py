@@ -37,6 +37,7 @@ _PROTOS = {
     "fdtd_set_kernel": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]),
     "fdtd_get_kernel": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "fdtd_get_counters": (C.c_int, [C.c_void_p, C.POINTER(C.c_longlong)]),
+    "fdtd_set_timing": (C.c_int, [C.c_void_p, C.c_int]),
     "fdtd_last_step_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
     "fdtd_plan_tiles": (C.c_int, [C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int, C.POINTER(C.c_int)]),
     "fdtd_plan_owner": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
@@ -228,6 +229,9 @@ class Fdtd:
         out = (C.c_longlong * 5)()
         self._check(self._lib.fdtd_debug_level_errors(self._h, out))
         return tuple(out)
+
+    def set_timing(self, on=True):
+        self._check(self._lib.fdtd_set_timing(self._h, int(bool(on))))
 
     def last_step_ms(self):
         ms = C.c_float()

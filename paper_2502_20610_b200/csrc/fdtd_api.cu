@@ -53,7 +53,12 @@ struct fdtd_ctx {
     // systolic state
     int* d_flags;     // flagE[cap] then flagH[cap]
     size_t flags_cap;
-    unsigned int* d_counter;
+    unsigned int* d_counter;   // ring of kCounterRing tile-claim counters: launch L uses slot L % ring; a TMA launch zeroes slot (L + ring/2) % ring
+    unsigned long long launch_seq;
+    // launch-to-launch overlap (row f2): shape and final flag value of the previous TMA launch, 0 = none / not reusable
+    int prev_nb[3], prev_T, prev_final;
+    bool no_overlap;           // FDTD_NO_OVERLAP in the environment at fdtd_create: every launch waits for the previous one
+    bool timing;               // fdtd_set_timing: record events around every fdtd_step call (they serialise consecutive launches)
     int* d_abort;
     long long* d_prof;   // FDTD_PROFILE build only
     int* d_order;        // wavefront claim order of the TMA kernel for the launch being enqueued
@@ -80,6 +85,8 @@ struct fdtd_ctx {
 };
 
 namespace {
+
+constexpr int kCounterRing = 64;
 
 // Every entry point that touches the device runs on the device the context was created on, whatever device is
 // current in the calling thread, and leaves the caller's current device unchanged.
@@ -234,6 +241,7 @@ int resolve_systolic(fdtd_ctx* c)
         }
     }
     c->tmaps_valid = false;
+    c->prev_final = 0;
     c->cfg_idx = found;
     for (int a = 0; a < 3; ++a) c->N[a] = N[a];
     c->resolved = true;
@@ -275,6 +283,7 @@ int ensure_flags(fdtd_ctx* c, size_t ntiles)
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(flags)");
     c->flags_cap = ntiles;
     c->flag_base = 0;
+    c->prev_final = 0;
     return FDTD_OK;
 }
 
@@ -540,6 +549,7 @@ int step_systolic(fdtd_ctx* c, int n)
             cudaError_t e = cudaMemsetAsync(c->d_flags, 0, 2 * c->flags_cap * sizeof(int), c->stream);
             if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(flags)");
             c->flag_base = 0;
+            c->prev_final = 0;
         }
         P.order = nullptr;
         if (c->use_tma && !c->dbg_lex_order) {
@@ -554,7 +564,14 @@ int step_systolic(fdtd_ctx* c, int n)
         P.ntiles = (int)ntiles;
         P.flagE = c->d_flags;
         P.flagH = c->d_flags + c->flags_cap;
-        P.counter = c->d_counter;
+        P.counter = c->d_counter + (c->launch_seq % kCounterRing);
+        P.counter_zero = c->use_tma ? c->d_counter + ((c->launch_seq + kCounterRing / 2) % kCounterRing) : nullptr;
+        // overlap with the previous launch: same tile grid, same flag arrays still holding its final values, nothing but that
+        // kernel before this one in the stream (a ghost refill or a copy in between serialises anyway: the wait is then free)
+        P.pred_final = 0;
+        if (c->use_tma && !c->use_pad && c->prev_final != 0 && c->prev_T == T && c->prev_nb[0] == P.ax[0].nb && c->prev_nb[1] == P.ax[1].nb &&
+            c->prev_nb[2] == P.ax[2].nb && T >= 2 && !c->dbg_levels && !c->no_overlap)
+            P.pred_final = c->prev_final;
         P.abort_flag = c->d_abort;
         P.spin_budget = c->spin_budget;
         P.delay_seed = c->delay_seed;
@@ -587,8 +604,11 @@ int step_systolic(fdtd_ctx* c, int n)
             P.levH = c->d_lev + cells;
             P.lev_err = c->d_lev_err;
         }
-        cudaError_t e = cudaMemsetAsync(c->d_counter, 0, sizeof(unsigned int), c->stream);
-        if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
+        cudaError_t e = cudaSuccess;
+        if (!c->use_tma) {      // the other kernels do not maintain the ring
+            e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int), c->stream);
+            if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
+        }
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
         e = c->tma_h16   ? launch_systolic_tma_h16(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->tma_by8 ? launch_systolic_tma_by8(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
@@ -596,6 +616,13 @@ int step_systolic(fdtd_ctx* c, int n)
             : c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream)
                          : launch_systolic(c->cfg_idx, P, ctas, c->stream);
         if (e != cudaSuccess) return cuda_fail(c, e, "systolic launch");
+        c->prev_final = 0;
+        if (c->use_tma) {
+            c->prev_final = c->flag_base + T;
+            c->prev_T = T;
+            for (int a = 0; a < 3; ++a) c->prev_nb[a] = P.ax[a].nb;
+        }
+        c->launch_seq++;
         c->flag_base += T + 2;
         c->t += T;
         left -= T;
@@ -621,6 +648,7 @@ int check_async(fdtd_ctx* c)
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(abort flag)");
     if (flag != 0) {
         cudaMemset(c->d_abort, 0, sizeof(int));
+        c->prev_final = 0;      // the flags of the aborted launch are not final: the next launch must not wait on them
         return fail(c, FDTD_ETIMEOUT, "systolic hand-off watchdog fired: a tile waited longer than the spin budget; fields are invalid");
     }
     return FDTD_OK;
@@ -690,6 +718,11 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->d_flags = nullptr;
     c->flags_cap = 0;
     c->d_counter = nullptr;
+    c->launch_seq = 0;
+    c->prev_final = 0;
+    c->prev_T = 0;
+    c->timing = false;
+    c->no_overlap = false;
     c->d_abort = nullptr;
     c->d_prof = nullptr;
     c->d_mon_w = nullptr;
@@ -706,6 +739,7 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->env_T = 0;
     c->env_tile[0] = c->env_tile[1] = c->env_tile[2] = 0;
     if (const char* env = getenv("FDTD_T")) c->env_T = atoi(env);
+    c->no_overlap = getenv("FDTD_NO_OVERLAP") != nullptr;
     if (const char* env = getenv("FDTD_TILE")) {
         int x, y, z;
         if (sscanf(env, "%dx%dx%d", &x, &y, &z) == 3 && x > 0 && y > 0 && z > 0) { c->env_tile[0] = x; c->env_tile[1] = y; c->env_tile[2] = z; }
@@ -727,7 +761,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->spin_budget = (long long)(budget_ms * (double)(prop.clockRate > 0 ? prop.clockRate : 1965000));
     c->ev_valid = false;
     memset(c->counters, 0, sizeof c->counters);
-    e = cudaMalloc(&c->d_counter, sizeof(unsigned int));
+    e = cudaMalloc(&c->d_counter, kCounterRing * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(c->d_counter, 0, kCounterRing * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_abort, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(c->d_abort, 0, sizeof(int));
 #ifdef FDTD_PROFILE
@@ -896,12 +931,17 @@ int fdtd_step(fdtd_ctx* c, int n)
     DeviceGuard guard(c);
     if (n < 0) return fail(c, FDTD_EINVAL, "fdtd_step: n < 0");
     if (!c->fields_set) return fail(c, FDTD_ESTATE, "fdtd_step before fdtd_set_fields");
-    cudaError_t e = cudaEventRecord(c->ev0, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
+    cudaError_t e = cudaSuccess;
+    if (c->timing) {
+        e = cudaEventRecord(c->ev0, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
+    }
     const int rc = (effective_kernel(c) == FDTD_KERNEL_NAIVE) ? step_naive(c, n) : step_systolic(c, n);
-    e = cudaEventRecord(c->ev1, c->stream);
-    if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
-    c->ev_valid = true;
+    if (c->timing) {
+        e = cudaEventRecord(c->ev1, c->stream);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventRecord");
+        c->ev_valid = true;
+    }
     return rc;
 }
 
@@ -1008,11 +1048,19 @@ int fdtd_get_counters(const fdtd_ctx* c, long long out[4])
     return FDTD_OK;
 }
 
+int fdtd_set_timing(fdtd_ctx* c, int on)
+{
+    if (!c) return FDTD_EINVAL;
+    c->timing = on != 0;
+    if (!c->timing) c->ev_valid = false;
+    return FDTD_OK;
+}
+
 int fdtd_last_step_ms(fdtd_ctx* c, float* ms)
 {
     if (!c || !ms) return FDTD_EINVAL;
     DeviceGuard guard(c);
-    if (!c->ev_valid) return fail(c, FDTD_ESTATE, "fdtd_last_step_ms before fdtd_step");
+    if (!c->ev_valid) return fail(c, FDTD_ESTATE, "fdtd_last_step_ms: no timed fdtd_step call yet (fdtd_set_timing(ctx, 1) first)");
     cudaError_t e = cudaEventSynchronize(c->ev1);
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaEventSynchronize");
     e = cudaEventElapsedTime(ms, c->ev0, c->ev1);

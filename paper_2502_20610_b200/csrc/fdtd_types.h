@@ -125,7 +125,12 @@ struct SysParams {
     int ntiles;
     int* flagE;            // [ntiles]  = flag_base + (number of E phases published)
     int* flagH;            // [ntiles]
-    unsigned int* counter; // tile claim counter, zeroed before the launch
+    unsigned int* counter; // tile claim counter of this launch (zero at launch)
+    unsigned int* counter_zero;  // systolic_tma.cu: the claim counter of a launch 32 launches ahead, zeroed by this one (NULL: none)
+    // Launch-to-launch overlap (row f2, "global synchronization operations are still required"): the launch may
+    // start while the previous launch of the same tile grid is still draining (programmatic dependent launch); a tile then
+    // waits until the tiles of the previous launch that finalised the cells of its box have raised their last flag.
+    int pred_final;        // 0: the previous launch has completed (stream order); else the value those flags reach
     int* abort_flag;       // != 0: a watchdog fired; every CTA leaves
     long long spin_budget; // clock64 ticks a single wait may take
     const int* order;      // systolic_tma.cu: claim index -> tile, sorted by wavefront bx+by+bz (NULL: identity)

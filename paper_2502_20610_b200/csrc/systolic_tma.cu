@@ -48,6 +48,7 @@
 // multiples of 16 bytes); P.g.per[] only says which low walls freeze tangential E.
 #include <cuda.h>
 #include <cuda_fp16.h>
+#include <string.h>
 
 #include <type_traits>
 
@@ -984,6 +985,9 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
     __shared__ __align__(8) unsigned long long mb[MB_COUNT];
     __shared__ Ctl ctl;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // the next launch of the stream may be scheduled as soon as SMs drain (its tiles wait on flags, see pred_final)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (blockIdx.x == 0 && tid == 0 && P.counter_zero) *P.counter_zero = 0u;
     if (tid == 0) {
 #ifdef FDTD_PROFILE
         trace_on_ = 0;
@@ -1052,6 +1056,42 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
         for (int q = 0; q < 3; ++q) {
             const int wq = q == 0 ? W0 : q == 1 ? W1 : W2;
             fast = fast && (t.a[q] - k1 >= 1) && (t.a[q] - k0 + wq <= P.g.n[q]);
+        }
+        if (P.pred_final != 0 && tid < 27 && !ctl.abort) {
+            // Launch-to-launch overlap.  Read-after-write: the cells of the box [a-1, a+w) were finalised, at step T-1 of the
+            // previous launch, by the tiles whose start lies in (a-1+T-w, a+w-1+T] on every axis: two per axis, indices jlo
+            // and jlo+1.  Write-after-read: those final values are also the last minus shells of the downwind neighbours of
+            // these tiles (index +1 per axis), which must have read them before anything of this launch overwrites them.
+            // Every tile of this launch therefore waits for the last flag of the 3 x 3 x 3 tiles jlo .. jlo+2 of the previous
+            // launch (cells that reach a tile later, through shells, were covered by the tile that loaded them in its box).
+            int u = 0, div = 9;
+            const bool ok = true;
+            for (int q = 2; q >= 0; --q) {
+                const int wq = q == 0 ? W0 : q == 1 ? W1 : W2;
+                const int lo = t.a[q] - 1 + T - wq;
+                const int jlo = (lo >= 0 ? lo / wq : -((-lo + wq - 1) / wq)) + 1;      // floor(lo / w) + 1
+                // clamped to the tile grid: beyond it there is nothing to wait for on this axis, but the other axes still
+                // count, and a tile must never raise a flag that its own predecessor (same index, <= every tile waited for)
+                // has not finished with -- the flag values of the two launches share one array
+                const int j = min(max(jlo + (tid / div) % 3, 0), P.ax[q].nb - 1);
+                div /= 3;
+                u = u * P.ax[q].nb + j;
+            }
+            if (ok && ld_acquire(P.flagH + u) < P.pred_final) {
+                const long long t_start = clock64();
+                unsigned spins = 0;
+                while (ld_acquire(P.flagH + u) < P.pred_final) {
+                    if ((++spins & 63u) == 0u) {
+                        if (ld_volatile(P.abort_flag) != 0) { *(volatile int*)&ctl.abort = 1; break; }
+                        if (clock64() - t_start > P.spin_budget) {
+                            atomicExch(P.abort_flag, 1);
+                            *(volatile int*)&ctl.abort = 1;
+                            break;
+                        }
+                    }
+                    __nanosleep(64);
+                }
+            }
         }
         if (k0 > 0 && warp < NWARPS_C) {
             // started late: nothing is loaded from the grid; the box holds zero fields (registers) and zero coefficients
@@ -1273,5 +1313,16 @@ cudaError_t FDTD_TMA_NAME(launch_systolic_tma)(int coef, const SysParams& p, con
     const void* fn = p.mon.on ? (coef ? (const void*)&systolic_tma_kernel<true, true> : (const void*)&systolic_tma_kernel<false, true>)
                               : (coef ? (const void*)&systolic_tma_kernel<true, false> : (const void*)&systolic_tma_kernel<false, false>);
     void* args[] = {(void*)&p, (void*)&maps};
-    return cudaLaunchKernel(fn, dim3((unsigned)ctas), dim3((unsigned)NT), args, FDTD_TMA_NAME(systolic_tma_smem)(coef), st);
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)ctas);
+    cfg.blockDim = dim3((unsigned)NT);
+    cfg.dynamicSmemBytes = FDTD_TMA_NAME(systolic_tma_smem)(coef);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = p.pred_final != 0 ? 1 : 0;       // overlap with the previous launch only when its flags are this launch's gate
+    return cudaLaunchKernelExC(&cfg, fn, args);
 }

@@ -280,3 +280,45 @@ def test_f16_storage_fma_build_within_tolerance_and_other_schedules_rejected(cud
         with pytest.raises(binding.FdtdError) as e:
             _h16_gpu(w, 4, kernel, tile, 4)
         assert e.value.code == binding.EINVAL
+
+
+# ---- f2: launch-to-launch overlap (consecutive launches of one tile grid run concurrently, gated by per-tile flags) ----
+OVERLAP_T = [2, 3, 7, 8, 15, 16, 31, 32, 33]
+
+
+@pytest.mark.parametrize("name", ["C2s", "C5s", "C1"])
+def test_overlapping_launches_bit_exact_for_every_depth(cuda_device, oracle_cache, name):
+    """Many short launches back to back: each may start while the previous one drains.  Depths around the tile widths
+    (7, 15, 31) exercise every shape of the predecessor set."""
+    w, steps = CASES[name]
+    for T in OVERLAP_T:
+        E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=T)
+        compare((E, H), oracle_cache(name), exact=True)
+    E, H, info = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 7, 7), T=9)
+    compare((E, H), oracle_cache(name), exact=True)
+
+
+def test_overlapping_launches_under_perturbed_cta_order(cuda_device, oracle_cache, monkeypatch):
+    """The same with pseudo-random sleeps between phases (developer build), which stretch the drain of a launch far into
+    the next one; and with the overlap switched off (FDTD_NO_OVERLAP) the result is the same."""
+    w, steps = CASES["C2s"]
+    for seed, T in ((7, 4), (99, 9), (1234, 17), (5, 33)):
+        monkeypatch.setenv("FDTD_DEBUG_DELAY", str(seed))
+        E, H, _ = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=T, variant="dbg")
+        compare((E, H), oracle_cache("C2s"), exact=True)
+    monkeypatch.delenv("FDTD_DEBUG_DELAY")
+    monkeypatch.setenv("FDTD_NO_OVERLAP", "1")
+    E, H, _ = gpu_run(w, steps, binding.KERNEL_SYSTOLIC, tile=(31, 15, 7), T=9)
+    compare((E, H), oracle_cache("C2s"), exact=True)
+
+
+def test_timing_is_opt_in(cuda_device):
+    w, _ = CASES["C1"]
+    E, H, sim = binding.run_workload(w, kernel=binding.KERNEL_SYSTOLIC, steps=3)
+    with pytest.raises(binding.FdtdError) as e:
+        sim.last_step_ms()
+    assert e.value.code == binding.ESTATE
+    sim.set_timing(True)
+    sim.step(5)
+    assert sim.last_step_ms() > 0
+    sim.close()

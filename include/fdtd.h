@@ -103,6 +103,18 @@ int fdtd_load_fields(fdtd_ctx* ctx, const float* const E[3], const float* const 
  * Generator side (not the library's business): ca=(2eps-sigma dt)/(2eps+sigma dt), cb=2dt/(2eps+sigma dt). */
 int fdtd_set_coeffs(fdtd_ctx* ctx, const float* const ca[3], const float* const cb[3], const float db[3]);
 
+/* Compressed coefficients for grids of few materials (row f2; the structural fields "double the number of
+ * memory operations needed per iteration"): instead of six float arrays, one material index per cell and component and a
+ * table,   ca_a[cell] = ca_lut[a*nmat + idx[a][cell]],   cb_a[cell] = cb_lut[a*nmat + idx[a][cell]].
+ * idx[3]: host array of DEVICE pointers to nx*ny*nz bytes each (x fastest, 16-byte aligned, borrowed, read-only, values
+ * < nmat); ca_lut, cb_lut: HOST arrays [3][nmat], copied; nmat 1..256; db as in fdtd_set_coeffs.  Replaces any arrays
+ * bound with fdtd_set_coeffs (and vice versa).  The update is the one of fdtd_set_coeffs with the expanded arrays, bit for
+ * bit; the systolic kernel moves 3 bytes per entering cell instead of 24 and expands them through the table on chip.
+ * Runs FDTD_KERNEL_NAIVE and FDTD_KERNEL_SYSTOLIC (tile 31x15x7, f32 fields; a periodic axis or nx % 16 != 0 uses the
+ * padded working copy); other schedules return FDTD_EINVAL from fdtd_step. */
+int fdtd_set_coeff_lut(fdtd_ctx* ctx, const unsigned char* const idx[3], int nmat, const float* ca_lut, const float* cb_lut,
+                       const float db[3]);
+
 /* Additive soft source on one E component over a box (excluded from the paper's own benchmark, PAPER.md:106;
  * DESIGN.md reading #6): after the E half-step of step t,  E_comp[box] += amp[q] * wave[t]  while 0 <= t < nwave
  * (product rounded to fp32, then the add).  comp 0..2 = Ex,Ey,Ez; box origin (i0,j0,k0), extent (ni,nj,nk);

@@ -26,6 +26,7 @@ _PROTOS = {
     "fdtd_set_fields_f16": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "fdtd_load_fields": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
     "fdtd_set_coeffs": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_float)]),
+    "fdtd_set_coeff_lut": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]),
     "fdtd_set_source": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int,
                                   C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int]),
     "fdtd_set_monitor": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_void_p]),
@@ -165,6 +166,21 @@ class Fdtd:
         self._keep.append((ca, cb))
         dbp = None if db is None else (C.c_float * 3)(*[float(x) for x in db])
         self._check(self._lib.fdtd_set_coeffs(self._h, _ptr3(ca), _ptr3(cb), dbp))
+
+    def set_coeff_lut(self, idx, ca_lut, cb_lut, db=None):
+        """Material-index coefficients: idx = three uint8 CUDA tensors (nz, ny, nx); ca_lut, cb_lut: numpy (3, nmat)."""
+        import numpy as np
+        import torch
+        shape = (self.n[2], self.n[1], self.n[0])
+        for t in idx:
+            assert t.is_cuda and t.dtype == torch.uint8 and t.is_contiguous() and tuple(t.shape) == shape, "bad index tensor"
+        ca_lut = np.ascontiguousarray(ca_lut, dtype=np.float32)
+        cb_lut = np.ascontiguousarray(cb_lut, dtype=np.float32)
+        assert ca_lut.shape == cb_lut.shape and ca_lut.ndim == 2 and ca_lut.shape[0] == 3
+        self._keep.append(list(idx))
+        fp = C.POINTER(C.c_float)
+        dbp = None if db is None else (C.c_float * 3)(*[float(x) for x in db])
+        self._check(self._lib.fdtd_set_coeff_lut(self._h, _ptr3(idx), int(ca_lut.shape[1]), ca_lut.ctypes.data_as(fp), cb_lut.ctypes.data_as(fp), dbp))
 
     def set_source(self, comp, box, amp, wave):
         import numpy as np

@@ -24,6 +24,7 @@ struct fdtd_ctx {
     std::vector<float> h_wave;
     long long t;
     MonitorParams mon;   // running-DFT monitor in CALLER coordinates (G = 0); mon.on == 0: none
+    float* d_lut;        // device copy of the (ca, cb) table of fdtd_set_coeff_lut: [3][nmat][2]
     float* d_mon_w;      // device copy of the weight tables: wE[nt][F][2] then wH[nt][F][2]
     // schedule
     int which;
@@ -35,6 +36,7 @@ struct fdtd_ctx {
     bool use_tma;     // resolved: its TMA-staged version runs
     bool tma_by8;     // resolved: the 31x7x7 build of it (two CTAs per SM)
     bool tma_h16;     // resolved: the binary16-field-storage build of it (g.fld16)
+    bool tma_lut;     // resolved: the material-index build of it (g.cidx)
     // resolved: the TMA kernel runs on a padded working copy of the grid (periodic axis or nx % 4 != 0)
     bool use_pad;
     PadGeom pg;
@@ -116,7 +118,8 @@ int cuda_fail(fdtd_ctx* c, cudaError_t e, const char* what)
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-bool has_coef(const fdtd_ctx* c) { return c->g.ca[0] != nullptr; }
+bool has_lut(const fdtd_ctx* c) { return c->g.cidx[0] != nullptr; }
+bool has_coef(const fdtd_ctx* c) { return c->g.ca[0] != nullptr || has_lut(c); }
 
 // both-or-neither rule for the systolic kernel (the naive kernel takes any combination)
 bool coef_mixed(const fdtd_ctx* c) { return (c->g.ca[0] != nullptr) != (c->g.cb[0] != nullptr); }
@@ -167,18 +170,22 @@ int resolve_systolic(fdtd_ctx* c)
     c->use_reg = !smem_only && N[0] == 31 && N[1] == 15 && N[2] == 7;
     c->tma_by8 = c->which == FDTD_KERNEL_SYSTOLIC && N[0] == 31 && N[1] == 7 && N[2] == 7;
     c->tma_h16 = c->g.fld16 != 0;
+    c->tma_lut = has_lut(c);
+    if (c->tma_lut && (c->tma_h16 || !(c->which == FDTD_KERNEL_SYSTOLIC && N[0] == 31 && N[1] == 15 && N[2] == 7)))
+        return fail(c, FDTD_EINVAL, "material-index coefficients run FDTD_KERNEL_NAIVE or FDTD_KERNEL_SYSTOLIC with tile 31x15x7 and f32 fields");
     if (c->tma_h16 && !(c->which == FDTD_KERNEL_SYSTOLIC && N[0] == 31 && N[1] == 15 && N[2] == 7))
         return fail(c, FDTD_EINVAL, "binary16 field storage runs FDTD_KERNEL_NAIVE or FDTD_KERNEL_SYSTOLIC with tile 31x15x7");
     c->use_tma = (c->use_reg && c->which == FDTD_KERNEL_SYSTOLIC && !c->dbg_no_tma) || c->tma_by8;
-    c->use_pad = c->use_tma && (c->g.per[0] || c->g.per[1] || c->g.per[2] || c->g.n[0] % (c->tma_h16 ? 8 : 4) != 0);
+    c->use_pad = c->use_tma && (c->g.per[0] || c->g.per[1] || c->g.per[2] || c->g.n[0] % (c->tma_lut ? 16 : c->tma_h16 ? 8 : 4) != 0);
     int found = -1;
     int per_sm = 0;
     if (c->use_tma) {
-        cudaError_t e = c->tma_h16   ? systolic_tma_prepare_h16(want_coef, &per_sm)
+        cudaError_t e = c->tma_lut   ? systolic_tma_prepare_lut(want_coef, &per_sm)
+                        : c->tma_h16 ? systolic_tma_prepare_h16(want_coef, &per_sm)
                         : c->tma_by8 ? systolic_tma_prepare_by8(want_coef, &per_sm)
                                      : systolic_tma_prepare(want_coef, &per_sm);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
-        c->smem = c->tma_h16 ? systolic_tma_smem_h16(want_coef) : c->tma_by8 ? systolic_tma_smem_by8(want_coef) : systolic_tma_smem(want_coef);
+        c->smem = c->tma_lut ? systolic_tma_smem_lut(want_coef) : c->tma_h16 ? systolic_tma_smem_h16(want_coef) : c->tma_by8 ? systolic_tma_smem_by8(want_coef) : systolic_tma_smem(want_coef);
     } else if (c->use_reg) {
         cudaError_t e = systolic_reg_prepare(want_coef, &per_sm);
         if (e != cudaSuccess) return cuda_fail(c, e, "cudaFuncSetAttribute(max dynamic shared memory) / occupancy query");
@@ -228,13 +235,13 @@ int resolve_systolic(fdtd_ctx* c)
             c->pg.G[a] = c->g.per[a] ? c->T : 0;
             c->pg.m[a] = c->g.n[a] + 2 * c->pg.G[a];
         }
-        c->pg.ldx = c->tma_h16 ? (c->pg.m[0] + 7) / 8 * 8 : (c->pg.m[0] + 3) / 4 * 4;   // rows are multiples of 16 bytes
+        c->pg.ldx = c->tma_lut ? (c->pg.m[0] + 15) / 16 * 16 : c->tma_h16 ? (c->pg.m[0] + 7) / 8 * 8 : (c->pg.m[0] + 3) / 4 * 4;   // rows are multiples of 16 bytes
         cells = c->pg.ldx * c->pg.m[1] * c->pg.m[2];
         if (c->pg.m[0] > (1 << 16) || c->pg.m[1] > (1 << 16) || c->pg.m[2] > (1 << 16) || cells >= (1ll << 40))
             return fail(c, FDTD_EINVAL, "padded working grid too large; use a smaller temporal depth");
         c->pad_stride = (cells + 63) / 64 * 64;
         cudaError_t e = cudaMalloc(&c->pad_fld, (size_t)c->pad_stride * 6 * sizeof(float));
-        if (e == cudaSuccess && want_coef) e = cudaMalloc(&c->pad_coef, (size_t)c->pad_stride * 6 * sizeof(float));
+        if (e == cudaSuccess && want_coef) e = cudaMalloc(&c->pad_coef, c->tma_lut ? (size_t)c->pad_stride * 3 : (size_t)c->pad_stride * 6 * sizeof(float));
         if (e != cudaSuccess) {
             free_pad(c);
             return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(padded working copy): ") + cudaGetErrorString(e));
@@ -260,8 +267,10 @@ GridParams work_grid(const fdtd_ctx* c, long long* ldx)
         const size_t es = c->g.fld16 ? 2 : 4;
         g.E[a] = reinterpret_cast<float*>(reinterpret_cast<char*>(c->pad_fld) + es * (size_t)c->pad_stride * a);
         g.H[a] = reinterpret_cast<float*>(reinterpret_cast<char*>(c->pad_fld) + es * (size_t)c->pad_stride * (3 + a));
-        g.ca[a] = c->pad_coef ? c->pad_coef + c->pad_stride * a : nullptr;
-        g.cb[a] = c->pad_coef ? c->pad_coef + c->pad_stride * (3 + a) : nullptr;
+        const bool lutm = has_lut(c);
+        g.ca[a] = (c->pad_coef && !lutm) ? c->pad_coef + c->pad_stride * a : nullptr;
+        g.cb[a] = (c->pad_coef && !lutm) ? c->pad_coef + c->pad_stride * (3 + a) : nullptr;
+        g.cidx[a] = (c->pad_coef && lutm) ? reinterpret_cast<const unsigned char*>(c->pad_coef) + c->pad_stride * a : nullptr;
         g.n[a] = c->pg.m[a];
         g.src_box[a] = c->g.src_box[a] + c->pg.G[a];
     }
@@ -307,6 +316,7 @@ int ensure_tmaps(fdtd_ctx* c)
     }
     int box_fld[3][3], box_coef[3][3];
     if (c->tma_h16) systolic_tma_boxes_h16(box_fld, box_coef);
+    else if (c->tma_lut) systolic_tma_boxes_lut(box_fld, box_coef);
     else if (c->tma_by8) systolic_tma_boxes_by8(box_fld, box_coef);
     else systolic_tma_boxes(box_fld, box_coef);
     long long ldx = 0;
@@ -315,7 +325,7 @@ int ensure_tmaps(fdtd_ctx* c)
     for (int a = 0; a < 3; ++a) {
         arr[a] = wg.E[a];
         arr[3 + a] = wg.H[a];
-        arr[6 + a] = wg.ca[a];
+        arr[6 + a] = wg.cidx[a] ? (const void*)wg.cidx[a] : (const void*)wg.ca[a];
         arr[9 + a] = wg.cb[a];
     }
     static_assert(sizeof(CUtensorMap) * 36 == sizeof(TmaMaps), "TmaMaps layout");
@@ -325,7 +335,7 @@ int ensure_tmaps(fdtd_ctx* c)
     // arrays first..first+count-1 at one positive stride (multiple of 16 bytes, no overlap)? -> the stride, else 0
     auto uniform_stride = [&](int first, int count) -> cuuint64_t {
         if (!arr[first] || c->dbg_no_group) return 0;
-        const cuuint64_t nbytes = ncells * ((first < 6 && c->g.fld16) ? 2u : 4u);
+        const cuuint64_t nbytes = ncells * ((first < 6 && c->g.fld16) ? 2u : (first >= 6 && has_lut(c)) ? 1u : 4u);
         const char* b0 = (const char*)arr[first];
         const char* b1 = (const char*)arr[first + 1];
         if (b1 <= b0) return 0;
@@ -338,14 +348,15 @@ int ensure_tmaps(fdtd_ctx* c)
     auto encode_maps = [&](CUtensorMap* dst, const void* base, int narr, cuuint64_t astride, bool fld) -> int {
         // extents are the logical grid (elements beyond it are delivered as zeros), strides follow the row pitch
         const bool h16 = fld && c->g.fld16;
-        const cuuint64_t es = h16 ? 2u : 4u;
+        const bool u8 = !fld && has_lut(c);
+        const cuuint64_t es = h16 ? 2u : u8 ? 1u : 4u;
         const int (*box)[3] = fld ? box_fld : box_coef;
         const cuuint64_t dims[4] = {(cuuint64_t)wg.n[0], (cuuint64_t)wg.n[1], (cuuint64_t)wg.n[2], (cuuint64_t)narr};
         const cuuint64_t strides[3] = {(cuuint64_t)ldx * es, (cuuint64_t)ldx * wg.n[1] * es, astride};
         const cuuint32_t estr[4] = {1, 1, 1, 1};
         for (int f = 0; f < 3; ++f) {
             const cuuint32_t b[4] = {(cuuint32_t)box[f][0], (cuuint32_t)box[f][1], (cuuint32_t)box[f][2], (cuuint32_t)narr};
-            const CUresult r = encode(dst + f, h16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, narr > 1 ? 4 : 3, const_cast<void*>(base), dims, strides, b, estr,
+            const CUresult r = encode(dst + f, h16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : u8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, narr > 1 ? 4 : 3, const_cast<void*>(base), dims, strides, b, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) {
@@ -357,7 +368,7 @@ int ensure_tmaps(fdtd_ctx* c)
         return FDTD_OK;
     };
     // groups: E = arrays 0..2 (slot 0), H = 3..5 (slot 9), coefficients = 6..11 (slot 18)
-    const int first[3] = {0, 3, 6}, count[3] = {3, 3, 6};
+    const int first[3] = {0, 3, 6}, count[3] = {3, 3, has_lut(c) ? 3 : 6};
     for (int g = 0; g < 3; ++g) {
         c->tma_group[g] = 0;
         if (!arr[first[g]]) continue;
@@ -368,7 +379,7 @@ int ensure_tmaps(fdtd_ctx* c)
         if (d) {
             c->tma_group[g] = 1;
             rc = encode_maps(dst, arr[first[g]], count[g], d, g < 2);
-        } else if (g == 2 && (da = uniform_stride(6, 3)) && (db = uniform_stride(9, 3))) {
+        } else if (g == 2 && !has_lut(c) && (da = uniform_stride(6, 3)) && (db = uniform_stride(9, 3))) {
             c->tma_group[g] = 2;
             rc = encode_maps(dst, arr[6], 3, da, false);
             if (rc == FDTD_OK) rc = encode_maps(dst + 9, arr[9], 3, db, false);
@@ -505,11 +516,11 @@ int step_systolic(fdtd_ctx* c, int n)
         for (int a = 0; a < 3; ++a) {
             pf.usr[a] = c->g.E[a];
             pf.usr[3 + a] = c->g.H[a];
-            pc.usr[a] = const_cast<float*>(c->g.ca[a]);
+            pc.usr[a] = has_lut(c) ? reinterpret_cast<float*>(const_cast<unsigned char*>(c->g.cidx[a])) : const_cast<float*>(c->g.ca[a]);
             pc.usr[3 + a] = const_cast<float*>(c->g.cb[a]);
         }
         pf.ext = c->pad_fld; pf.stride = c->pad_stride; pf.narr = 6; pf.elem16 = c->g.fld16;
-        pc.ext = c->pad_coef; pc.stride = c->pad_stride; pc.narr = 6;
+        pc.ext = c->pad_coef; pc.stride = c->pad_stride; pc.narr = has_lut(c) ? 3 : 6; pc.elem16 = has_lut(c) ? 2 : 0;
         if (c->pad_coef && !c->pad_coef_valid) {           // constants of the run: copied (with their images) once
             cudaError_t e = launch_pad_copy_in(c->pg, pc, c->stream);
             if (e != cudaSuccess) return cuda_fail(c, e, "padded copy of the coefficient arrays");
@@ -610,7 +621,8 @@ int step_systolic(fdtd_ctx* c, int n)
             if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         }
         const int ctas = ntiles < c->ctas ? (int)ntiles : c->ctas;
-        e = c->tma_h16   ? launch_systolic_tma_h16(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
+        e = c->tma_lut   ? launch_systolic_tma_lut(1, P, c->tmaps, ctas, c->stream)
+            : c->tma_h16 ? launch_systolic_tma_h16(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->tma_by8 ? launch_systolic_tma_by8(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->use_tma ? launch_systolic_tma(has_coef(c) ? 1 : 0, P, c->tmaps, ctas, c->stream)
             : c->use_reg ? launch_systolic_reg(has_coef(c) ? 1 : 0, P, ctas, c->stream)
@@ -705,6 +717,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->use_tma = false;
     c->tma_by8 = false;
     c->tma_h16 = false;
+    c->tma_lut = false;
+    c->d_lut = nullptr;
     c->use_pad = false;
     c->pad_fld = c->pad_coef = nullptr;
     c->pad_stride = 0;
@@ -848,10 +862,51 @@ int fdtd_set_coeffs(fdtd_ctx* c, const float* const ca[3], const float* const cb
         c->g.ca[a] = ca ? ca[a] : nullptr;
         c->g.cb[a] = cb ? cb[a] : nullptr;
         c->g.db[a] = db ? db[a] : c->dt;
+        c->g.cidx[a] = nullptr;          // coefficient arrays replace a material-index binding
     }
+    c->g.lut = nullptr;
+    c->g.nmat = 0;
     c->cfg_idx = -1;   // the coefficient-carrying kernels are separate instantiations
     c->resolved = false;
     c->tmaps_valid = false;
+    c->pad_coef_valid = false;
+    return FDTD_OK;
+}
+
+int fdtd_set_coeff_lut(fdtd_ctx* c, const unsigned char* const idx[3], int nmat, const float* ca_lut, const float* cb_lut, const float db[3])
+{
+    if (!c) return FDTD_EINVAL;
+    DeviceGuard guard(c);
+    if (!idx || !ca_lut || !cb_lut || nmat < 1 || nmat > 256) return fail(c, FDTD_EINVAL, "fdtd_set_coeff_lut: NULL argument or nmat outside 1..256");
+    for (int a = 0; a < 3; ++a) {
+        if (!idx[a] || !aligned16(idx[a])) return fail(c, FDTD_EINVAL, "fdtd_set_coeff_lut: idx needs three 16-byte aligned device pointers");
+        if (db && !isfinite(db[a])) return fail(c, FDTD_EINVAL, "fdtd_set_coeff_lut: db not finite");
+    }
+    cudaError_t e = cudaStreamSynchronize(c->stream);   // the old table may still be in use
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
+    if (c->d_lut) cudaFree(c->d_lut);
+    c->d_lut = nullptr;
+    std::vector<float> h((size_t)3 * nmat * 2);
+    for (int a = 0; a < 3; ++a)
+        for (int m = 0; m < nmat; ++m) {
+            h[((size_t)a * nmat + m) * 2] = ca_lut[a * nmat + m];
+            h[((size_t)a * nmat + m) * 2 + 1] = cb_lut[a * nmat + m];
+        }
+    e = cudaMalloc(&c->d_lut, h.size() * sizeof(float));
+    if (e != cudaSuccess) return fail(c, FDTD_ENOMEM, std::string("cudaMalloc(coefficient table): ") + cudaGetErrorString(e));
+    e = cudaMemcpy(c->d_lut, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemcpy(coefficient table)");
+    for (int a = 0; a < 3; ++a) {
+        c->g.cidx[a] = idx[a];
+        c->g.ca[a] = c->g.cb[a] = nullptr;
+        c->g.db[a] = db ? db[a] : c->dt;
+    }
+    c->g.lut = c->d_lut;
+    c->g.nmat = nmat;
+    c->cfg_idx = -1;
+    c->resolved = false;
+    c->tmaps_valid = false;
+    c->pad_coef_valid = false;
     return FDTD_OK;
 }
 
@@ -1132,6 +1187,7 @@ void fdtd_destroy(fdtd_ctx* c)
     if (c->d_amp) cudaFree(c->d_amp);
     if (c->d_wave) cudaFree(c->d_wave);
     if (c->d_mon_w) cudaFree(c->d_mon_w);
+    if (c->d_lut) cudaFree(c->d_lut);
     if (c->d_flags) cudaFree(c->d_flags);
     if (c->d_counter) cudaFree(c->d_counter);
     if (c->d_abort) cudaFree(c->d_abort);

@@ -46,6 +46,13 @@ void systolic_tma_boxes_h16(int fld[3][3], int coef[3][3]);
 cudaError_t systolic_tma_prepare_h16(int coef, int* blocks_per_sm);
 cudaError_t launch_systolic_tma_h16(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
 
+// implemented in systolic_tma_lut.cu: the same kernel for material-index coefficients (GridParams::cidx), tile 31x15x7, coef = 1
+size_t systolic_tma_smem_lut(int coef);
+int systolic_tma_threads_lut();
+void systolic_tma_boxes_lut(int fld[3][3], int coef[3][3]);
+cudaError_t systolic_tma_prepare_lut(int coef, int* blocks_per_sm);
+cudaError_t launch_systolic_tma_lut(int coef, const SysParams& p, const TmaMaps& maps, int ctas, cudaStream_t st);
+
 // implemented in pad_kernels.cu: copies between the caller's arrays and the padded working copy (periodic images)
 cudaError_t launch_pad_copy_in(const PadGeom& g, const PadArrays& a, cudaStream_t st);     // all padded cells <- images
 cudaError_t launch_pad_ghost_fill(const PadGeom& g, const PadArrays& a, cudaStream_t st);  // ghost cells <- interior

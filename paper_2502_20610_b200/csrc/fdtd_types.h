@@ -18,6 +18,11 @@ struct GridParams {
     float* H[3];
     const float* ca[3];  // all NULL or all set
     const float* cb[3];  // all NULL or all set
+    // compressed coefficients (row f2): one material index per cell and component and a table of (ca, cb)
+    // pairs per component; replaces ca / cb (which are then NULL):  ca_a[p] = lut[(a*nmat + cidx[a][p])*2], cb_a[p] = ...*2 + 1
+    const unsigned char* cidx[3];   // all NULL or all set
+    const float* lut;               // device, [3][nmat][2]
+    int nmat;
     int fld16;           // 1: E and H point to IEEE binary16 arrays (row f1); arithmetic stays f32
     int n[3];
     int per[3];          // 1 = periodic axis
@@ -86,7 +91,7 @@ struct PadArrays {
     float* ext;           // narr padded arrays of ldx*m[1]*m[2] elements at a uniform stride
     long long stride;     // in elements
     int narr;
-    int elem16;           // 1: the arrays hold binary16 elements (usr / ext are then __half arrays behind float pointers)
+    int elem16;           // 1: binary16 elements, 2: one-byte elements (material indices); usr / ext then hide them behind float pointers
 };
 
 // Running-DFT monitor on one plane of the grid (PAPER.md:106 names outputs as what real runs carry;

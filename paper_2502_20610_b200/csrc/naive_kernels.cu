@@ -116,7 +116,8 @@ __global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__
     const long long ym_off = (j > 0) ? -(long long)nx : (long long)nx * (ny - 1);
     const long long xm_off = (i0 > 0) ? -1 : (long long)(nx - 1);
     const float rdx = g.rd[0], rdy = g.rd[1], rdz = g.rd[2];
-    const bool has_ca = g.ca[0] != nullptr, has_cb = g.cb[0] != nullptr;
+    const bool has_lut = g.cidx[0] != nullptr;       // material-index tables instead of coefficient arrays (row f2)
+    const bool has_ca = g.ca[0] != nullptr || has_lut, has_cb = g.cb[0] != nullptr || has_lut;
     const FT* __restrict__ Hx = reinterpret_cast<const FT*>(g.H[0]);
     const FT* __restrict__ Hy = reinterpret_cast<const FT*>(g.H[1]);
     const FT* __restrict__ Hz = reinterpret_cast<const FT*>(g.H[2]);
@@ -148,8 +149,19 @@ __global__ void __launch_bounds__(kThreads) e_half_naive(const __grid_constant__
         ldv<VEC>(Ey + p, ey);
         ldv<VEC>(Ez + p, ez);
         float ca0[VEC], ca1[VEC], ca2[VEC], cb0[VEC], cb1[VEC], cb2[VEC];
-        if (has_ca) { ldv<VEC>(g.ca[0] + p, ca0); ldv<VEC>(g.ca[1] + p, ca1); ldv<VEC>(g.ca[2] + p, ca2); }
-        if (has_cb) { ldv<VEC>(g.cb[0] + p, cb0); ldv<VEC>(g.cb[1] + p, cb1); ldv<VEC>(g.cb[2] + p, cb2); }
+        if (has_lut) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const int m0 = g.cidx[0][p + v], m1 = g.cidx[1][p + v], m2 = g.cidx[2][p + v];
+                const float2 q0 = __ldg(reinterpret_cast<const float2*>(g.lut) + m0);
+                const float2 q1 = __ldg(reinterpret_cast<const float2*>(g.lut) + g.nmat + m1);
+                const float2 q2 = __ldg(reinterpret_cast<const float2*>(g.lut) + 2 * g.nmat + m2);
+                ca0[v] = q0.x; cb0[v] = q0.y; ca1[v] = q1.x; cb1[v] = q1.y; ca2[v] = q2.x; cb2[v] = q2.y;
+            }
+        } else {
+            if (has_ca) { ldv<VEC>(g.ca[0] + p, ca0); ldv<VEC>(g.ca[1] + p, ca1); ldv<VEC>(g.ca[2] + p, ca2); }
+            if (has_cb) { ldv<VEC>(g.cb[0] + p, cb0); ldv<VEC>(g.cb[1] + p, cb1); ldv<VEC>(g.cb[2] + p, cb2); }
+        }
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             const bool wall_x = !perx && (i0 + v) == 0;

@@ -74,21 +74,24 @@ __global__ void __launch_bounds__(kThreads) pad_copy_out_kernel(PadGeom g, PadAr
 
 cudaError_t launch_pad_copy_in(const PadGeom& g, const PadArrays& a, cudaStream_t st)
 {
-    if (a.elem16) pad_copy_in_kernel<__half><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
+    if (a.elem16 == 2) pad_copy_in_kernel<unsigned char><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
+    else if (a.elem16) pad_copy_in_kernel<__half><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
     else pad_copy_in_kernel<float><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_pad_ghost_fill(const PadGeom& g, const PadArrays& a, cudaStream_t st)
 {
-    if (a.elem16) pad_ghost_fill_kernel<__half><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
+    if (a.elem16 == 2) pad_ghost_fill_kernel<unsigned char><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
+    else if (a.elem16) pad_ghost_fill_kernel<__half><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
     else pad_ghost_fill_kernel<float><<<dim3((unsigned)((long long)g.m[1] * g.m[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
     return cudaGetLastError();
 }
 
 cudaError_t launch_pad_copy_out(const PadGeom& g, const PadArrays& a, cudaStream_t st)
 {
-    if (a.elem16) pad_copy_out_kernel<__half><<<dim3((unsigned)((long long)g.n[1] * g.n[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
+    if (a.elem16 == 2) pad_copy_out_kernel<unsigned char><<<dim3((unsigned)((long long)g.n[1] * g.n[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
+    else if (a.elem16) pad_copy_out_kernel<__half><<<dim3((unsigned)((long long)g.n[1] * g.n[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
     else pad_copy_out_kernel<float><<<dim3((unsigned)((long long)g.n[1] * g.n[2]), (unsigned)a.narr), kThreads, 0, st>>>(g, a);
     return cudaGetLastError();
 }

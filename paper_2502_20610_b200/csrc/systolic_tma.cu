@@ -116,6 +116,22 @@ static_assert((FZF * sizeof(fld_t)) % 128 == 0 && (FYF * sizeof(fld_t)) % 128 ==
 __device__ __forceinline__ int zidxF(int a, int ly, int x) { return a * FZF + ly * RXF + x; }
 __device__ __forceinline__ int yidxF(int a, int l, int x) { return 3 * FZF + a * FYF + (l - 1) * RXF + x; }
 __device__ __forceinline__ int xidxF(int a, int ly, int l) { return 3 * (FZF + FYF) + a * FXF + ((l - 1) * BY + ly) * CWF; }
+// Compressed coefficients (row f2, "doubles the number of memory operations"): FDTD_COEF_LUT builds
+// (systolic_tma_lut.cu) read one material index (a byte) per cell and component instead of two floats and expand it through
+// a table of (ca, cb) pairs held in shared memory when the cell ENTERS the chip; the resident copy stays a float2 pair, so
+// the E phase is the one of the coefficient-array build.  A byte box needs 16 elements per 16 bytes: index boxes start at
+// o0 & ~15, are 48 cells wide, and the x column box is 16 cells wide.
+#ifndef FDTD_COEF_LUT
+#define FDTD_COEF_LUT 0
+#endif
+constexpr bool LUT = FDTD_COEF_LUT != 0;
+constexpr int RXB = BX + 16, CWB = 16, MAXMAT = 256;
+constexpr int ZB = RXB * BY, YB = RXB * BZ, XB = CWB * BY * W2;              // bytes of one index array's shell pieces
+static_assert(ZB % 128 == 0 && YB % 128 == 0 && XB % 128 == 0, "TMA destinations are 128-byte aligned");
+constexpr int B_ARR = (ZB + YB + XB) / 4;                                    // floats of staging per index array and step
+__device__ __forceinline__ int zidxB(int a, int ly, int x) { return a * ZB + ly * RXB + x; }
+__device__ __forceinline__ int yidxB(int a, int l, int x) { return 3 * ZB + a * YB + (l - 1) * RXB + x; }
+__device__ __forceinline__ int xidxB(int a, int ly, int l) { return 3 * (ZB + YB) + a * XB + ((l - 1) * BY + ly) * CWB; }
 // coefficient arrays are always f32
 constexpr int RX = BX + 4;
 constexpr int FZ = RX * BY;                  // box (36,16,1)   [y][x]      576 floats: plane l_z = 0
@@ -136,7 +152,8 @@ struct Lay {
     static constexpr int stgh = 0;
     static constexpr int stge = stgh + 3 * F_ARR_F;
     static constexpr int stgc = stge + 3 * F_ARR_F;
-    static constexpr int xpkh = stgc + (COEF ? 6 * F_ARR : 0);
+    static constexpr int lut = stgc + (COEF ? (LUT ? 3 * B_ARR : 6 * F_ARR) : 0);     // (ca, cb) table [3][MAXMAT] of the index build
+    static constexpr int xpkh = lut + (COEF && LUT ? 3 * MAXMAT * 2 : 0);
     static constexpr int xpke = xpkh + XPK;
     static constexpr int xoute = xpke + XPK;           // leaving x column of E, [y slot][component][8], stored by the signal warp
     static constexpr int xouth = xoute + XPK;
@@ -361,6 +378,27 @@ __device__ __forceinline__ void issue_shell(const CUtensorMap* maps, int grouped
     }
 }
 
+// the same for the three material-index arrays (bytes): maps[0..2] one 4-D map per piece when grouped, else maps[a*3 + piece]
+__device__ __forceinline__ void issue_index_shell(const CUtensorMap* maps, int grouped, float* stg, int o0, int o1, int o2, unsigned long long* bar)
+{
+    const int q0 = o0 & ~(CWB - 1);
+    mbar_expect_tx(bar, 3u * (unsigned)(ZB + YB + XB));
+    float* dz = stg;
+    float* dy = stg + 3 * ZB / 4;
+    float* dx = stg + 3 * (ZB + YB) / 4;
+    if (grouped == 1) {
+        tma_load_4d(dz, maps + 0, q0, o1, o2, 0, bar);
+        tma_load_4d(dy, maps + 1, q0, o1, o2 + 1, 0, bar);
+        tma_load_4d(dx, maps + 2, q0, o1, o2 + 1, 0, bar);
+    } else {
+        for (int a = 0; a < 3; ++a) {
+            tma_load_3d(dz + a * ZB / 4, maps + a * 3 + 0, q0, o1, o2, bar);
+            tma_load_3d(dy + a * YB / 4, maps + a * 3 + 1, q0, o1, o2 + 1, bar);
+            tma_load_3d(dx + a * XB / 4, maps + a * 3 + 2, q0, o1, o2 + 1, bar);
+        }
+    }
+}
+
 // cb mask of component c for the cell at (gx,gy,gz) when there are no coefficient arrays: dt inside the grid, 0 on
 // frozen wall components and outside the grid
 __device__ __forceinline__ float cb_mask(const SysParams& P, int c, int gx, int gy, int gz)
@@ -389,9 +427,11 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const float* stg = sm + Lay<COEF>::stgc;
+    const unsigned char* stgb = reinterpret_cast<const unsigned char*>(sm + Lay<COEF>::stgc);
+    const float2* lut = reinterpret_cast<const float2*>(sm + Lay<COEF>::lut);
     float* const cmask = sm + Lay<COEF>::coef;
     float2* const cpair = reinterpret_cast<float2*>(sm + Lay<COEF>::coef);
-    const int r0 = o0 & 3;
+    const int r0 = o0 & 3, r0b = o0 & (CWB - 1);
     const bool wall = (o0 <= 0) | (o1 <= 0) | (o2 <= 0);   // CTA-uniform: only then can a shell cell be frozen
     auto put = [&](int slot, int gx, int gy, int gz, const float (&v)[6]) {
 #pragma unroll
@@ -400,12 +440,22 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
             else cmask[slot + c * (BZ * PLANE)] = cb_mask(P, c, gx, gy, gz);
         }
     };
+    // index build: the staged bytes of a cell -> its three (ca, cb) pairs.  A cell outside the grid was delivered as index 0
+    // (TMA zero fill), which is a real material: it gets (0, 0) like the zero-filled arrays of the other build.
+    auto expand = [&](int b0, int b1, int b2, int gx, int gy, int gz, float (&v)[6]) {
+        const bool in = ((unsigned)gx < (unsigned)P.g.n[0]) & ((unsigned)gy < (unsigned)P.g.n[1]) & ((unsigned)gz < (unsigned)P.g.n[2]);
+        const float2 p0 = lut[stgb[b0]], p1 = lut[MAXMAT + stgb[b1]], p2 = lut[2 * MAXMAT + stgb[b2]];
+        v[0] = in ? p0.x : 0.0f; v[3] = in ? p0.y : 0.0f;
+        v[1] = in ? p1.x : 0.0f; v[4] = in ? p1.y : 0.0f;
+        v[2] = in ? p2.x : 0.0f; v[5] = in ? p2.y : 0.0f;
+    };
     // the entering plane: this thread's own cells
 #pragma unroll
     for (int r = 0; r < NROW; ++r) {
         float v[6];
 #pragma unroll
-        for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[zidx<6>(c, ly[r], r0 + lx)] : 0.0f;
+        for (int c = 0; c < 6; ++c) v[c] = (COEF && !LUT) ? stg[zidx<6>(c, ly[r], r0 + lx)] : 0.0f;
+        if (COEF && LUT) expand(zidxB(0, ly[r], r0b + lx), zidxB(1, ly[r], r0b + lx), zidxB(2, ly[r], r0b + lx), o0 + lx, o1 + ly[r], o2, v);
         put((o2 & (BZ - 1)) * PLANE + (ys0 + r) * SX + lane, o0 + lx, o1 + ly[r], o2, v);
     }
     constexpr int ROW_WARPS = W2, COL_WARPS = (W1 * W2 + 31) / 32;
@@ -415,7 +465,8 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
         const int l = it + 1, gx = o0 + lane;
         float v[6];
 #pragma unroll
-        for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
+        for (int c = 0; c < 6; ++c) v[c] = (COEF && !LUT) ? stg[yidx<6>(c, l, r0 + lane)] : 0.0f;
+        if (COEF && LUT) expand(yidxB(0, l, r0b + lane), yidxB(1, l, r0b + lane), yidxB(2, l, r0b + lane), gx, o1, o2 + l, v);
         put(((o2 + l) & (BZ - 1)) * PLANE + (o1 & (BY - 1)) * SX + (gx & (BX - 1)), gx, o1, o2 + l, v);
     } else {                                   // the entering column: idx = (l-1)*W1 + (ly-1)
         const int idx = (it - ROW_WARPS) * 32 + lane;
@@ -423,7 +474,8 @@ __device__ __forceinline__ void absorb_coef_shell(const SysParams& P, float* sm,
             const int cy = 1 + idx % W1, l = 1 + idx / W1;
             float v[6];
 #pragma unroll
-            for (int c = 0; c < 6; ++c) v[c] = COEF ? stg[xidx<6>(c, cy, l) + r0] : 0.0f;
+            for (int c = 0; c < 6; ++c) v[c] = (COEF && !LUT) ? stg[xidx<6>(c, cy, l) + r0] : 0.0f;
+            if (COEF && LUT) expand(xidxB(0, cy, l) + r0b, xidxB(1, cy, l) + r0b, xidxB(2, cy, l) + r0b, o0, o1 + cy, o2 + l, v);
             put(((o2 + l) & (BZ - 1)) * PLANE + ((o1 + cy) & (BY - 1)) * SX + (o0 & (BX - 1)), o0, o1 + cy, o2 + l, v);
         }
     }
@@ -639,7 +691,11 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
                     const int cidx = r * SX + (gz & (BZ - 1)) * PLANE;
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
-                        if (COEF) {
+                        if (COEF && LUT) {
+                            const float2* lut = reinterpret_cast<const float2*>(sm + Lay<COEF>::lut);
+                            const float2 pr = ok ? lut[c * MAXMAT + __ldg(P.g.cidx[c] + off)] : make_float2(0.0f, 0.0f);
+                            cpair[cidx + c * (BZ * PLANE)] = coef_pair(P, c, pr.x, pr.y, gx, gy[r], gz);
+                        } else if (COEF) {
                             const float a = ok ? __ldg(P.g.ca[c] + off) : 0.0f;
                             const float b = ok ? __ldg(P.g.cb[c] + off) : 0.0f;
                             cpair[cidx + c * (BZ * PLANE)] = coef_pair(P, c, a, b, gx, gy[r], gz);
@@ -1012,6 +1068,12 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
     // the garbage must be finite.  Shared memory keeps the bits of earlier kernels (possibly NaN patterns), so it is
     // cleared once per CTA; from then on every value in it derives from finite data.
     for (int i = tid; i < Lay<COEF>::total; i += NT) sm[i] = 0.0f;
+    if (COEF && LUT) {      // the (ca, cb) table of the index build: [3][nmat] pairs from global memory, rest stays 0
+        __syncthreads();
+        const float2* src = reinterpret_cast<const float2*>(P.g.lut);
+        float2* dst = reinterpret_cast<float2*>(sm + Lay<COEF>::lut);
+        for (int i = tid; i < 3 * P.g.nmat; i += NT) dst[(i / P.g.nmat) * MAXMAT + i % P.g.nmat] = src[i];
+    }
     const CUtensorMap* maps = reinterpret_cast<const CUtensorMap*>(M.bytes);   // [E0 E1 E2 H0 H1 H2 ca0..2 cb0..2][3 faces]
     // Acquire the flags of step k+1 (and run the ~0.7 us proxy fence) while the copy of step k is in flight, instead of
     // at the top of iteration k+1.  Measured: +5 % at 768^3 without coefficient arrays, -2 % on config 2 with them (the
@@ -1170,7 +1232,10 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                         if (k > hk0) { mbar_wait(mb + MB_CFREE, n_cfree & 1u); ++n_cfree; }
                         PROF_MARK(0);
                         TRACE(2, 1, k);
-                        if (lane == 0 && !FDTD_DBG(P, 2)) issue_shell<6, false>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        if (lane == 0 && !FDTD_DBG(P, 2)) {
+                            if (LUT) issue_index_shell(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                            else issue_shell<6, false>(maps + 6 * 3, P.tma_group[2], sm + Lay<COEF>::stgc, o0, o1, o2, mb + MB_CFULL);
+                        }
                         __syncwarp();
                         PROF_MARK(1);
                         }
@@ -1289,7 +1354,7 @@ int FDTD_TMA_NAME(systolic_tma_threads)() { return NT; }
 void FDTD_TMA_NAME(systolic_tma_boxes)(int fld[3][3], int coef[3][3])
 {
     const int bf[3][3] = {{RXF, BY, 1}, {RXF, 1, BZ}, {CWF, BY, W2}};
-    const int bc[3][3] = {{RX, BY, 1}, {RX, 1, BZ}, {4, BY, W2}};
+    const int bc[3][3] = {{LUT ? RXB : RX, BY, 1}, {LUT ? RXB : RX, 1, BZ}, {LUT ? CWB : 4, BY, W2}};
     for (int f = 0; f < 3; ++f)
         for (int q = 0; q < 3; ++q) {
             fld[f][q] = bf[f][q];

@@ -283,6 +283,36 @@ def make_coeffs(w: Workload, window=None, device=None):
     return ca, cb
 
 
+def make_coeff_lut(w: Workload, window=None, device=None):
+    """Material-index form of make_coeffs for the few-material workloads (C2 "blocks": eps in {1.0, 2.1, 12.1}; C3
+    "waveguide": cladding 2.1 / core 12.1): -> (idx, ca_lut, cb_lut) with idx = three uint8 per-cell arrays and
+    ca_lut, cb_lut float32 arrays of shape (3, nmat), such that ca_lut[a][idx[a]] == make_coeffs(w)[0][a] bit for bit
+    (the same double expression, rounded once).  None for the other workloads."""
+    if w.coeffs not in ("blocks", "waveguide"):
+        return None
+    i, j, k, idx = _lin_index(w.n, window, like=device)
+    if w.coeffs == "blocks":
+        nbx, nby = (w.n[0] + 7) // 8, (w.n[1] + 7) // 8
+        bid = (i >> 3) + nbx * ((j >> 3) + nby * (k >> 3))
+        sel = hash24(w.seed, AID_BLOCK, bid) % 3 + 0 * idx
+        eps_of = [1.0, 2.1, 12.1]
+    else:
+        j0, j1, k0, k1 = waveguide_rect(w.n)
+        core = (j >= j0) & (j < j1) & (k >= k0) & (k < k1)
+        sel = core * 1 + 0 * idx
+        eps_of = [2.1, 12.1]
+    if isinstance(sel, np.ndarray):
+        m = np.ascontiguousarray(sel.astype(np.uint8))
+        mats = [m, m.copy(), m.copy()]
+    else:
+        import torch
+        m = sel.to(torch.uint8).contiguous()
+        mats = [m, m.clone(), m.clone()]
+    ca_lut = np.ones((3, len(eps_of)), np.float32)
+    cb_lut = np.array([[np.float32(w.dt * (1.0 + 1.0) / (2.0 * e)) for e in eps_of]] * 3, np.float32)
+    return mats, ca_lut, cb_lut
+
+
 # ----------------------------------------------------------------------------------------------
 # sources (host tables, computed in double then rounded: oracle and GPU consume identical bits)
 # ----------------------------------------------------------------------------------------------

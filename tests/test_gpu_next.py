@@ -322,3 +322,77 @@ def test_timing_is_opt_in(cuda_device):
     sim.step(5)
     assert sim.last_step_ms() > 0
     sim.close()
+
+
+# ---- f2: material-index coefficients (fdtd_set_coeff_lut) ------------------------------------------------------------
+def test_lut_recipe_expands_to_the_coefficient_arrays():
+    """(no GPU needed, but it guards the GPU cases below) the index form of a workload is its array form, bit for bit."""
+    for name in ("C2s", "C3s", "allper"):
+        w, _ = CASES[name]
+        ca, cb = workloads.make_coeffs(w)
+        idx, ca_lut, cb_lut = workloads.make_coeff_lut(w)
+        for a in range(3):
+            assert idx[a].dtype == np.uint8 and int(idx[a].max()) < ca_lut.shape[1]
+            assert np.array_equal(ca_lut[a][idx[a]], ca[a]) and np.array_equal(cb_lut[a][idx[a]], cb[a])
+
+
+LUT_RUNS = [("C2s", "naive", 0), ("C3s", "naive", 0), ("allper", "naive", 0),
+            ("C2s", "systolic", 32), ("C2s", "systolic", 5), ("C2s", "systolic", 128), ("C3s", "systolic", 16), ("C3s", "systolic", 7),
+            ("allper", "systolic", 5)]
+
+
+@pytest.mark.parametrize("name,kernel,T", LUT_RUNS)
+def test_lut_coefficients_match_oracle_bit_exact(cuda_device, oracle_cache, name, kernel, T):
+    """The oracle runs on the expanded arrays (the definition of the table form); the CUDA path reads bytes and a table."""
+    import torch
+    w, steps = CASES[name]
+    dev = torch.device("cuda:0")
+    E, H = workloads.make_fields(w, device=dev)
+    idx, ca_lut, cb_lut = workloads.make_coeff_lut(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+    sim.set_fields(E, H)
+    sim.set_coeff_lut(idx, ca_lut, cb_lut)
+    src = workloads.make_source(w)
+    if src is not None:
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_NAIVE if kernel == "naive" else binding.KERNEL_SYSTOLIC, (31, 15, 7) if kernel == "systolic" else None, T)
+    sim.step(steps // 2)
+    sim.step(steps - steps // 2)
+    sim.sync()
+    sim.close()
+    compare(([x.cpu().numpy() for x in E], [x.cpu().numpy() for x in H]), oracle_cache(name), exact=True)
+
+
+def test_lut_per_component_tables_and_rebinding(cuda_device):
+    """Three different index arrays and three different tables (lossy materials), then back to arrays on the same context."""
+    import torch
+    w = workloads.config(4).scaled((64, 40, 36), steps=60)
+    rng = np.random.default_rng(17)
+    shape = (w.n[2], w.n[1], w.n[0])
+    nmat = 7
+    idx_h = [rng.integers(0, nmat, shape).astype(np.uint8) for _ in range(3)]
+    ca_lut = rng.uniform(0.97, 1.0, (3, nmat)).astype(np.float32)
+    cb_lut = rng.uniform(0.02, 0.25, (3, nmat)).astype(np.float32)
+    ca_h = [np.ascontiguousarray(ca_lut[a][idx_h[a]]) for a in range(3)]
+    cb_h = [np.ascontiguousarray(cb_lut[a][idx_h[a]]) for a in range(3)]
+    E, H = workloads.make_fields(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca_h, cb_h, None)
+    src = workloads.make_source(w)
+    orc.set_source(src.comp, src.box, src.amp, src.wave)
+    orc.step(60)
+    dev = torch.device("cuda:0")
+    for mode in ("lut", "arrays", "lut-naive"):
+        Ed, Hd = workloads.make_fields(w, device=dev)
+        sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+        sim.set_fields(Ed, Hd)
+        if mode == "arrays":           # bind the table first, then replace it by arrays
+            sim.set_coeff_lut([torch.from_numpy(a).to(dev) for a in idx_h], ca_lut, cb_lut)
+            sim.set_coeffs([torch.from_numpy(a).to(dev) for a in ca_h], [torch.from_numpy(a).to(dev) for a in cb_h], None)
+        else:
+            sim.set_coeff_lut([torch.from_numpy(a).to(dev) for a in idx_h], ca_lut, cb_lut)
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+        sim.set_kernel(binding.KERNEL_NAIVE if mode == "lut-naive" else binding.KERNEL_SYSTOLIC, None, 0 if mode == "lut-naive" else 16)
+        sim.step(60)
+        sim.sync()
+        sim.close()
+        compare(([x.cpu().numpy() for x in Ed], [x.cpu().numpy() for x in Hd]), (E, H), exact=True)

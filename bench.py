@@ -52,6 +52,8 @@ def parse():
                     help="nofma = the product library (bit-exact); fma = optional contracted build")
     ap.add_argument("--storage", default="f32", choices=["f32", "f16"],
                     help="f16 = binary16 field storage with f32 arithmetic (row f1, PAPER.md:104); the headline is f32")
+    ap.add_argument("--coeffs", default="arrays", choices=["arrays", "lut"],
+                    help="lut = material-index coefficients (row f2, PAPER.md:103); configs 2 and 3 only; the headline uses arrays")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sweep", action="store_true")
@@ -105,22 +107,22 @@ class ClockSampler(threading.Thread):
                 "samples": len(s)}
 
 
-def algorithmic_bytes_per_cell_update(kernel, tile, T, has_coef, fbytes=4):
+def algorithmic_bytes_per_cell_update(kernel, tile, T, has_coef, fbytes=4, cbytes=24):
     """SURVEY.md 8(d) / DESIGN.md 6.5: global-memory bytes the schedule must move per 6-component cell update.
     T is the depth of the launch that was actually timed (min(library depth, steps per call)); fbytes = bytes per stored
-    field value (4, or 2 with binary16 field storage); coefficients are always 4 bytes."""
+    field value (4, or 2 with binary16 field storage); cbytes = coefficient bytes per cell (24: six float arrays; 3: three
+    material-index bytes)."""
     if kernel == "naive":
-        return 18.0 * fbytes + (24.0 if has_coef else 0.0)
+        return 18.0 * fbytes + (float(cbytes) if has_coef else 0.0)
     Nx, Ny, Nz = tile
     V = Nx * Ny * Nz
     B = (Nx + 1) * (Ny + 1) * (Nz + 1)
     X = B - V                                   # minus shell of the box
     D = V - (Nx - 1) * (Ny - 1) * (Nz - 1)      # plus shell of the tile
-    nc = 6 if has_coef else 0
     f_loads = 3 * B + 3 * V + (T - 1) * 6 * X              # step 0: box of H, E on the tile; then the minus shells
-    c_loads = nc * B + (T - 1) * nc * X                    # coefficients of the box, then of the entering shells
+    c_cells = (B + (T - 1) * X) if has_coef else 0         # coefficients of the box, then of the entering shells
     stores = (T - 1) * 6 * D + 6 * V                       # plus shells; the whole tile at the last step
-    return (fbytes * (f_loads + stores) + 4.0 * c_loads) / (V * T)
+    return (fbytes * (f_loads + stores) + float(cbytes) * c_cells) / (V * T)
 
 
 def max_over_ranks(dist, value, device):
@@ -209,18 +211,22 @@ def run_reference(args):
 
 
 # ---- one timed case on the device --------------------------------------------------------------------------------
-def setup_case(w, kernel, variant, dev, tile=None, T=0, storage="f32"):
+def setup_case(w, kernel, variant, dev, tile=None, T=0, storage="f32", coeffs="arrays"):
     """Seeded inputs of workload w on the device, a context bound to them."""
     import torch
     from paper_2502_20610_b200 import binding, workloads
     E, H = workloads.make_fields(w, device=dev)
     if storage == "f16":
         E, H = [a.to(torch.float16) for a in E], [a.to(torch.float16) for a in H]
-    ca, cb = workloads.make_coeffs(w, device=dev)
     sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant=variant)
     sim.set_fields(E, H)
-    if ca is not None:
-        sim.set_coeffs(ca, cb, None)
+    if coeffs == "lut":
+        ca, cb, _ = workloads.make_coeff_lut(w, device=dev)       # (index arrays, ca table, cb table)
+        sim.set_coeff_lut(ca, cb, _)
+    else:
+        ca, cb = workloads.make_coeffs(w, device=dev)
+        if ca is not None:
+            sim.set_coeffs(ca, cb, None)
     src = workloads.make_source(w)
     if src is not None:
         sim.set_source(src.comp, src.box, src.amp, src.wave)
@@ -236,10 +242,10 @@ def load_counters():
         return {}
 
 
-def roofline_of(kernel, w, info, has_coef, S, tcups, peak_gbs, counters, storage="f32"):
+def roofline_of(kernel, w, info, has_coef, S, tcups, peak_gbs, counters, storage="f32", coeffs="arrays"):
     """HBM roofline of one case: algorithmic bytes per cell update of the launch that was timed x achieved rate / peak."""
     T = min(info["T"], S) if kernel == "systolic" else 0
-    bpc = algorithmic_bytes_per_cell_update(kernel, info["tile"], max(T, 1), has_coef, 2 if storage == "f16" else 4)
+    bpc = algorithmic_bytes_per_cell_update(kernel, info["tile"], max(T, 1), has_coef, 2 if storage == "f16" else 4, 3 if coeffs == "lut" else 24)
     achieved = bpc * tcups * 1e12 / 1e9
     out = {"bytes_per_cell_update": bpc, "T_launched": T, "achieved_gbs": achieved, "frac": achieved / peak_gbs,
            "roof_tcups": peak_gbs * 1e9 / bpc / 1e12}
@@ -277,7 +283,9 @@ def time_case(sim, S, K, W, barrier=None):
 SWEEP = [("C1", 0, None, "f32"), ("C4-64", 3, 64, "f32"), ("C4-128", 3, 128, "f32"), ("C4-256", 3, 256, "f32"), ("C2", 1, None, "f32"),
          ("C4-512", 3, 512, "f32"), ("C3", 2, None, "f32"), ("C4-768", 3, 768, "f32"), ("C4-1024", 3, 1024, "f32"), ("C5", 4, None, "f32"),
          # row f1: binary16 field storage, f32 arithmetic (the paper's own configuration)
-         ("C2", 1, None, "f16"), ("C4-1024", 3, 1024, "f16"), ("C5", 4, None, "f16")]
+         ("C2", 1, None, "f16"), ("C4-1024", 3, 1024, "f16"), ("C5", 4, None, "f16"),
+         # row f2: material-index coefficients (three bytes per cell instead of six floats)
+         ("C2", 1, None, "lut"), ("C3", 2, None, "lut")]
 
 
 def run_sweep(variant, dev, peak_gbs, counters, headline, skip_name):
@@ -286,6 +294,8 @@ def run_sweep(variant, dev, peak_gbs, counters, headline, skip_name):
     from paper_2502_20610_b200 import workloads
     rows = []
     for name, idx, size, storage in SWEEP:
+        coeffs = "lut" if storage == "lut" else "arrays"
+        storage = "f32" if storage == "lut" else storage
         w0 = workloads.config(idx, size)
         if w0.name == skip_name and storage == "f32":            # the headline workload was just timed: reuse its numbers
             rows.append(headline)
@@ -293,17 +303,18 @@ def run_sweep(variant, dev, peak_gbs, counters, headline, skip_name):
         # S time steps per call, K calls: the config's own step count where that is a few launches, never less than 2 calls
         S = min(w0.steps, 100 if w0.cells > (1 << 24) else 200)
         fb = 2 if storage == "f16" else 4
-        row = {"workload": w0.name, "grid": list(w0.n), "field_storage": storage,
-               "working_set_mb": (6 * fb + (24 if w0.has_coeff_arrays else 0)) * w0.cells / 1e6, "time_steps_per_call": S}
+        cbytes = 3 if coeffs == "lut" else 24
+        row = {"workload": w0.name, "grid": list(w0.n), "field_storage": storage, "coefficients": coeffs if w0.has_coeff_arrays else "uniform",
+               "working_set_mb": (6 * fb + (cbytes if w0.has_coeff_arrays else 0)) * w0.cells / 1e6, "time_steps_per_call": S}
         for kernel in ("naive", "systolic"):
             K, W = (2, 1) if w0.cells > (1 << 27) else (3, 2)
             Sk = S if kernel == "systolic" else max(10, min(S, int(2e10 / w0.cells)))       # the naive rate does not depend on S
             w = replace(w0, steps=max(w0.steps, (K + W) * Sk + 1))
-            sim, keep = setup_case(w, kernel, variant, dev, storage=storage)
+            sim, keep = setup_case(w, kernel, variant, dev, storage=storage, coeffs=coeffs)
             info = sim.get_kernel()
             ms, launches = time_case(sim, Sk, K, W)
             tc = w.cells * Sk * K / (ms * 1e-3) / 1e12
-            r = roofline_of(kernel, w, info, w.has_coeff_arrays, Sk, tc, peak_gbs, counters, storage)
+            r = roofline_of(kernel, w, info, w.has_coeff_arrays, Sk, tc, peak_gbs, counters, storage, coeffs)
             row[kernel + "_tcups"] = tc
             row[kernel + "_frac"] = r["frac"]
             row[kernel + "_bytes_per_cell_update"] = r["bytes_per_cell_update"]
@@ -349,7 +360,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     tile = tuple(int(x) for x in args.tile.split("x")) if args.tile else None
-    sim, keep = setup_case(w, args.kernel, args.variant, dev, tile, args.T, args.storage)
+    sim, keep = setup_case(w, args.kernel, args.variant, dev, tile, args.T, args.storage, args.coeffs)
     info = sim.get_kernel()
     has_coef = keep[2] is not None
 
@@ -420,7 +431,7 @@ def main():
         pass
     peak = float(peaks.get("hbm_gbs", 6650.0))
     counters = load_counters()
-    r = roofline_of(args.kernel, w, info, has_coef, S, value / world, peak, counters, args.storage)
+    r = roofline_of(args.kernel, w, info, has_coef, S, value / world, peak, counters, args.storage, args.coeffs)
     tma = info["smem"] in (229632, 147456)
     roofline = {"bound": "hbm", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"], "traffic": None,
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy)" if "hbm_gbs" in peaks else "fallback 6.65 TB/s",
@@ -442,7 +453,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": "TCUPS", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "field_storage": args.storage, "grid": list(w.n), "time_steps_per_bench_step": S, "kernel": args.kernel,
+            "config": {"workload": w.name, "field_storage": args.storage, "coefficients": (args.coeffs if has_coef else "uniform"), "grid": list(w.n), "time_steps_per_bench_step": S, "kernel": args.kernel,
                        "tile": list(info["tile"]), "T": info["T"], "tiles_per_launch": info["tiles"], "ctas": info["ctas"],
                        "smem_per_cta": info["smem"], "variant": args.variant, "parallelism": "replicas" if world > 1 else "single",
                        "l2": "inputs exceed L2 (%.0f MB of fields+coefficients vs 126 MB)" % (ws / 1e6) if ws > 200e6
@@ -457,7 +468,7 @@ def main():
                     args.kernel + "_tcups": value / world, args.kernel + "_frac": r["frac"],
                     args.kernel + "_bytes_per_cell_update": r["bytes_per_cell_update"], "T": r["T_launched"],
                     "tiles_per_launch": info["tiles"]}
-    if world == 1 and not args.no_sweep and args.kernel == "systolic" and not args.tile and not args.T and args.storage == "f32":
+    if world == 1 and not args.no_sweep and args.kernel == "systolic" and not args.tile and not args.T and args.storage == "f32" and args.coeffs == "arrays":
         # the headline row still needs its naive leg
         other = replace(w, steps=max(w.steps, 64))
         Sn = max(10, min(S, int(2e10 / w.cells)))

@@ -79,7 +79,7 @@ int fdtd_set_fields(fdtd_ctx* ctx, float* const E[3], float* const H[3]);
 
 /* The same with the six field arrays stored as IEEE binary16 (row f1; section 4: the paper's engine "halves
  * the number of bytes needed to be loaded per field value, by utilizing 16-bit floating-point representations for the
- * field values"; reading #14).  E[3], H[3]: host arrays of DEVICE pointers to nx*ny*nz binary16 values each,
+ * field values"; reading #16).  E[3], H[3]: host arrays of DEVICE pointers to nx*ny*nz binary16 values each,
  * same layout, 16-byte aligned, borrowed and updated in place.  Arithmetic is unchanged (f32, the same expression tree;
  * coefficients, 1/d and source tables stay f32); every newly computed field value -- each half-step, and the source add --
  * is rounded to binary16, nearest-even, before it is stored or used again, so the result does not depend on the schedule
@@ -124,7 +124,7 @@ int fdtd_set_source(fdtd_ctx* ctx, int comp, int i0, int j0, int k0, int ni, int
                     const float* amp, const float* wave, int nwave);
 
 /* Running-DFT output monitor on one plane (outputs are excluded from the paper's benchmark but named as what real runs
- * carry; reading #13).  While the step counter t is in [0, nt), every step adds, for each cell of
+ * carry; reading #15).  While the step counter t is in [0, nt), every step adds, for each cell of
  * the plane `axis` = `index`, each frequency f < nfreq and each component a:
  *     after the E half-step and the source:  acc[a][f][0|1][cell]     += E_a * wE[t][f][0|1]
  *     after the H half-step:                 acc[3 + a][f][0|1][cell] += H_a * wH[t][f][0|1]
@@ -197,7 +197,7 @@ int fdtd_plan_owner(int n, int boundary, int N, int T, int g, int s, int* tile, 
 int fdtd_debug_level_errors(fdtd_ctx* ctx, long long out[5]);
 
 /* Adiabatic-absorber coefficient generator (section 4: "does not use PMLs, but instead relies on the
- * imaginary part of the permittivity to allow for the formation of adiabatic absorbers [5]"; reading #12).
+ * imaginary part of the permittivity to allow for the formation of adiabatic absorbers [5]"; reading #14).
  * Context-free; runs one kernel on `cuda_stream` of the current device and returns without synchronising.
  * Writes the six per-cell update-coefficient arrays that fdtd_set_coeffs takes, for a conductivity that rises as
  * sigma_max * u^order (u = 0 at the inner edge of a layer, 1 at the wall) over `thickness` cells in front of each face:

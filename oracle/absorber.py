@@ -5,7 +5,7 @@ path and shares no code with it.
 
 What the paper says (section 4): the engine "does not use PMLs, but instead relies on the imaginary part of
 the permittivity to allow for the formation of adiabatic absorbers [5]" -- Oskooi et al. 2008: a conductivity that rises
-smoothly (polynomially) from zero over a layer in front of the wall.  The paper gives no formula; reading #12
+smoothly (polynomially) from zero over a layer in front of the wall.  The paper gives no formula; reading #14
 fixes the one below.  Pins: tests/test_oracle_next_pins.py (uniform lossy medium against the analytic decay rate,
 round-trip reflection of a graded layer against exp(-2 sigma_max L d / ((p+1) n)), mirror symmetry of the half-cell
 staggering, sum rule at corners).

@@ -4,7 +4,7 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline leg may import 
 path and shares no code with it.
 
 The paper excludes outputs from its benchmark but names them as what real runs carry ("the output volume and format",
-PAPER.md:106).  DESIGN.md reading #13 fixes the definition: a monitor is a plane (axis q, index m) of the grid, a list of
+PAPER.md:106).  DESIGN.md reading #15 fixes the definition: a monitor is a plane (axis q, index m) of the grid, a list of
 F frequencies and two caller-supplied tables of complex weights, one per time step and frequency; during step t (t = the
 context's step counter, 0-based)
 

@@ -85,7 +85,7 @@ YEE_GRID_STRUCT(double, yee_grid_f64);
 
 /* f16 field storage with f32 arithmetic (section 4: "halves the number of bytes needed
  * to be loaded per field value, by utilizing 16-bit floating-point representations for the field values").
- * reading #14: the six field arrays hold IEEE binary16 values; every update reads them (exact conversion to f32),
+ * reading #16: the six field arrays hold IEEE binary16 values; every update reads them (exact conversion to f32),
  * evaluates the same f32 expression tree, and rounds the new value to binary16 (nearest-even) when it is stored -- at every
  * half-step, so that the result does not depend on how long a value stays on chip.  The source add rounds likewise.
  * Coefficients, 1/d and the source tables stay f32.  The arrays of this build are float arrays whose values are

@@ -2,7 +2,7 @@
 //
 // PAPER.md:103 (section 4): the engine "does not use PMLs, but instead relies on the imaginary part of the permittivity
 // to allow for the formation of adiabatic absorbers [5]": a conductivity that rises polynomially from zero over a layer
-// in front of a wall (Oskooi et al. 2008).  DESIGN.md reading #12 fixes the formula; this kernel writes the six
+// in front of a wall (Oskooi et al. 2008).  DESIGN.md reading #14 fixes the formula; this kernel writes the six
 // per-cell update-coefficient arrays of fdtd_set_coeffs straight into device memory (config 5's are 43 GB: they are
 // generated where they are used).  One thread per cell, one statement per rounded operation: with -fmad=false the
 // arrays are bit-identical to the fp32 CPU oracle's.

@@ -95,7 +95,7 @@ struct PadArrays {
 };
 
 // Running-DFT monitor on one plane of the grid (PAPER.md:106 names outputs as what real runs carry;
-// DESIGN.md reading #13).  During step t (0 <= t < nt), for every cell of the plane and every frequency f:
+// DESIGN.md reading #15).  During step t (0 <= t < nt), for every cell of the plane and every frequency f:
 //     after the E half-step and the source:  acc[a][f][re|im][cell]     += E_a * wE[t][f][re|im]     a = 0..2
 //     after the H half-step:                 acc[3 + a][f][re|im][cell] += H_a * wH[t][f][re|im]
 // (product rounded, then the add).  Plane cells are numbered x fastest over the two remaining axes of the CALLER's grid.

@@ -91,7 +91,7 @@ constexpr int W_HPROD = NWARPS_C, W_HAUX = NWARPS_C + 1, W_EPROD = NWARPS_C + 2;
 // then be fetched by ONE 4-D box per piece and lands exactly where per-array 3-D boxes would put it.
 // Field storage (row f1): FDTD_FLD16 builds keep the six field arrays in IEEE binary16 (systolic_tma_h16.cu);
 // arithmetic and the on-chip copies stay f32, every newly computed value is rounded to binary16 before it is used again
-// (reading #14), so the result does not depend on the schedule.  A binary16 box needs 8 elements per 16 bytes:
+// (reading #16), so the result does not depend on the schedule.  A binary16 box needs 8 elements per 16 bytes:
 // field boxes start at o0 & ~7, are 40 cells wide, and the x column box is 8 cells wide.
 #ifdef FDTD_FLD16
 using fld_t = __half;
@@ -567,7 +567,7 @@ __shared__ unsigned trace_cur_;
 #define TRACE_C(ev, k)
 #endif
 
-// Running-DFT monitor (row f4, reading #13): the cells of the plane that this thread has just updated in step
+// Running-DFT monitor (row f4, reading #15): the cells of the plane that this thread has just updated in step
 // t0 + k are accumulated into the caller's device array.  Every (cell, step) pair is updated by exactly one thread of one
 // tile; successive steps of a cell are ordered by program order inside a tile and by the flag hand-off between tiles (the
 // read-modify-write below is issued before the warp arrives on the DONE barrier that the signal warp's fence covers, and

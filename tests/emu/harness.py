@@ -13,6 +13,7 @@ _FP = C.POINTER(C.c_float)
 
 class GridParams(C.Structure):   # mirrors csrc/fdtd_types.h
     _fields_ = [("E", _FP * 3), ("H", _FP * 3), ("ca", _FP * 3), ("cb", _FP * 3),
+                ("cidx", C.c_void_p * 3), ("lut", _FP), ("nmat", C.c_int), ("fld16", C.c_int),
                 ("n", C.c_int * 3), ("per", C.c_int * 3), ("rd", C.c_float * 3), ("cb_scalar", C.c_float),
                 ("db", C.c_float * 3), ("src_comp", C.c_int), ("src_box", C.c_int * 6),
                 ("src_amp", _FP), ("src_wave", _FP), ("src_nwave", C.c_int)]
@@ -26,6 +27,7 @@ def build():
         os.replace(LIB + ".tmp", LIB)
     lib = C.CDLL(LIB)
     lib.systolic_emu_run.restype = C.c_int
+    assert lib.systolic_emu_sizeof_grid() == C.sizeof(GridParams), "harness.GridParams is out of step with csrc/fdtd_types.h"
     return lib
 
 

@@ -147,3 +147,6 @@ int systolic_emu_run(const GridParams* g, const int box[3], int T, int nsteps, l
 }
 
 }  // extern "C"
+
+// layout check for the ctypes mirror in harness.py
+extern "C" int systolic_emu_sizeof_grid() { return (int)sizeof(GridParams); }

@@ -464,7 +464,8 @@ def main():
     if cpu is not None:
         line["cpu_baseline"] = cpu
     sim.close()
-    headline_row = {"workload": w.name, "grid": list(w.n), "field_storage": args.storage, "working_set_mb": ws / 1e6, "time_steps_per_call": S,
+    headline_row = {"workload": w.name, "grid": list(w.n), "field_storage": args.storage,
+                    "coefficients": (args.coeffs if has_coef else "uniform"), "working_set_mb": ws / 1e6, "time_steps_per_call": S,
                     args.kernel + "_tcups": value / world, args.kernel + "_frac": r["frac"],
                     args.kernel + "_bytes_per_cell_update": r["bytes_per_cell_update"], "T": r["T_launched"],
                     "tiles_per_launch": info["tiles"]}

@@ -396,3 +396,97 @@ def test_lut_per_component_tables_and_rebinding(cuda_device):
         sim.sync()
         sim.close()
         compare(([x.cpu().numpy() for x in Ed], [x.cpu().numpy() for x in Hd]), (E, H), exact=True)
+
+
+# ---- combinations of the 8(f) rows ------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,T", [("naive", 0), ("systolic", 16)])
+def test_monitor_with_f16_storage(cuda_device, kernel, T):
+    """Running DFT of binary16-stored fields: the monitor sees the rounded values, as the oracle's f16-storage build does."""
+    import torch
+    from oracle.monitor import MonitorOracle
+    w, steps = CASES["C2s"]
+    wE, wH = _weights(steps, 2, 3)
+    r16 = lambda a: a.astype(np.float16).astype(np.float32)
+    E, H = workloads.make_fields(w)
+    E, H = [r16(a) for a in E], [r16(a) for a in H]
+    ca, cb = workloads.make_coeffs(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None, storage="f16")
+    src = workloads.make_source(w)
+    orc.set_source(src.comp, src.box, src.amp, src.wave)
+    mon = MonitorOracle(orc, 1, 30, wE, wH)
+    mon.step(steps)
+    want = mon.acc.reshape(6, 2, 2, -1)
+    dev = torch.device("cuda:0")
+    Ed, Hd = workloads.make_fields(w, device=dev)
+    Ed, Hd = [a.to(torch.float16) for a in Ed], [a.to(torch.float16) for a in Hd]
+    cad, cbd = workloads.make_coeffs(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+    sim.set_fields(Ed, Hd)
+    sim.set_coeffs(cad, cbd, None)
+    sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_NAIVE if kernel == "naive" else binding.KERNEL_SYSTOLIC, (31, 15, 7) if kernel == "systolic" else None, T)
+    acc = torch.zeros((6, 2, 2, want.shape[3]), dtype=torch.float32, device=dev)
+    sim.set_monitor(1, 30, wE, wH, acc)
+    sim.step(steps)
+    sim.sync()
+    sim.close()
+    assert float(np.abs(want).max()) > 0
+    assert np.array_equal(acc.cpu().numpy(), want)
+    compare(([x.float().cpu().numpy() for x in Ed], [x.float().cpu().numpy() for x in Hd]), (E, H), exact=True)
+
+
+def test_monitor_with_lut_and_lut_with_f16(cuda_device, oracle_cache):
+    """Monitor on a material-index run (systolic); material indices with binary16 fields: naive runs it, the systolic
+    schedule says FDTD_EINVAL."""
+    import torch
+    from oracle.monitor import MonitorOracle
+    w, steps = CASES["C3s"]
+    wE, wH = _weights(steps, 1, 5)
+    E, H = workloads.make_fields(w)
+    ca, cb = workloads.make_coeffs(w)
+    orc = YeeOracle(w.n, w.d, w.dt, w.boundary, E, H, ca, cb, None)
+    src = workloads.make_source(w)
+    orc.set_source(src.comp, src.box, src.amp, src.wave)
+    mon = MonitorOracle(orc, 2, 19, wE, wH)
+    mon.step(steps)
+    want = mon.acc.reshape(6, 1, 2, -1)
+    dev = torch.device("cuda:0")
+    Ed, Hd = workloads.make_fields(w, device=dev)
+    idx, ca_lut, cb_lut = workloads.make_coeff_lut(w, device=dev)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+    sim.set_fields(Ed, Hd)
+    sim.set_coeff_lut(idx, ca_lut, cb_lut)
+    sim.set_source(src.comp, src.box, src.amp, src.wave)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC, (31, 15, 7), 8)
+    acc = torch.zeros((6, 1, 2, want.shape[3]), dtype=torch.float32, device=dev)
+    sim.set_monitor(2, 19, wE, wH, acc)
+    sim.step(steps)
+    sim.sync()
+    sim.close()
+    assert np.array_equal(acc.cpu().numpy(), want)
+    compare(([x.cpu().numpy() for x in Ed], [x.cpu().numpy() for x in Hd]), (E, H), exact=True)
+    # binary16 fields + material indices
+    r16 = lambda a: a.astype(np.float16).astype(np.float32)
+    E2, H2 = workloads.make_fields(w)
+    E2, H2 = [r16(a) for a in E2], [r16(a) for a in H2]
+    orc2 = YeeOracle(w.n, w.d, w.dt, w.boundary, E2, H2, ca, cb, None, storage="f16")
+    orc2.set_source(src.comp, src.box, src.amp, src.wave)
+    orc2.step(steps)
+    for kernel in (binding.KERNEL_NAIVE, binding.KERNEL_SYSTOLIC):
+        Ed, Hd = workloads.make_fields(w, device=dev)
+        Ed, Hd = [a.to(torch.float16) for a in Ed], [a.to(torch.float16) for a in Hd]
+        sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary)
+        sim.set_fields(Ed, Hd)
+        sim.set_coeff_lut(idx, ca_lut, cb_lut)
+        sim.set_source(src.comp, src.box, src.amp, src.wave)
+        if kernel == binding.KERNEL_NAIVE:
+            sim.set_kernel(kernel, None, 0)
+            sim.step(steps)
+            sim.sync()
+            compare(([x.float().cpu().numpy() for x in Ed], [x.float().cpu().numpy() for x in Hd]), (E2, H2), exact=True)
+        else:
+            with pytest.raises(binding.FdtdError) as e:      # rejected when the schedule is chosen, or at the latest by fdtd_step
+                sim.set_kernel(kernel, (31, 15, 7), 8)
+                sim.step(steps)
+            assert e.value.code == binding.EINVAL
+        sim.close()

@@ -1202,6 +1202,7 @@ void fdtd_destroy(fdtd_ctx* c)
             for (int i = 0; i < 32; ++i) fprintf(stderr, "%s%lld", i % 8 == 0 ? "\n  " : " ", h[i]);
             fprintf(stderr, "\n");
         }
+#ifdef FDTD_PROFILE
         // event trace of one CTA (systolic_tma.cu TRACE): clock << 20 | role << 16 | event << 12 | step
         if (const char* path = getenv("FDTD_TRACE_FILE")) {
             std::vector<long long> tr(FDTD_TRACE_CAP);
@@ -1215,6 +1216,7 @@ void fdtd_destroy(fdtd_ctx* c)
                 }
             }
         }
+#endif
         cudaFree(c->d_prof);
     }
     if (c->ev0) cudaEventDestroy(c->ev0);

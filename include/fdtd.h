@@ -44,6 +44,11 @@
  * returns FDTD_ECUDA.
  *
  * Thread safety: one ctx per host thread at a time.
+ *
+ * Environment (read ONCE, in fdtd_create; tuning only, none of them changes a result): FDTD_T = default temporal depth,
+ * FDTD_TILE = "NXxNYxNZ" default tile, FDTD_SPIN_BUDGET_MS = hand-off watchdog budget (default 10 s), FDTD_NO_OVERLAP =
+ * consecutive systolic launches wait for each other instead of overlapping.  Debug switches exist only in the developer
+ * builds (libfdtd_b200_dbg.so / _prof.so).
  */
 #ifndef FDTD_B200_H
 #define FDTD_B200_H

@@ -211,27 +211,39 @@ def run_reference(args):
 
 
 # ---- one timed case on the device --------------------------------------------------------------------------------
-def setup_case(w, kernel, variant, dev, tile=None, T=0, storage="f32", coeffs="arrays"):
-    """Seeded inputs of workload w on the device, a context bound to them."""
-    import torch
+def bind_context(w, kernel, variant, E, H, coef, tile=None, T=0, stream=None):
+    """A context on `stream` bound to the field arrays E, H and to the coefficient objects `coef` (shared, read-only)."""
     from paper_2502_20610_b200 import binding, workloads
-    E, H = workloads.make_fields(w, device=dev)
-    if storage == "f16":
-        E, H = [a.to(torch.float16) for a in E], [a.to(torch.float16) for a in H]
-    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant=variant)
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, stream=stream, variant=variant)
     sim.set_fields(E, H)
-    if coeffs == "lut":
-        ca, cb, _ = workloads.make_coeff_lut(w, device=dev)       # (index arrays, ca table, cb table)
-        sim.set_coeff_lut(ca, cb, _)
-    else:
-        ca, cb = workloads.make_coeffs(w, device=dev)
-        if ca is not None:
-            sim.set_coeffs(ca, cb, None)
+    if coef is not None and coef[0] == "lut":
+        sim.set_coeff_lut(coef[1], coef[2], coef[3])
+    elif coef is not None:
+        sim.set_coeffs(coef[1], coef[2], None)
     src = workloads.make_source(w)
     if src is not None:
         sim.set_source(src.comp, src.box, src.amp, src.wave)
     sim.set_kernel(binding.KERNEL_SYSTOLIC if kernel == "systolic" else binding.KERNEL_NAIVE, tile, T)
-    return sim, (E, H, ca, cb)
+    return sim
+
+
+def setup_case(w, kernel, variant, dev, tile=None, T=0, storage="f32", coeffs="arrays"):
+    """Seeded inputs of workload w on the device, a context bound to them.  Returns (sim, (E, H, coef)) with coef = None |
+    ("arrays", ca, cb) | ("lut", index arrays, ca table, cb table)."""
+    import torch
+    from paper_2502_20610_b200 import workloads
+    E, H = workloads.make_fields(w, device=dev)
+    if storage == "f16":
+        E, H = [a.to(torch.float16) for a in E], [a.to(torch.float16) for a in H]
+    coef = None
+    if coeffs == "lut":
+        coef = ("lut",) + tuple(workloads.make_coeff_lut(w, device=dev))
+    else:
+        ca, cb = workloads.make_coeffs(w, device=dev)
+        if ca is not None:
+            coef = ("arrays", ca, cb)
+    sim = bind_context(w, kernel, variant, E, H, coef, tile, T)
+    return sim, (E, H, coef)
 
 
 def load_counters():
@@ -329,6 +341,75 @@ def run_sweep(variant, dev, peak_gbs, counters, headline, skip_name):
     return rows
 
 
+def e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier):
+    """The same metric end to end through the C ABI with HOST buffers (copies inside the timed region).  A function of its
+    own so that its device and pinned buffers die with it."""
+    import torch
+    from paper_2502_20610_b200 import workloads
+    shape = (w.n[2], w.n[1], w.n[0])
+    fdtype = torch.float16 if args.storage == "f16" else torch.float32
+    nbytes = 6 * w.cells * (2 if args.storage == "f16" else 4)
+    ke = 2 if nbytes > (8 << 30) else max(2, min(K, 5))
+    if w.fields == "zero":
+        Ein = [torch.zeros(shape, dtype=fdtype).pin_memory() for _ in range(3)]
+        Hin = [torch.zeros(shape, dtype=fdtype).pin_memory() for _ in range(3)]
+    else:
+        Eh, Hh = workloads.make_fields(w)
+        Ein, Hin = [torch.from_numpy(a).to(fdtype).pin_memory() for a in Eh], [torch.from_numpy(a).to(fdtype).pin_memory() for a in Hh]
+        del Eh, Hh
+    Eout = [torch.empty(shape, dtype=fdtype).pin_memory() for _ in range(3)]
+    Hout = [torch.empty(shape, dtype=fdtype).pin_memory() for _ in range(3)]
+
+    # Two independent jobs in flight, each with its own device copy of the six field arrays, its own context and stream (the
+    # coefficient arrays are shared, read-only): while one job computes, the other's results go device -> host and its next
+    # inputs host -> device.  Every job still does the whole path: pinned host -> device, S time steps, device -> pinned host.
+    jobs = []
+    try:
+        for j in range(2):
+            st = torch.cuda.Stream(device=dev)
+            Ej, Hj = (keep[0], keep[1]) if j == 0 else ([torch.empty_like(a) for a in keep[0]], [torch.empty_like(a) for a in keep[1]])
+            jobs.append((bind_context(w, args.kernel, args.variant, Ej, Hj, keep[2], tile, args.T, stream=st.cuda_stream), st, Ej, Hj))
+    except torch.cuda.OutOfMemoryError:
+        pass                                  # one job in flight if a second copy of the fields does not fit
+    sim.sync()
+
+    def submit(job):
+        job[0].set_time(0)
+        job[0].load_fields(Ein, Hin)
+        job[0].step(S)
+
+    def collect(job):
+        job[0].get_fields(Eout, Hout)        # waits for the job's steps, then enqueues the copies out
+
+    def run(n):
+        nj = len(jobs)
+        for i in range(min(nj, n)):
+            submit(jobs[i])                              # fill the pipeline
+        for i in range(n):
+            collect(jobs[i % nj])                        # job i's steps are done: its results start to leave
+            if i + nj < n:
+                submit(jobs[i % nj])                     # its next inputs follow on the same stream
+        for job in jobs:
+            job[0].sync()
+    ke = 2 * ke if len(jobs) > 1 else ke
+    run(2)
+    barrier()
+    t0 = time.perf_counter()
+    run(ke)
+    barrier()
+    dt = max_over_ranks(dist, time.perf_counter() - t0, dev)
+    e2e = {"value": job_tcups(world, w.cells * S * ke, dt), "unit": "TCUPS", "h2d_bytes_per_step": nbytes,
+           "d2h_bytes_per_step": nbytes, "steps": ke, "jobs_in_flight": len(jobs),
+           "note": "per bench step: six field arrays pinned host->device, S time steps, six arrays device->pinned host, all "
+                   "through the C ABI; two independent jobs in flight on two streams (copies of one overlap the steps of the "
+                   "other); the coefficient arrays are problem constants bound once"}
+    for job in jobs:
+        job[0].close()
+    del jobs
+    del Ein, Hin, Eout, Hout
+    return e2e
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -385,37 +466,8 @@ def main():
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     e2e = None
     if not args.no_e2e:
-        shape = (w.n[2], w.n[1], w.n[0])
-        fdtype = torch.float16 if args.storage == "f16" else torch.float32
-        nbytes = 6 * w.cells * (2 if args.storage == "f16" else 4)
-        ke = 2 if nbytes > (8 << 30) else max(2, min(K, 5))
-        if w.fields == "zero":
-            Ein = [torch.zeros(shape, dtype=fdtype).pin_memory() for _ in range(3)]
-            Hin = [torch.zeros(shape, dtype=fdtype).pin_memory() for _ in range(3)]
-        else:
-            Eh, Hh = workloads.make_fields(w)
-            Ein, Hin = [torch.from_numpy(a).to(fdtype).pin_memory() for a in Eh], [torch.from_numpy(a).to(fdtype).pin_memory() for a in Hh]
-            del Eh, Hh
-        Eout = [torch.empty(shape, dtype=fdtype).pin_memory() for _ in range(3)]
-        Hout = [torch.empty(shape, dtype=fdtype).pin_memory() for _ in range(3)]
-
-        def one():
-            sim.set_time(0)
-            sim.load_fields(Ein, Hin)
-            sim.step(S)
-            sim.get_fields(Eout, Hout)
-        one()
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(ke):
-            one()
-        barrier()
-        dt = max_over_ranks(dist, time.perf_counter() - t0, dev)
-        e2e = {"value": job_tcups(world, w.cells * S * ke, dt), "unit": "TCUPS", "h2d_bytes_per_step": nbytes,
-               "d2h_bytes_per_step": nbytes, "steps": ke,
-               "note": "six field arrays pinned host->device, S time steps, six arrays device->host, per bench step; "
-                       "the six coefficient arrays are problem constants bound once"}
-        del Ein, Hin, Eout, Hout
+        e2e = e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier)
+        torch.cuda.empty_cache()
 
     if rank != 0:
         sim.close()

@@ -17,4 +17,9 @@ def cuda_device():
     import torch
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
+    # the in-tree libraries travel with the repository snapshot; (re)build whatever is missing or stale on this box
+    from paper_2502_20610_b200 import build
+    build.build()
+    from oracle import build_oracle
+    build_oracle.build()
     return torch.device("cuda:0")

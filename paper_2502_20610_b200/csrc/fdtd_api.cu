@@ -886,7 +886,8 @@ int fdtd_set_coeff_lut(fdtd_ctx* c, const unsigned char* const idx[3], int nmat,
     if (e != cudaSuccess) return cuda_fail(c, e, "cudaStreamSynchronize");
     if (c->d_lut) cudaFree(c->d_lut);
     c->d_lut = nullptr;
-    std::vector<float> h((size_t)3 * nmat * 2);
+    // 256 pairs of zero padding behind the table: an index >= nmat (a caller error) reads (0, 0), never past the allocation
+    std::vector<float> h((size_t)3 * nmat * 2 + 512, 0.0f);
     for (int a = 0; a < 3; ++a)
         for (int m = 0; m < nmat; ++m) {
             h[((size_t)a * nmat + m) * 2] = ca_lut[a * nmat + m];

@@ -217,6 +217,43 @@ int fdtd_debug_level_errors(fdtd_ctx* ctx, long long out[5]);
 int fdtd_absorber_coeffs(int nx, int ny, int nz, float dt, const float* const eps[3], const int thickness[6],
                          const float sigma_max[6], int order, float* const ca[3], float* const cb[3], void* cuda_stream);
 
+/* The systolic kernel for callers that must not allocate device memory.
+ *
+ * Who this is for: fdtd_create / fdtd_step cudaMalloc the bookkeeping of the systolic schedule (two hand-off flags per
+ * tile, tile-claim counters, the claim order, a watchdog word).  A host application that has given all of HBM to its own
+ * memory pool has nothing left for that (and config 5 alone is 81 GiB of fields); a stepping loop that shares the GPU
+ * with other streams cannot afford the device-wide stall a cudaMalloc or cudaFree may bring.  This one call serves them:
+ * it advances the fields by nsteps steps with the same kernel as FDTD_KERNEL_SYSTOLIC (tile 31x15x7, f32), and calls no
+ * cudaMalloc, cudaFree or other allocating routine.  The bookkeeping lives in a fixed __device__ array inside the
+ * library, about 1.5 MiB, which every GPU that loads the library holds until the process exits.
+ *
+ * Scope: PEC walls on all three axes, nx a multiple of 4 (other grids need the padded working copy, i.e. an allocation),
+ * no source, no monitor, f32 fields.  Inputs and outputs stay the caller's: E[3], H[3] (updated in place), and either
+ * ca[3] and cb[3] or neither (NULL, NULL = ca 1, cb dt), all host arrays of 16-byte aligned DEVICE pointers to
+ * nx*ny*nz floats, x fastest; db: HOST array of three scalars or NULL (= dt).  T = temporal depth, 0 = 128.
+ * Limit: a launch of min(T, nsteps) steps may have at most FDTD_NOALLOC_MAX_TILES tiles,
+ *     ceil((nx+T)/31) * ceil((ny+T)/15) * ceil((nz+T)/7)      (fdtd_plan_tiles computes it on the host);
+ * e.g. 512^3 at T = 128 is 83 076 tiles and fits, 768^3 at T = 128 does not (pass T = 32).  A larger job returns
+ * FDTD_EINVAL and says so in errbuf; it is checked before anything touches the GPU.
+ *
+ * Behaviour to know about.
+ *   - The call works on the CURRENT device and on cuda_stream (NULL = legacy default stream), and returns only after
+ *     the GPU work has finished: it has to read the watchdog word.  FDTD_ETIMEOUT = a hand-off waited more than 10 s,
+ *     fields invalid.
+ *   - The first call on each device does a one-time set-up (it asks the runtime for the array's device address and sets
+ *     the kernel's shared-memory attribute).  Make that first call before any stream capture begins.
+ *   - All calls share the one array, and it still holds whatever the previous call wrote.  Each call therefore clears
+ *     the flags, counters and watchdog word on cuda_stream before its first launch.  Two runs in flight on one GPU
+ *     would raise and poll the same flags and corrupt each other, so the library holds a lock for the whole call:
+ *     a second host thread calling in waits until the first run is done.
+ *   - The step counter is not kept anywhere: state = the six arrays.
+ * errbuf (may be NULL): receives a NUL-terminated message of at most errbuf_len bytes on failure, "" on success.
+ * Results are bit-identical to fdtd_step on the same inputs (same kernel, same per-cell arithmetic). */
+enum { FDTD_NOALLOC_MAX_TILES = 131072 };
+int fdtd_step_noalloc(int nx, int ny, int nz, float dx, float dy, float dz, float dt, float* const E[3], float* const H[3],
+                      const float* const ca[3], const float* const cb[3], const float db[3], int nsteps, int T,
+                      void* cuda_stream, char* errbuf, int errbuf_len);
+
 const char* fdtd_last_error(const fdtd_ctx* ctx); /* text of the last failure on this ctx; never NULL */
 const char* fdtd_build_info(void);                /* e.g. "sm_100a fmad=true" */
 void fdtd_destroy(fdtd_ctx* ctx);                 /* NULL-safe; never frees borrowed buffers */

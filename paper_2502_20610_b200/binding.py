@@ -45,6 +45,8 @@ _PROTOS = {
     "fdtd_debug_level_errors": (C.c_int, [C.c_void_p, C.POINTER(C.c_longlong)]),
     "fdtd_absorber_coeffs": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_float, C.POINTER(C.c_void_p), C.POINTER(C.c_int), C.POINTER(C.c_float),
                                        C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_void_p]),
+    "fdtd_step_noalloc": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_float, C.c_float, C.c_float, C.c_float, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                    C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_float), C.c_int, C.c_int, C.c_void_p, C.c_char_p, C.c_int]),
     "fdtd_last_error": (C.c_char_p, [C.c_void_p]),
     "fdtd_build_info": (C.c_char_p, []),
     "fdtd_destroy": (None, [C.c_void_p]),
@@ -114,6 +116,25 @@ def absorber_coeffs(n, dt, eps, thickness, sigma_max, order, ca, cb, stream=None
                                             C.c_void_p(int(stream) or None))
     if rc != OK:
         raise FdtdError(rc, "fdtd_absorber_coeffs")
+
+
+NOALLOC_MAX_TILES = 131072
+
+
+def step_noalloc(n, d, dt, E, H, ca=None, cb=None, db=None, nsteps=1, T=0, stream=None, variant="nofma"):
+    """fdtd_step_noalloc: advance the six float32 CUDA tensors E[3], H[3] (shape (nz, ny, nx)) in place by `nsteps` steps
+    with the systolic kernel, without any device allocation inside the library (its flags, counters and claim order sit in
+    a fixed array inside the .so).  For hosts that own all device memory themselves or cannot stall on cudaMalloc.  PEC
+    walls, nx % 4 == 0, no source; blocks until the GPU work is done.  Raises FdtdError with the library's message."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+    err = C.create_string_buffer(512)
+    dbp = None if db is None else (C.c_float * 3)(*[float(x) for x in db])
+    rc = load(variant).fdtd_step_noalloc(int(n[0]), int(n[1]), int(n[2]), float(d[0]), float(d[1]), float(d[2]), float(dt), _ptr3(E), _ptr3(H),
+                                         _ptr3(ca), _ptr3(cb), dbp, int(nsteps), int(T), C.c_void_p(int(stream) or None), err, len(err))
+    if rc != OK:
+        raise FdtdError(rc, err.value.decode())
 
 
 class Fdtd:

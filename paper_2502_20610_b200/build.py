@@ -17,7 +17,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["absorber_kernels.cu", "fdtd_api.cu", "naive_kernels.cu", "pad_kernels.cu", "systolic_kernel.cu", "systolic_reg.cu", "systolic_tma.cu", "systolic_tma_by8.cu", "systolic_tma_h16.cu", "systolic_tma_lut.cu"]
+SOURCES = ["absorber_kernels.cu", "fdtd_api.cu", "fdtd_noalloc.cu", "naive_kernels.cu", "pad_kernels.cu", "systolic_kernel.cu", "systolic_reg.cu", "systolic_tma.cu", "systolic_tma_by8.cu", "systolic_tma_h16.cu", "systolic_tma_lut.cu"]
 HEADERS = ["fdtd_internal.h", "fdtd_types.h", "yee_update.h", "systolic_tile.cuh", os.path.join("..", "..", "include", "fdtd.h")]
 LIBS = {
     "nofma": (os.path.join(HERE, "libfdtd_b200.so"), ["-fmad=false", "-DFDTD_NOFMA"]),

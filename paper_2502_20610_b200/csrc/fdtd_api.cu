@@ -55,8 +55,11 @@ struct fdtd_ctx {
     // systolic state
     int* d_flags;     // flagE[cap] then flagH[cap]
     size_t flags_cap;
-    unsigned int* d_counter;   // ring of kCounterRing tile-claim counters: launch L uses slot L % ring; a TMA launch zeroes slot (L + ring/2) % ring
-    unsigned long long launch_seq;
+    // ring of kCounterRing tile-claim counters for the TMA kernel: its launch L uses slot L % ring and zeroes slot
+    // (L + ring/2) % ring; one more slot behind the ring serves every launch of the other systolic kernels (memset before
+    // each of them), which therefore never touch the ring
+    unsigned int* d_counter;
+    unsigned long long launch_seq;   // TMA launches so far
     // launch-to-launch overlap (row f2): shape and final flag value of the previous TMA launch, 0 = none / not reusable
     int prev_nb[3], prev_T, prev_final;
     bool no_overlap;           // FDTD_NO_OVERLAP in the environment at fdtd_create: every launch waits for the previous one
@@ -575,7 +578,7 @@ int step_systolic(fdtd_ctx* c, int n)
         P.ntiles = (int)ntiles;
         P.flagE = c->d_flags;
         P.flagH = c->d_flags + c->flags_cap;
-        P.counter = c->d_counter + (c->launch_seq % kCounterRing);
+        P.counter = c->use_tma ? c->d_counter + (c->launch_seq % kCounterRing) : c->d_counter + kCounterRing;
         P.counter_zero = c->use_tma ? c->d_counter + ((c->launch_seq + kCounterRing / 2) % kCounterRing) : nullptr;
         // overlap with the previous launch: same tile grid, same flag arrays still holding its final values, nothing but that
         // kernel before this one in the stream (a ghost refill or a copy in between serialises anyway: the wait is then free)
@@ -616,7 +619,7 @@ int step_systolic(fdtd_ctx* c, int n)
             P.lev_err = c->d_lev_err;
         }
         cudaError_t e = cudaSuccess;
-        if (!c->use_tma) {      // the other kernels do not maintain the ring
+        if (!c->use_tma) {      // the other kernels do not maintain the ring: their own slot, cleared before every launch
             e = cudaMemsetAsync(P.counter, 0, sizeof(unsigned int), c->stream);
             if (e != cudaSuccess) return cuda_fail(c, e, "cudaMemsetAsync(counter)");
         }
@@ -634,7 +637,7 @@ int step_systolic(fdtd_ctx* c, int n)
             c->prev_T = T;
             for (int a = 0; a < 3; ++a) c->prev_nb[a] = P.ax[a].nb;
         }
-        c->launch_seq++;
+        if (c->use_tma) c->launch_seq++;      // the ring position moves with TMA launches only (slot L is zeroed by TMA launch L - ring/2)
         c->flag_base += T + 2;
         c->t += T;
         left -= T;
@@ -775,8 +778,8 @@ int fdtd_create(fdtd_ctx** out, int nx, int ny, int nz, float dx, float dy, floa
     c->spin_budget = (long long)(budget_ms * (double)(prop.clockRate > 0 ? prop.clockRate : 1965000));
     c->ev_valid = false;
     memset(c->counters, 0, sizeof c->counters);
-    e = cudaMalloc(&c->d_counter, kCounterRing * sizeof(unsigned int));
-    if (e == cudaSuccess) e = cudaMemset(c->d_counter, 0, kCounterRing * sizeof(unsigned int));
+    e = cudaMalloc(&c->d_counter, (kCounterRing + 1) * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(c->d_counter, 0, (kCounterRing + 1) * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_abort, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(c->d_abort, 0, sizeof(int));
 #ifdef FDTD_PROFILE

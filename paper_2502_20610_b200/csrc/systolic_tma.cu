@@ -198,6 +198,15 @@ __device__ __forceinline__ void raise_flag(const SysParams& P, int* flags, int t
     FDTD_DEBUG_ONLY(if (tile == P.withhold_tile) return;)   // fault injection: the downwind tiles' watchdog must fire
     st_release(flags + tile, v);
 }
+// The same for the one raise that no tile of the launch itself waits for (the trailing jump to flag_base + T of a tile
+// that left the grid early): with launch overlap the tile of the same index of the NEXT launch may already have raised
+// this flag past that value, and a plain store arriving late would lower it (its downwind tiles would then spin until the
+// watchdog).  max keeps every flag monotone whatever the timing.
+__device__ __forceinline__ void raise_flag_max(const SysParams& P, int* flags, int tile, int v)
+{
+    FDTD_DEBUG_ONLY(if (tile == P.withhold_tile) return;)
+    asm volatile("red.release.gpu.global.max.s32 [%0], %1;" ::"l"(flags + tile), "r"(v) : "memory");
+}
 __device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ void st_relaxed(int* p, int v)
 {
@@ -1335,8 +1344,8 @@ __global__ void __launch_bounds__(NT, CTAS_PER_SM) systolic_tma_kernel(const __g
                 TRACE(4, 6, k);
             }
             if (k1 < T && lane == 0) {
-                raise_flag(P, P.flagE, tile, P.flag_base + T);
-                raise_flag(P, P.flagH, tile, P.flag_base + T);
+                raise_flag_max(P, P.flagE, tile, P.flag_base + T);
+                raise_flag_max(P, P.flagH, tile, P.flag_base + T);
             }
         }
     }

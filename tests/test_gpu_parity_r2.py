@@ -272,11 +272,15 @@ def test_full_size_config3_default_kernel(cuda_device):
 
 
 # ---- (e) windows at the default temporal depth, more steps than one launch ------------------------------------------
-def _window_check(w, steps, win, origins, need_free):
+def _window_check(w, steps, win, origins, need_free, nonzero=False):
+    import gc
     import torch
-    free, _ = torch.cuda.mem_get_info()
+    gc.collect()
+    torch.cuda.empty_cache()           # earlier tests leave tens of GB in torch's caching allocator
+    free, total = torch.cuda.mem_get_info()
     if free < need_free:
-        pytest.skip(f"needs {need_free / 1e9:.0f} GB of free device memory")
+        assert total < 170e9, f"only {free / 1e9:.0f} GB free of {total / 1e9:.0f} GB: something holds device memory"
+        pytest.skip(f"needs {need_free / 1e9:.0f} GB of free device memory (device has {total / 1e9:.0f} GB)")
     E, H, sim = binding.run_workload(w, steps=steps, variant="nofma")
     info = sim.get_kernel()
     assert info["which"] == binding.KERNEL_SYSTOLIC and steps > info["T"] >= 64       # default depth, at least two launches
@@ -299,8 +303,27 @@ def _window_check(w, steps, win, origins, need_free):
         sl_g = (slice(k0, k0 + win), slice(j0, j0 + win), slice(i0, i0 + win))
         for g, o in zip(E + H, Eo + Ho):
             got = g[sl_g].cpu().numpy()
+            if nonzero:
+                assert float(np.abs(o[sl_o]).max()) > 0.0, f"window at {(i0, j0, k0)} compares zero with zero"
             assert np.array_equal(got, o[sl_o]), f"window at {(i0, j0, k0)}: max diff {np.abs(got - o[sl_o]).max():.3e}"
     sim.close()
+    del E, H
+    gc.collect()
+    torch.cuda.empty_cache()
+
+
+def test_config5_random_fields_windows_default_depth(cuda_device):
+    """BASELINE configs[4] starts from zero fields, so after 160 steps only windows within 160 cells of the source hold
+    data.  The same recipe (lossy coefficients, anisotropic cells, point source, 81 GiB) with seeded random initial fields
+    puts data under every window: low corner, high corner, a high wall face, a point where tile seams of all three axes
+    meet -- frozen low walls, high-wall clipping and offsets beyond 2^32 bytes are checked on non-zero values, at the
+    library's default depth with more steps than one launch holds (the launch configuration bench.py times)."""
+    from dataclasses import replace
+    w = replace(workloads.config(4), fields="uniform", name="C5-lossy-random-fields")
+    nx, ny, nz = w.n
+    win = 24
+    origins = [(0, 0, 0), (nx - win, ny - win, nz - win), (nx - win, ny // 2 - 7, nz // 3), (31 * 20 - win // 2, 15 * 40 - win // 2, 7 * 50 - win // 2)]
+    _window_check(w, 160, win, origins, 100e9, nonzero=True)
 
 
 def test_config5_windows_default_depth(cuda_device):
@@ -426,4 +449,30 @@ def test_rejected_set_kernel_keeps_the_previous_choice(cuda_device):
     sim.sync()
     assert sim.get_kernel()["which"] == before["which"]
     sim.close()
+    _compare(E, H, Eo, Ho, exact=True)
+
+
+def test_switch_from_other_systolic_kernels_to_tma_on_one_context(cuda_device):
+    """The TMA kernel's tile-claim counters form a ring that its own launches maintain (launch L zeroes the slot of launch
+    L + 32).  Launches of the cross-check kernels on the same context must not consume or dirty ring slots: 70 of them,
+    then the TMA kernel, and the result is still the oracle's bit for bit (before the fix the first TMA launches found
+    counters >= ntiles and advanced nothing)."""
+    w = workloads.Workload("ring", (36, 20, 12), (1.0, 0.7, 1.2), (PEC,) * 3, 0, "uniform", "lossy", "none")
+    E0, H0 = workloads.make_fields(w)
+    ca, cb = workloads.make_coeffs(w)
+    E, H = _to_dev(E0), _to_dev(H0)
+    g = _to_dev(list(ca) + list(cb))
+    sim = binding.Fdtd(w.n, w.d, w.dt, w.boundary, variant="nofma")
+    sim.set_fields(E, H)
+    sim.set_coeffs(g[:3], g[3:], None)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC_REG, (31, 15, 7), 1)
+    sim.step(70)                                               # 70 launches of one step each
+    sim.set_kernel(binding.KERNEL_SYSTOLIC_SMEM, (31, 15, 7), 1)
+    sim.step(3)
+    sim.set_kernel(binding.KERNEL_SYSTOLIC, (31, 15, 7), 2)
+    sim.step(80)                                               # 40 TMA launches: past the 32 that used to start on stale slots
+    sim.sync()
+    assert sim.counters()["launches"] == 70 + 3 + 40
+    sim.close()
+    Eo, Ho = _run_oracle(w.n, w.d, w.dt, w.boundary, E0, H0, ca, cb, None, None, 153)
     _compare(E, H, Eo, Ho, exact=True)

@@ -195,6 +195,40 @@ def test_m1_running_dft_equals_fft_of_recorded_series(axis, index):
             assert np.allclose(mon.acc[c, f, 1], F[b, c].imag, atol=1e-12)
 
 
+def test_m1b_e_components_take_wE_and_h_components_take_wH():
+    """M1 again with DIFFERENT tables (wE on bins 1, 5, 9; wH on bins 2, 6, 11 and scaled by 3): the E accumulators must
+    be the fft bins of wE's frequencies and the H accumulators those of wH's, so a swap of the two tables inside the
+    oracle -- which passes every pin that feeds the same table twice -- fails here."""
+    n, d, dt = (8, 7, 6), (1, 1, 1), 0.4
+    nt = 32
+    binsE, binsH, scaleH = [1, 5, 9], [2, 6, 11], 3.0
+    tt = np.arange(nt)
+    wE, wH = np.zeros((nt, 3, 2)), np.zeros((nt, 3, 2))
+    for f in range(3):
+        wE[:, f, 0] = np.cos(2 * np.pi * binsE[f] * tt / nt)
+        wE[:, f, 1] = -np.sin(2 * np.pi * binsE[f] * tt / nt)
+        wH[:, f, 0] = scaleH * np.cos(2 * np.pi * binsH[f] * tt / nt)
+        wH[:, f, 1] = -scaleH * np.sin(2 * np.pi * binsH[f] * tt / nt)
+    E, H = _random_run(n, (PERIODIC,) * 3, 11)
+    E2, H2 = [a.copy() for a in E], [a.copy() for a in H]
+    mon = MonitorOracle(YeeOracle(n, d, dt, (PERIODIC,) * 3, E, H), 1, 2, wE, wH)
+    mon.step(nt)
+    y = YeeOracle(n, d, dt, (PERIODIC,) * 3, E2, H2)
+    sl = plane_slice(1, 2)
+    rec = []
+    for _ in range(nt):
+        y.step(1)
+        rec.append([a[sl].copy() for a in E2 + H2])
+    F = np.fft.fft(np.array(rec), axis=0)
+    for f in range(3):
+        for c in range(6):
+            want = F[binsE[f], c] if c < 3 else scaleH * F[binsH[f], c]
+            assert np.allclose(mon.acc[c, f, 0], want.real, atol=1e-11)
+            assert np.allclose(mon.acc[c, f, 1], want.imag, atol=1e-11)
+            other = scaleH * F[binsH[f], c] if c < 3 else F[binsE[f], c]          # what a swapped oracle would give
+            assert not np.allclose(mon.acc[c, f, 0], other.real, atol=1e-3)
+
+
 # ------------------------------------------------------------------------------------------------
 # M2  closed form: a single cavity mode E_z(t) = A cos(w t) -> sum_t cos(w (t+1) dt) e^{-i W (t+1) dt} (geometric sums)
 # ------------------------------------------------------------------------------------------------

@@ -105,7 +105,12 @@ int fdtd_load_fields(fdtd_ctx* ctx, const float* const E[3], const float* const 
  *   If ca / cb is non-NULL all three entries must be non-NULL.  (Same note as for the fields: six arrays at one
  *   stride, ca first, are fetched with one box per shell piece.)
  * db[3]: HOST array of three scalars (non-magnetic media); NULL -> {dt, dt, dt}.
- * Generator side (not the library's business): ca=(2eps-sigma dt)/(2eps+sigma dt), cb=2dt/(2eps+sigma dt). */
+ * Generator side (not the library's business): ca=(2eps-sigma dt)/(2eps+sigma dt), cb=2dt/(2eps+sigma dt).
+ * Contents are constants of the run: treat the arrays as frozen from this call until the next fdtd_set_coeffs /
+ * fdtd_set_coeff_lut.  On grids that run on the padded working copy (a periodic axis, or nx % 4 != 0; % 8 with binary16
+ * fields, % 16 with material indices) the library copies them once, at the first fdtd_step after this call, and does not
+ * look at the caller's arrays again; elsewhere the kernels read the caller's arrays at every launch.  A caller that
+ * edits them in place must call fdtd_set_coeffs again (same pointers) to have the edit seen on every grid. */
 int fdtd_set_coeffs(fdtd_ctx* ctx, const float* const ca[3], const float* const cb[3], const float db[3]);
 
 /* Compressed coefficients for grids of few materials (row f2; the structural fields "double the number of

@@ -5,11 +5,13 @@
 // memory; per-tile acquire/release flags on the seven upwind neighbours).  How a B200 SM
 // executes it:
 //
-//   * box 32 x 16 x 8 cells (tile 31 x 15 x 7).  Compute thread (lane, warp w) owns the x slot gx mod 32 and the TWO
-//     y slots 2w, 2w+1 (gy mod 16) and keeps both 8-cell z columns of all six field components in REGISTERS
-//     (102 registers); the slide in x/y is modular addressing, the slide in z a register renaming inside the
-//     unrolled z march.  Neighbours: z = registers, x = warp shuffle, y = the thread's other row for half of the
-//     links and a shared-memory exchange row (written by the neighbouring warp) for the other half.
+//   * box 32 x 16 x 8 cells (tile 31 x 15 x 7), 640 threads: 16 compute warps (warps 0-15) and 4 auxiliary warps
+//     (16-19).  Compute thread (lane, warp w) owns the x slot gx mod 32 and the ONE y slot w (gy mod 16) and keeps the
+//     8-cell z column of all six field components in REGISTERS (FDTD_NROW = 1: 104 registers per compute thread, 64 per
+//     auxiliary thread via setmaxnreg); the slide in x/y is modular addressing, the slide in z a register renaming
+//     inside the unrolled z march.  Neighbours: z = registers, x = warp shuffle, y = a shared-memory exchange row
+//     written by the neighbouring warp.  (FDTD_NROW = 2, two rows per thread and 8 compute warps, is a rejected
+//     experiment that still compiles; FDTD_BY = 8 is the 31x7x7 build with two CTAs per SM.)
 //   * the (ca, cb) pair of every resident cell and component sits in a thread-private shared-memory slot and is read
 //     with one 64-bit load.
 //   * the compute warps execute NO per-cell predicate: walls and the outside of the domain are data.  Cells
@@ -19,29 +21,33 @@
 //   * the minus shell of every step is fetched by TMA (cp.async.bulk.tensor, three boxes per array or -- when the
 //     component arrays sit at a uniform stride -- per group of arrays: a z plane 36x16x1, a y row 36x1x8, an x column
 //     4x16x7, each starting on a 16-byte boundary in x) into shared-memory staging, completing on mbarriers;
-//     auxiliary warps poll the upwind flags, issue the copies one step ahead of the compute warps, scatter the
-//     entering row/column coefficients into the owner threads' private shared-memory slots and repack the x column
-//     so that its single owner lane absorbs it with 16-byte loads.
-//   * every hand-off inside the CTA is an mbarrier with one elected arrive per warp; the only CTA-wide barrier is the
-//     256-thread named barrier between absorb and phase.
+//     auxiliary warps poll the upwind flags, issue the copies one step ahead of the compute warps and repack the x
+//     column so that its single owner lane absorbs it with 16-byte loads.  The coefficient shell is copied by an
+//     auxiliary warp too, but scattered into the owner threads' private slots by the compute warps (one row or column
+//     piece per warp) after E phase k, a whole step before E phase k+1 reads it.
+//   * every hand-off inside the CTA is an mbarrier with one elected arrive per warp; the only CTA-wide barriers are the
+//     two 512-thread named barriers of a step (exchange rows of H visible before the E phase, of E before the H phase).
 //   * ONE gpu-scope fence per step: the signal warp copies the leaving x columns of E and of H out of shared memory
 //     (acknowledging each at once, so the compute warps never wait for the fence), stores them, fences, and raises
 //     flagE and flagH together.
-//   * tiles are claimed in wavefront order (bx+by+bz) and skip the steps at which their region lies outside the grid.
+//   * tiles are claimed in wavefront order (bx+by+bz) and skip the steps at which their region lies outside the grid;
+//     consecutive launches of one tile grid overlap (griddepcontrol + the pred_final wait in next_tile).
 //
-//   compute (warps 0-7)          warp 8: field H shell       warp 9: coefficient shell    warp 10: field E shell     warp 11: flags
+//   compute (warps 0-15)         warp 16: field H shell      warp 17: coefficient shell   warp 18: field E shell     warp 19: flags
 //   --------------------         ------------------------    -------------------------    -----------------------    ---------------
 //   wait HREADY(k), absorb H     poll flagH[u] >= base+k     wait CFREE(k-1)              poll flagE[u] >= base+k+1
 //     -> HFREE                   fence.proxy.async           TMA coefficient shell k      fence.proxy.async
-//   E phase k                    wait HFREE(k-1)             wait EDONE(k-1), landed      wait EFREE(k-1)
-//   wait CREADY(k), absorb       TMA H shell k               scatter row + column         TMA E shell k, landed
-//     coefficient plane -> CFREE wait landed, pack x column  -> CREADY(k)                 pack x column
-//   wait ACKE(k-1), publish E    -> HREADY(k)                                             wait HDONE(k-1)            wait EDONE(k): x column
-//     -> EDONE                                                                            write E exchange column      -> registers -> ACKE
-//   wait EREADY(k), absorb E                                                              -> EREADY(k)               wait HDONE(k): x column
-//     -> EFREE                                                                                                         -> registers -> ACKH
-//   H phase k                                                                                                        store both columns, fence,
-//   wait ACKH(k-1), publish H -> HDONE                                                                                 flagE = flagH = base+k+1
+//   barrier (512)                wait HFREE(k-1)               -> CFULL(k) on landing     wait EFREE(k-1)
+//   E phase k, source, monitor   TMA H shell k                                            TMA E shell k, landed
+//   wait ACKE(k-1), publish E    wait landed, pack x column                               pack x column
+//     -> EDONE                   -> HREADY(k)                                             wait HDONE(k-1)            wait EDONE(k): x column
+//   wait EREADY(k), absorb E                                                              write E exchange column      -> registers -> ACKE
+//     -> EFREE                                                                            -> EREADY(k)               wait HDONE(k): x column
+//   barrier (512)                                                                                                      -> registers -> ACKH
+//   wait CFULL(k), scatter the                                                                                       store both columns, fence,
+//     coefficient shell -> CFREE                                                                                       flagE = flagH = base+k+1
+//   H phase k, monitor
+//   wait ACKH(k-1), publish H -> HDONE
 //
 // Per-cell arithmetic is yee_update.h, unchanged: with -fmad=false the result is bit-identical to the oracle.
 // Scope: every axis is a wall axis of the (possibly padded) grid and nx % 4 == 0 (TMA strides are

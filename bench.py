@@ -177,8 +177,22 @@ def cpu_baseline(w_full, config_steps, budget_s=12.0):
     t0 = time.perf_counter()
     orc.step(n)
     dt = time.perf_counter() - t0
-    return {"value": w.cells * n / dt / 1e12, "unit": "TCUPS", "cores": orc.nthreads, "kind": "oracle",
-            "sample": f"{what}, {n} of the config's {config_steps} time steps (after 4 warm-up steps)"}
+    out = {"value": w.cells * n / dt / 1e12, "unit": "TCUPS", "cores": orc.nthreads, "kind": "oracle",
+           "sample": f"{what}, {n} of the config's {config_steps} time steps (after 4 warm-up steps)",
+           # the CPU number belongs to sample_grid; any ratio against the GPU's full-grid value extrapolates it
+           "sample_grid": list(w.n), "full_grid": list(w_full.n), "extrapolated": tuple(w.n) != tuple(w_full.n)}
+    if w.fields == "zero":
+        # The config starts from zero fields: as the pulse spreads, its front is a shell of subnormal values, which the
+        # host cores handle slowly.  The same sample with seeded random fields (every value normal) times the oracle's
+        # arithmetic without that effect.
+        del orc
+        orc = make_oracle(replace(w, fields="uniform"))
+        orc.step(2)
+        n2 = max(2, n // 2)
+        t0 = time.perf_counter()
+        orc.step(n2)
+        out["value_random_fields"] = w.cells * n2 / (time.perf_counter() - t0) / 1e12
+    return out
 
 
 def run_reference(args):
@@ -341,6 +355,62 @@ def run_sweep(variant, dev, peak_gbs, counters, headline, skip_name):
     return rows
 
 
+def feature_rows(variant, dev, peak_gbs):
+    """Rows f3 and f4 of SURVEY.md 8(f) measured (performance "does indeed depend on ... the output volume"):
+    the absorber-coefficient generator against its 36 B/cell HBM roof (three permittivity arrays read, six coefficient
+    arrays written), and config 2 with one running-DFT monitor plane switched on, as overhead against the plain run."""
+    import numpy as np
+    import torch
+    from paper_2502_20610_b200 import binding, workloads
+    rows = []
+    # f3: fdtd_absorber_coeffs on 512^3, 12-cell layers on all six faces
+    n = (512, 512, 512)
+    shape = (n[2], n[1], n[0])
+    eps = [torch.full(shape, 2.1, dtype=torch.float32, device=dev) for _ in range(3)]
+    ca = [torch.empty(shape, dtype=torch.float32, device=dev) for _ in range(3)]
+    cb = [torch.empty(shape, dtype=torch.float32, device=dev) for _ in range(3)]
+    call = lambda: binding.absorber_coeffs(n, 0.25, eps, (12,) * 6, (0.4,) * 6, 3, ca, cb, variant=variant)
+    for _ in range(3):
+        call()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(10):
+        call()
+    ev1.record()
+    torch.cuda.synchronize()
+    gbs = 36.0 * n[0] * n[1] * n[2] * 10 / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
+    rows.append({"feature": "f3 fdtd_absorber_coeffs", "grid": list(n), "bytes_per_cell": 36.0, "achieved_gbs": gbs, "peak_gbs": peak_gbs,
+                 "frac": gbs / peak_gbs, "launches": 10})
+    del eps, ca, cb
+    torch.cuda.empty_cache()
+    # f4: config 2, systolic kernel, one z-plane monitor with 4 frequencies
+    w0 = workloads.config(1)
+    S, K, W = 200, 3, 2
+    w = replace(w0, steps=(K + W) * S + 1)
+    tc = {}
+    for mon in (False, True):
+        sim, keep = setup_case(w, "systolic", variant, dev)
+        if mon:
+            F, nt = 4, (K + W) * S
+            tt = np.arange(nt)[:, None]
+            om = 2 * np.pi * (0.02 + 0.01 * np.arange(F))[None, :]
+            wE = np.stack([np.cos(om * (tt + 1) * w.dt), -np.sin(om * (tt + 1) * w.dt)], axis=2).astype(np.float32)
+            wH = np.stack([np.cos(om * (tt + 1.5) * w.dt), -np.sin(om * (tt + 1.5) * w.dt)], axis=2).astype(np.float32)
+            acc = torch.zeros((6, F, 2, w.n[0] * w.n[1]), dtype=torch.float32, device=dev)
+            sim.set_monitor(2, w.n[2] // 2, wE, wH, acc)
+        ms, _ = time_case(sim, S, K, W)
+        tc[mon] = w.cells * S * K / (ms * 1e-3) / 1e12
+        if mon:
+            assert float(acc.abs().max()) > 0.0
+        sim.close()
+        del sim, keep
+        torch.cuda.empty_cache()
+    rows.append({"feature": "f4 running-DFT monitor, one z plane, 4 frequencies", "workload": w0.name, "grid": list(w0.n), "plain_tcups": tc[False],
+                 "monitor_tcups": tc[True], "overhead_pct": 100.0 * (tc[False] / tc[True] - 1.0)})
+    return rows
+
+
 def e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier):
     """The same metric end to end through the C ABI with HOST buffers (copies inside the timed region).  A function of its
     own so that its device and pinned buffers die with it."""
@@ -379,7 +449,9 @@ def e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier):
         job[0].step(S)
 
     def collect(job):
-        job[0].get_fields(Eout, Hout)        # waits for the job's steps, then enqueues the copies out
+        # fdtd_get_fields waits for the job's steps, enqueues the six copies out and returns only when they have landed, so
+        # the copies of two jobs into the shared pinned Eout / Hout never overlap in time (each collect overwrites the last)
+        job[0].get_fields(Eout, Hout)
 
     def run(n):
         nj = len(jobs)
@@ -391,6 +463,7 @@ def e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier):
                 submit(jobs[i % nj])                     # its next inputs follow on the same stream
         for job in jobs:
             job[0].sync()
+    ke1 = ke
     ke = 2 * ke if len(jobs) > 1 else ke
     run(2)
     barrier()
@@ -398,8 +471,43 @@ def e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier):
     run(ke)
     barrier()
     dt = max_over_ranks(dist, time.perf_counter() - t0, dev)
+    # one simulation at a time (what a single caller sees): copy in, S steps, copy out, strictly one after the other
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke1):
+        submit(jobs[0])
+        collect(jobs[0])
+    barrier()
+    dt1 = max_over_ranks(dist, time.perf_counter() - t0, dev)
+    # The host path is checked once: the arrays job 0 just delivered to the host against a device-resident run of the same
+    # S steps from the same initial state (generated on the device, never through the host), bit for bit.
+    ref = jobs[-1]
+    if w.fields == "zero":
+        for a in ref[2] + ref[3]:
+            a.zero_()
+    else:
+        Ed, Hd = workloads.make_fields(w, device=dev)
+        for dst, src in zip(ref[2] + ref[3], Ed + Hd):
+            dst.copy_(src.to(fdtype))
+        del Ed, Hd
+    if len(jobs) == 1:
+        host = [t.clone() for t in Eout + Hout]          # job 0's arrays are about to be reused
+    else:
+        host = Eout + Hout
+    torch.cuda.synchronize()
+    ref[0].set_time(0)
+    ref[0].step(S)
+    ref[0].sync()
+    verified = True
+    for hst, d in zip(host, ref[2] + ref[3]):
+        verified = verified and bool(torch.equal(hst.to(dev), d))
+    if not verified:
+        raise SystemExit("bench.py: the end-to-end leg's host output differs from the device-resident run")
+    del host
     e2e = {"value": job_tcups(world, w.cells * S * ke, dt), "unit": "TCUPS", "h2d_bytes_per_step": nbytes,
-           "d2h_bytes_per_step": nbytes, "steps": ke, "jobs_in_flight": len(jobs),
+           "d2h_bytes_per_step": nbytes, "steps": ke, "jobs_in_flight": len(jobs), "ranks": world,
+           "single_job": {"value": job_tcups(world, w.cells * S * ke1, dt1), "unit": "TCUPS", "steps": ke1},
+           "verified": "host output of one job == device-resident run of the same steps, bit for bit",
            "note": "per bench step: six field arrays pinned host->device, S time steps, six arrays device->pinned host, all "
                    "through the C ABI; two independent jobs in flight on two streams (copies of one overlap the steps of the "
                    "other); the coefficient arrays are problem constants bound once"}
@@ -466,7 +574,18 @@ def main():
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     e2e = None
     if not args.no_e2e:
-        e2e = e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier)
+        # every rank pins two host copies of the six field arrays (config 5: 87 GB); N replicas do that N times.  Where
+        # the host cannot hold it, rank 0 alone runs the leg (one replica's end-to-end rate, "ranks": 1).
+        import psutil
+        pinned = 2 * 6 * w.cells * (2 if args.storage == "f16" else 4)
+        if world > 1 and world * pinned > 0.6 * psutil.virtual_memory().total:
+            if rank == 0:
+                e2e = e2e_leg(args, w, sim, keep, tile, S, K, dev, None, 1, torch.cuda.synchronize)
+                e2e["ranks"] = 1
+                e2e["note"] += "; measured on rank 0 only: %d replicas would pin %.0f GB of host memory" % (world, world * pinned / 1e9)
+            barrier()
+        else:
+            e2e = e2e_leg(args, w, sim, keep, tile, S, K, dev, dist, world, barrier)
         torch.cuda.empty_cache()
 
     if rank != 0:
@@ -506,7 +625,7 @@ def main():
             "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "field_storage": args.storage, "coefficients": (args.coeffs if has_coef else "uniform"), "grid": list(w.n), "time_steps_per_bench_step": S, "kernel": args.kernel,
-                       "tile": list(info["tile"]), "T": info["T"], "tiles_per_launch": info["tiles"], "ctas": info["ctas"],
+                       "tile": list(info["tile"]), "T": r["T_launched"] if args.kernel == "systolic" else 0, "T_library": info["T"], "tiles_per_launch": info["tiles"], "ctas": info["ctas"],
                        "smem_per_cta": info["smem"], "variant": args.variant, "parallelism": "replicas" if world > 1 else "single",
                        "l2": "inputs exceed L2 (%.0f MB of fields+coefficients vs 126 MB)" % (ws / 1e6) if ws > 200e6
                              else "inputs fit L2 (no flush): below-L2 point of the size sweep"},
@@ -538,6 +657,7 @@ def main():
         del nsim, nkeep
         torch.cuda.empty_cache()
         line["sweep"] = run_sweep(args.variant, dev, peak, counters, headline_row, w.name)
+        line["features"] = feature_rows(args.variant, dev, peak)
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -11,6 +11,8 @@
 //   low layer of L cells:  u = (L - s)/L where s < L;   high layer:  u = (s - (n - L))/L where s > n - L
 //   sigma_q = smax * u^p;  sigma = (sigma_x + sigma_y) + sigma_z
 //   ca = (2 eps - sigma dt)/(2 eps + sigma dt),  cb = (2 dt)/(2 eps + sigma dt)
+#include <stdint.h>
+
 #include "fdtd_internal.h"
 
 namespace {
@@ -80,6 +82,61 @@ __global__ void __launch_bounds__(256) absorber_kernel(const __grid_constant__ A
     }
 }
 
+// The same arithmetic, four consecutive cells of a row per thread: 128-bit loads and stores, one index decomposition per
+// group instead of one per cell (the one-cell kernel above spends more issue slots on 64-bit divisions than on the
+// formula and reaches 0.31 of the 36 B/cell HBM roof).  Needs nx % 4 == 0 and 16-byte aligned arrays; every value is
+// produced by the same sequence of rounded operations, so the output is bit-identical.
+template <typename index_t>
+__global__ void __launch_bounds__(256) absorber_kernel_x4(const __grid_constant__ AbsorberParams p)
+{
+    const int G = p.n[0] >> 2;                                     // groups per row
+    const index_t groups = (index_t)G * p.n[1] * p.n[2];
+    const float dt2 = 2.0f * p.dt;
+    for (index_t q = blockIdx.x * (index_t)256 + threadIdx.x; q < groups; q += (index_t)256 * gridDim.x) {
+        const index_t row = q / G;
+        const int i0 = (int)(q - row * G) << 2;
+        const int k = (int)(row / p.n[1]);
+        const int j = (int)(row - (index_t)k * p.n[1]);
+        const long long idx = (long long)q << 2;
+        float sx[2][4] = {{0.0f, 0.0f, 0.0f, 0.0f}, {0.0f, 0.0f, 0.0f, 0.0f}};       // [own][cell]
+        // a low layer of L cells reaches cells g < L, a high one cells g >= n - L (either Yee offset): most groups lie in
+        // neither and keep the 0 that layer_sigma would return
+        if (i0 < p.L[0] || i0 + 3 >= p.n[0] - p.L[1]) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                sx[0][c] = layer_sigma(p, 0, i0 + c, false);
+                sx[1][c] = layer_sigma(p, 0, i0 + c, true);
+            }
+        }
+        const float sy[2] = {layer_sigma(p, 1, j, false), layer_sigma(p, 1, j, true)};
+        const float sz[2] = {layer_sigma(p, 2, k, false), layer_sigma(p, 2, k, true)};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float e[4] = {1.0f, 1.0f, 1.0f, 1.0f};
+            if (p.eps[a]) {
+                const float4 v = __ldcs(reinterpret_cast<const float4*>(p.eps[a] + idx));
+                e[0] = v.x; e[1] = v.y; e[2] = v.z; e[3] = v.w;
+            }
+            float ca[4], cb[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float sxy = sx[a == 0][c] + sy[a == 1];
+                const float sig = sxy + sz[a == 2];
+                const float e2 = 2.0f * e[c];
+                const float sd = sig * p.dt;
+                const float den = e2 + sd;
+                const float num = e2 - sd;
+                ca[c] = num / den;
+                cb[c] = dt2 / den;
+            }
+            __stcs(reinterpret_cast<float4*>(p.ca[a] + idx), make_float4(ca[0], ca[1], ca[2], ca[3]));
+            __stcs(reinterpret_cast<float4*>(p.cb[a] + idx), make_float4(cb[0], cb[1], cb[2], cb[3]));
+        }
+    }
+}
+
+bool aligned16(const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15u) == 0; }
+
 }  // namespace
 
 cudaError_t launch_absorber(const int n[3], float dt, const float* const eps[3], const int L[6], const float smax[6], int order,
@@ -99,8 +156,13 @@ cudaError_t launch_absorber(const int n[3], float dt, const float* const eps[3],
     p.order = order;
     p.dt = dt;
     const long long cells = (long long)n[0] * n[1] * n[2];
-    long long blocks = (cells + 255) / 256;
+    bool x4 = n[0] % 4 == 0;
+    for (int a = 0; a < 3; ++a) x4 = x4 && aligned16(p.eps[a]) && aligned16(p.ca[a]) && aligned16(p.cb[a]);
+    const long long work = x4 ? cells / 4 : cells;
+    long long blocks = (work + 255) / 256;
     if (blocks > 148ll * 32) blocks = 148ll * 32;      // grid-stride: a multiple of the SM count
-    absorber_kernel<<<(unsigned)blocks, 256, 0, st>>>(p);
+    if (!x4) absorber_kernel<<<(unsigned)blocks, 256, 0, st>>>(p);
+    else if (work + 148ll * 32 * 256 < (1ll << 31)) absorber_kernel_x4<unsigned int><<<(unsigned)blocks, 256, 0, st>>>(p);
+    else absorber_kernel_x4<unsigned long long><<<(unsigned)blocks, 256, 0, st>>>(p);
     return cudaGetLastError();
 }

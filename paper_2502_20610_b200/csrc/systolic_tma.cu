@@ -587,26 +587,40 @@ __shared__ unsigned trace_cur_;
 // tile; successive steps of a cell are ordered by program order inside a tile and by the flag hand-off between tiles (the
 // read-modify-write below is issued before the warp arrives on the DONE barrier that the signal warp's fence covers, and
 // goes through L2).  Rare path: the caller tests the CTA-uniform conditions first.
-template <int NV>
-__device__ __forceinline__ void monitor_add(const MonitorParams& m, const float* w, int base, int gx, int gy, int gz, const float (&v)[NV][3])
+// Kept small on purpose.  The path is rare (only tile steps whose region the plane cuts), but how it is written decides the
+// speed of EVERY step of the instantiation: unrolled over the seven planes it doubled the step loop (11.7k instead of 5.4k
+// instructions), and as a non-inlined call it made ptxas spill loop-carried values inside the step loop; both ran config 2
+// 22-28 % slower even on steps that never take it.  Here: a run-time loop over the planes, the plane's three values picked
+// from the register columns by a select chain, and per frequency six accumulator loads in flight, then six stores.
+// ax, ay, az: the thread's register columns; plane gz0 + l holds a?[OFF + l].
+template <int OFF, int NA>
+__device__ __forceinline__ void monitor_add(const MonitorParams& m, const float* w, int base, int gx, int gy, int gz0,
+                                            const float (&ax)[NA], const float (&ay)[NA], const float (&az)[NA])
 {
-    // v[l] = the three components at plane gz + l
-#pragma unroll
-    for (int l = 0; l < NV; ++l) {
-        const long long cell = m.cell(gx, gy, gz + l);
+    static_assert(OFF + W2 <= NA, "register column too short");
+    const long long ps = m.pcells, fs = 2 * ps, cs = fs * m.F;       // strides: re -> im, frequency, component
+#pragma unroll 1
+    for (int l = 0; l < W2; ++l) {
+        const long long cell = m.cell(gx, gy, gz0 + l);
         if (cell < 0) continue;
-        float* acc = m.acc + ((long long)base * m.F * 2) * m.pcells + cell;
-        for (int f = 0; f < m.F; ++f) {
-            const float wr = __ldg(w + 2 * f), wi = __ldg(w + 2 * f + 1);
+        float vx = ax[OFF], vy = ay[OFF], vz = az[OFF];
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                float* pr = acc + ((long long)(c * m.F + f) * 2) * m.pcells;
-                float* pi = pr + m.pcells;
-                const float qr = v[l][c] * wr;
-                const float qi = v[l][c] * wi;
-                __stcg(pr, __ldcg(pr) + qr);
-                __stcg(pi, __ldcg(pi) + qi);
-            }
+        for (int q = 1; q < W2; ++q)
+            if (l == q) { vx = ax[OFF + q]; vy = ay[OFF + q]; vz = az[OFF + q]; }
+        float* p0 = m.acc + (long long)base * cs + cell;
+#pragma unroll 1
+        for (int f = 0; f < m.F; ++f, p0 += fs) {
+            const float wr = __ldg(w + 2 * f), wi = __ldg(w + 2 * f + 1);
+            const float xr = __ldcg(p0), xi = __ldcg(p0 + ps);
+            const float yr = __ldcg(p0 + cs), yi = __ldcg(p0 + cs + ps);
+            const float zr = __ldcg(p0 + 2 * cs), zi = __ldcg(p0 + 2 * cs + ps);
+            const float qxr = vx * wr, qxi = vx * wi, qyr = vy * wr, qyi = vy * wi, qzr = vz * wr, qzi = vz * wi;
+            __stcg(p0, xr + qxr);
+            __stcg(p0 + ps, xi + qxi);
+            __stcg(p0 + cs, yr + qyr);
+            __stcg(p0 + cs + ps, yi + qyi);
+            __stcg(p0 + 2 * cs, zr + qzr);
+            __stcg(p0 + 2 * cs + ps, zi + qzi);
         }
     }
 }
@@ -849,10 +863,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 if ((lx >= 1) & (ly[r] >= 1) && col_in[r]) {
-                    float v[W2][3];
-#pragma unroll
-                    for (int l = 1; l < BZ; ++l) { v[l - 1][0] = ex[r][l + 1]; v[l - 1][1] = ey[r][l + 1]; v[l - 1][2] = ez[r][l + 1]; }
-                    monitor_add<W2>(P.mon, P.mon.wE + (P.t0 + k) * P.mon.F * 2, 0, gx, gy[r], o2 + 1, v);
+                    // planes o2 + 1 + l, l = 0..6, hold e?[r][l + 2]
+                    monitor_add<2>(P.mon, P.mon.wE + (P.t0 + k) * P.mon.F * 2, 0, gx, gy[r], o2 + 1, ex[r], ey[r], ez[r]);
                 }
             }
         }
@@ -992,10 +1004,8 @@ __device__ __forceinline__ void compute_tile(const SysParams& P, const TileGeom&
 #pragma unroll
             for (int r = 0; r < NROW; ++r) {
                 if ((lx <= W0 - 1) & (ly[r] <= W1 - 1) && col_in[r]) {
-                    float v[W2][3];
-#pragma unroll
-                    for (int l = 0; l < BZ - 1; ++l) { v[l][0] = hx[r][l + 1]; v[l][1] = hy[r][l + 1]; v[l][2] = hz[r][l + 1]; }
-                    monitor_add<W2>(P.mon, P.mon.wH + (P.t0 + k) * P.mon.F * 2, 3, gx, gy[r], o2, v);
+                    // planes o2 + l, l = 0..6, hold h?[r][l + 1]
+                    monitor_add<1>(P.mon, P.mon.wH + (P.t0 + k) * P.mon.F * 2, 3, gx, gy[r], o2, hx[r], hy[r], hz[r]);
                 }
             }
         }

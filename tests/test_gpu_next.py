@@ -47,6 +47,8 @@ ABSORBER_CASES = [
     ((64, 8, 8), 0.31, True, (32, 32, 0, 0, 0, 0), (0.25, 0.3, 0, 0, 0, 0), 1),       # the two layers of an axis meet
     ((16, 16, 16), 0.1, True, (3, 3, 3, 3, 3, 3), (0.5,) * 6, 0),                    # order 0: uniform inside the layer
     ((130, 70, 33), 0.2, True, (20, 20, 10, 10, 8, 8), (0.05,) * 6, 4),
+    ((48, 20, 12), 0.27, False, (5, 6, 7, 4, 3, 2), (0.3, 0.2, 0.1, 0.25, 0.15, 0.35), 2),   # four-cells-per-thread kernel without eps arrays
+    ((256, 96, 40), 0.22, True, (12, 12, 12, 12, 12, 12), (0.4,) * 6, 3),                     # many groups per row, several blocks per thread
 ]
 
 
@@ -66,6 +68,28 @@ def test_absorber_generator_bit_exact(cuda_device, n, dt, with_eps, thickness, s
     for a in range(3):
         assert np.array_equal(ca[a].cpu().numpy(), want_ca[a]), f"ca[{a}] differs"
         assert np.array_equal(cb[a].cpu().numpy(), want_cb[a]), f"cb[{a}] differs"
+
+
+def test_absorber_generator_unaligned_arrays_take_the_one_cell_kernel(cuda_device):
+    """nx % 4 == 0 but the output arrays start 4 bytes off a 16-byte boundary: the vector kernel does not apply, the
+    result is the same."""
+    import torch
+    n, dt, thickness, smax, order = (32, 12, 10), 0.3, (4, 5, 3, 2, 4, 3), (0.2, 0.3, 0.1, 0.4, 0.25, 0.15), 2
+    shape = (n[2], n[1], n[0])
+    cells = n[0] * n[1] * n[2]
+    eps = [np.random.default_rng(5 + a).uniform(1.0, 12.1, shape).astype(np.float32) for a in range(3)]
+    want_ca, want_cb = absorber_coeffs(n, np.float32(dt), eps, thickness, smax, order, np.float32)
+    dev = torch.device("cuda:0")
+    eps_d = [torch.from_numpy(e).to(dev) for e in eps]
+    block = torch.full((6 * (cells + 4),), -7.0, dtype=torch.float32, device=dev)
+    outs = [block[q * (cells + 4) + 1: q * (cells + 4) + 1 + cells].view(shape) for q in range(6)]
+    assert all(t.data_ptr() % 16 == 4 for t in outs)
+    binding.absorber_coeffs(n, dt, eps_d, thickness, smax, order, outs[:3], outs[3:])
+    torch.cuda.synchronize()
+    for a in range(3):
+        assert np.array_equal(outs[a].cpu().numpy(), want_ca[a]) and np.array_equal(outs[3 + a].cpu().numpy(), want_cb[a])
+    guard = block.view(6, cells + 4)
+    assert bool((guard[:, 0] == -7.0).all()) and bool((guard[:, cells + 1:] == -7.0).all())     # nothing written outside the arrays
 
 
 def test_absorber_rejects_bad_arguments(cuda_device):
